@@ -1,0 +1,254 @@
+"""CPU oracle (TEST INFRASTRUCTURE): ctypes wrapper around oracle/oracle.c.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  It imports nothing from paper_2606_01547_b200.
+
+Definitions: SURVEY.md §8(c) G, E, S, H, T, R, B, P, following PAPER.md:55 (three steps)
+and the profile names of PAPER.md:80, :85, :87, :103.  All arithmetic is float64 in
+oracle.c; this file only marshals numpy arrays.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.c")
+_LIB_PATH = os.path.join(_HERE, "liboracle.so")
+_lib = None
+
+_d = ctypes.c_double
+_i = ctypes.c_int
+_i64 = ctypes.c_int64
+_dp = ctypes.POINTER(ctypes.c_double)
+
+
+def build(force=False):
+    """Compile oracle.c -> liboracle.so with gcc (-O2, no fast-math; OpenMP on the outer loops only)."""
+    if (not force and os.path.exists(_LIB_PATH)
+            and os.path.getmtime(_LIB_PATH) >= os.path.getmtime(_SRC)):
+        return _LIB_PATH
+    cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+           "-o", _LIB_PATH, _SRC, "-lm"]
+    subprocess.run(cmd, check=True)
+    return _LIB_PATH
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(_dp)
+
+
+def _arr(a, shape=None):
+    if a is None:
+        return None
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if shape is not None:
+        a = a.reshape(shape)
+    return a
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB_PATH)
+        L.orc_set_threads.argtypes = [_i]
+        L.orc_get_max_threads.restype = _i
+        L.orc_grid.argtypes = [_i, _i, _d, _d, _d, _i, _dp, _dp]
+        L.orc_ellipticity.argtypes = [_d, _d, _dp, _dp]
+        L.orc_sie_alpha.argtypes = [_d, _d, _dp, _dp, _dp]
+        L.orc_sie_kappa.argtypes = [_d, _d, _dp]
+        L.orc_sie_kappa.restype = _d
+        L.orc_shear_alpha.argtypes = [_d, _d, _d, _d, _dp, _dp]
+        L.orc_pointmass_alpha.argtypes = [_d, _d, _d, _d, _d, _dp, _dp]
+        for name in ("orc_tnfw_F",):
+            getattr(L, name).argtypes = [_d]
+            getattr(L, name).restype = _d
+        for name in ("orc_tnfw_L", "orc_tnfw_g", "orc_tnfw_g_closed", "orc_tnfw_g_series"):
+            getattr(L, name).argtypes = [_d, _d]
+            getattr(L, name).restype = _d
+        L.orc_tnfw_alpha.argtypes = [_d, _d, _d, _d, _d, _d, _d, _dp, _dp]
+        L.orc_tnfw_kappa.argtypes = [_d] * 7
+        L.orc_tnfw_kappa.restype = _d
+        L.orc_ray_shoot.argtypes = [_i64, _dp, _dp, _dp, _dp, _i64, _dp, _dp, _dp]
+        L.orc_sersic.argtypes = [_d, _d, _dp]
+        L.orc_sersic.restype = _d
+        L.orc_source_brightness.argtypes = [_i64, _dp, _dp, _i, _dp, _dp]
+        L.orc_bin.argtypes = [_i, _i, _i, _d, _dp, _dp]
+        L.orc_convolve.argtypes = [_i, _i, _dp, _i, _i, _dp, _dp]
+        L.orc_prepsf_rows.argtypes = [_i, _i, _d, _d, _d, _i, _dp, _dp, _i64, _dp, _i, _dp, _i, _i, _dp]
+        L.orc_simulate_image.argtypes = [_i, _i, _d, _d, _d, _i, _dp, _dp, _i64, _dp, _i, _dp,
+                                         _i, _i, _dp, _dp, _dp]
+        L.orc_simulate_batch.argtypes = [_i64, _i, _i, _d, _d, _d, _i, _dp, _dp, _i64, _dp, _i, _dp,
+                                         _i, _i, _dp, _dp]
+        _lib = L
+    return _lib
+
+
+def set_threads(n):
+    lib().orc_set_threads(int(n))
+
+
+def max_threads():
+    return int(lib().orc_get_max_threads())
+
+
+# ----------------------------------------------------------------- scalar functions
+def ellipticity(e1, e2):
+    phi, q = _d(), _d()
+    lib().orc_ellipticity(e1, e2, ctypes.byref(phi), ctypes.byref(q))
+    return phi.value, q.value
+
+
+def sie_alpha(x, y, theta_E, e1, e2, cx=0.0, cy=0.0):
+    p = (_d * 5)(theta_E, e1, e2, cx, cy)
+    ax, ay = _d(), _d()
+    lib().orc_sie_alpha(x, y, p, ctypes.byref(ax), ctypes.byref(ay))
+    return ax.value, ay.value
+
+
+def sie_kappa(x, y, theta_E, e1, e2, cx=0.0, cy=0.0):
+    p = (_d * 5)(theta_E, e1, e2, cx, cy)
+    return lib().orc_sie_kappa(x, y, p)
+
+
+def shear_alpha(x, y, g1, g2):
+    ax, ay = _d(), _d()
+    lib().orc_shear_alpha(x, y, g1, g2, ctypes.byref(ax), ctypes.byref(ay))
+    return ax.value, ay.value
+
+
+def pointmass_alpha(x, y, theta_E, cx=0.0, cy=0.0):
+    ax, ay = _d(), _d()
+    lib().orc_pointmass_alpha(x, y, theta_E, cx, cy, ctypes.byref(ax), ctypes.byref(ay))
+    return ax.value, ay.value
+
+
+def tnfw_F(X):
+    return lib().orc_tnfw_F(X)
+
+
+def tnfw_L(X, tau):
+    return lib().orc_tnfw_L(X, tau)
+
+
+def tnfw_g(X, tau):
+    return lib().orc_tnfw_g(X, tau)
+
+
+def tnfw_g_closed(X, tau):
+    return lib().orc_tnfw_g_closed(X, tau)
+
+
+def tnfw_g_series(X, tau):
+    return lib().orc_tnfw_g_series(X, tau)
+
+
+def tnfw_alpha(x, y, cx, cy, Rs, alpha_Rs, r_trunc):
+    ax, ay = _d(), _d()
+    lib().orc_tnfw_alpha(x, y, cx, cy, Rs, alpha_Rs, r_trunc, ctypes.byref(ax), ctypes.byref(ay))
+    return ax.value, ay.value
+
+
+def tnfw_kappa(x, y, cx, cy, Rs, alpha_Rs, r_trunc):
+    return lib().orc_tnfw_kappa(x, y, cx, cy, Rs, alpha_Rs, r_trunc)
+
+
+def sersic(x, y, amp, R_sersic, n_sersic, e1, e2, cx, cy):
+    p = (_d * 7)(amp, R_sersic, n_sersic, e1, e2, cx, cy)
+    return lib().orc_sersic(x, y, p)
+
+
+# ----------------------------------------------------------------- array functions
+def grid(nx, ny, pixel_scale, cx=0.0, cy=0.0, supersample=1):
+    n = nx * supersample * ny * supersample
+    tx = np.empty(n)
+    ty = np.empty(n)
+    lib().orc_grid(nx, ny, pixel_scale, cx, cy, supersample, _ptr(tx), _ptr(ty))
+    return tx, ty
+
+
+def _lens_args(sie, shear, tnfw):
+    sie = _arr(sie)
+    shear = _arr(shear)
+    if tnfw is None:
+        tnfw = np.zeros((5, 0))
+    tnfw = _arr(tnfw)
+    assert tnfw.ndim == 2 and tnfw.shape[0] == 5
+    return sie, shear, tnfw
+
+
+def ray_shoot(theta_x, theta_y, sie=None, shear=None, tnfw=None):
+    tx = _arr(theta_x).ravel()
+    ty = _arr(theta_y).ravel()
+    sie, shear, tnfw = _lens_args(sie, shear, tnfw)
+    bx = np.empty_like(tx)
+    by = np.empty_like(ty)
+    lib().orc_ray_shoot(tx.size, _ptr(tx), _ptr(ty), _ptr(sie), _ptr(shear), tnfw.shape[1], _ptr(tnfw),
+                        _ptr(bx), _ptr(by))
+    return bx, by
+
+
+def source_brightness(beta_x, beta_y, sources):
+    bx = _arr(beta_x).ravel()
+    by = _arr(beta_y).ravel()
+    src = _arr(sources).reshape(-1, 7)
+    out = np.empty_like(bx)
+    lib().orc_source_brightness(bx.size, _ptr(bx), _ptr(by), src.shape[0], _ptr(src), _ptr(out))
+    return out
+
+
+def bin_rays(nx, ny, supersample, pixel_scale, flux):
+    f = _arr(flux).ravel()
+    assert f.size == nx * ny * supersample * supersample
+    img = np.empty((ny, nx))
+    lib().orc_bin(nx, ny, supersample, pixel_scale, _ptr(f), _ptr(img))
+    return img
+
+
+def convolve(image, kernel):
+    img = _arr(image)
+    ker = _arr(kernel)
+    out = np.empty_like(img)
+    lib().orc_convolve(img.shape[0], img.shape[1], _ptr(img), ker.shape[0], ker.shape[1], _ptr(ker), _ptr(out))
+    return out
+
+
+def prepsf_rows(w, j0=0, j1=None):
+    """Pre-PSF image rows [j0, j1) of a workloads.Workload-like object (duck-typed; no import)."""
+    j1 = w.ny if j1 is None else j1
+    sie, shear, tnfw = _lens_args(w.sie, w.shear, w.tnfw)
+    src = _arr(w.sources).reshape(-1, 7)
+    out = np.empty((j1 - j0, w.nx))
+    lib().orc_prepsf_rows(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample, _ptr(sie), _ptr(shear),
+                          tnfw.shape[1], _ptr(tnfw), src.shape[0], _ptr(src), j0, j1, _ptr(out))
+    return out
+
+
+def simulate_image(w):
+    """Whole pipeline on one system; returns (pre_psf, image)."""
+    sie, shear, tnfw = _lens_args(w.sie, w.shear, w.tnfw)
+    src = _arr(w.sources).reshape(-1, 7)
+    psf = _arr(w.psf)
+    pre = np.empty((w.ny, w.nx))
+    out = np.empty((w.ny, w.nx))
+    lib().orc_simulate_image(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample, _ptr(sie), _ptr(shear),
+                             tnfw.shape[1], _ptr(tnfw), src.shape[0], _ptr(src),
+                             psf.shape[0], psf.shape[1], _ptr(psf), _ptr(pre), _ptr(out))
+    return pre, out
+
+
+def simulate_batch(bw, systems=None):
+    """Batched pipeline; `systems` optionally selects a subset of system indices."""
+    idx = np.arange(bw.B) if systems is None else np.asarray(systems)
+    sie = _arr(bw.sie[idx])
+    shear = _arr(bw.shear[idx])
+    tnfw = _arr(bw.tnfw[idx])
+    src = _arr(bw.sources[idx])
+    psf = _arr(bw.psf[idx])
+    out = np.empty((idx.size, bw.ny, bw.nx))
+    lib().orc_simulate_batch(idx.size, bw.nx, bw.ny, bw.pixel_scale, bw.cx, bw.cy, bw.supersample,
+                             _ptr(sie), _ptr(shear), tnfw.shape[2], _ptr(tnfw), src.shape[1], _ptr(src),
+                             psf.shape[1], psf.shape[2], _ptr(psf), _ptr(out))
+    return out
