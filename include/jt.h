@@ -1,0 +1,154 @@
+/*
+ * jt.h -- C ABI of libjt: lensed-image simulation on one NVIDIA B200 (sm_100a).
+ *
+ * The hot path is the three-step image simulation of PAPER.md:55 (section "Improvements over
+ * lenstronomy in image simulation"): (1) a coordinate grid in the observer's angles is ray-traced
+ * through every deflector back to the source plane, (2) the source surface brightness is evaluated
+ * on the traced grid, (3) the lensed image is convolved with the PSF.  Where the time goes:
+ * PAPER.md:47 ("ray-tracing through tens of thousands of dark matter substructures").  Profile
+ * names: NIE/SIE PAPER.md:80, SHEAR :85, TNFW :87, SERSIC_ELLIPSE :103; FFT convolution :110-114.
+ * The paper prints no formula; the definitions used (G, E, S, H, T, R, B, P) are the readings
+ * listed in DESIGN.md "Readings of the paper".
+ *
+ * Conventions for EVERY function:
+ *   - extern "C", returns jt_status (0 = JT_OK), never throws, never exits.
+ *   - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default
+ *     stream).  No function synchronises the device; host structs are read before the call
+ *     returns, so the caller may free them immediately.
+ *   - The caller owns every buffer, workspace included.  The library allocates no device memory
+ *     and keeps no device state between calls.
+ *   - "device [n]" = pointer to device memory holding n elements of the call's dtype
+ *     (float for JT_F32, double for JT_F64), aligned to the element size.  "host" = ordinary
+ *     host memory.  Arrays are row-major, x (column) fastest.
+ *   - In/out aliasing is not allowed.  Outputs are unspecified after an error.
+ *   - JT_F32 mode: storage and the O(rays x subhalos) loop are float; the O(rays) per-ray work
+ *     (grid angle, SIE, shear, lens equation) is done in double because beta = theta - alpha
+ *     cancels near the Einstein ring.  JT_F64: everything double.
+ *   - There is no CPU fallback: on a machine without an sm_100 device every compute call returns
+ *     JT_ERR_UNSUPPORTED or JT_ERR_CUDA.
+ *
+ * Error codes: JT_ERR_INVALID_VALUE  null pointer where data is required, negative count,
+ *              nx/ny < 1, supersample < 1 or > JT_MAX_SUPERSAMPLE, pixel_scale <= 0,
+ *              even or < 1 kernel size, n_src < 0 or > JT_MAX_SOURCES, in == out;
+ *              JT_ERR_UNSUPPORTED    unknown dtype / method, device is not compute capability 10.x;
+ *              JT_ERR_WORKSPACE      workspace_bytes smaller than the matching *_workspace_bytes query
+ *                                    (or workspace NULL when the query is non-zero);
+ *              JT_ERR_CUDA           a CUDA call failed; jt_last_cuda_error() returns its cudaError_t.
+ * Parameter VALUES held in device arrays (Rs <= 0, r_trunc <= 0, NaN) are not validated:
+ * IEEE garbage in, garbage out, never a fault.  Zero-sized problems (n_rays = 0, B = 0) are no-ops.
+ * |e| >= 1 ellipticities are clamped to 0.9999 (definition E), not rejected.
+ */
+#ifndef JT_H
+#define JT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define JT_API __attribute__((visibility("default")))
+#else
+#define JT_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define JT_VERSION 100           /* 0.1.0 */
+#define JT_MAX_SUPERSAMPLE 16    /* s x s sub-rays per pixel, binned with warp shuffles */
+#define JT_MAX_SOURCES 16        /* Sersic components per system (host arrays, passed by value to kernels) */
+
+typedef enum { JT_OK = 0, JT_ERR_INVALID_VALUE = 1, JT_ERR_UNSUPPORTED = 2, JT_ERR_WORKSPACE = 3, JT_ERR_CUDA = 4 } jt_status;
+typedef enum { JT_F32 = 0, JT_F64 = 1 } jt_dtype;
+typedef enum { JT_CONV_AUTO = 0, JT_CONV_DIRECT = 1, JT_CONV_FFT = 2 } jt_conv_method;
+
+/* Definition G (observer grid).  Host struct.  Pixel (j,i), j = row (y), i = column (x); sub-ray
+ * (J,I), J in [0,ny*s), I in [0,nx*s): theta_x = cx + (I - (nx*s-1)/2) h, theta_y = cy + (J - (ny*s-1)/2) h,
+ * h = pixel_scale/s.  Sub-ray (J,I) belongs to pixel (J/s, I/s). */
+typedef struct {
+    int32_t nx, ny;          /* pixels */
+    double  pixel_scale;     /* arcsec per pixel, > 0 */
+    double  cx, cy;          /* grid centre, arcsec */
+    int32_t supersample;     /* s >= 1 */
+} jt_grid;
+
+/* Deflectors (host struct).  Definitions S (SIE), H (external shear about the origin,
+ * PAPER.md:85), T (truncated NFW).  The five TNFW arrays are DEVICE pointers of the
+ * call's dtype, each [n_tnfw]; they may be NULL iff n_tnfw == 0. */
+typedef struct {
+    int32_t has_sie;   double sie_theta_E, sie_e1, sie_e2, sie_cx, sie_cy;
+    int32_t has_shear; double shear_gamma1, shear_gamma2;
+    int64_t n_tnfw;
+    const void *tnfw_cx, *tnfw_cy, *tnfw_Rs, *tnfw_alpha_Rs, *tnfw_r_trunc;
+} jt_lens;
+
+/* Elliptical Sersic components (definition R).  HOST arrays of doubles, each [n]. */
+typedef struct {
+    int32_t n;
+    const double *amp, *R_sersic, *n_sersic, *e1, *e2, *cx, *cy;
+} jt_sources;
+
+/* Step 1 ("ray-traced through the deflectors back to the source plane"):
+ * beta = theta - alpha_SIE - alpha_shear - sum_j alpha_TNFW,j on caller-supplied ray positions.
+ * theta_x, theta_y: device [n_rays] (in).  beta_x, beta_y: device [n_rays] (out).
+ * workspace: device scratch of at least jt_ray_shoot_workspace_bytes(dtype, n_rays, n_tnfw) bytes
+ * (partial sums when the subhalo list is split over thread blocks; may be NULL when that is 0). */
+JT_API size_t    jt_ray_shoot_workspace_bytes(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw);
+JT_API jt_status jt_ray_shoot(jt_dtype dtype, int64_t n_rays, const void *theta_x, const void *theta_y,
+                       const jt_lens *lens, void *workspace, size_t workspace_bytes,
+                       void *beta_x, void *beta_y, void *stream);
+
+/* Step 2 ("surface brightness of the source is calculated on the ray-traced grid"):
+ * flux[i] = sum_k Sersic_k(beta_x[i], beta_y[i]) -- surface brightness, no pixel-area factor.
+ * beta_x, beta_y: device [n] (in).  flux: device [n] (out). */
+JT_API jt_status jt_source_brightness(jt_dtype dtype, int64_t n, const void *beta_x, const void *beta_y,
+                               const jt_sources *sources, void *flux, void *stream);
+
+/* Step 3 ("convolved by the point spread function"), definition P:
+ * out[j][i] = sum_{u<ky} sum_{v<kx} K[u][v] img[j-(u-ky/2)][i-(v-kx/2)], out-of-range terms dropped
+ * (zero padding, 'same' size, true convolution -- kernel flipped relative to correlation).
+ * image: device [ny][nx] (in).  kernel: device [ky][kx], ky and kx odd (in); used as given, never
+ * renormalised.  out: device [ny][nx].  method: DIRECT = shared-memory tiled sum; FFT = zero-pad
+ * to a power of two P >= n+K-1, hand-written shared-memory FFTs; AUTO picks by kernel size.
+ * workspace: device scratch >= jt_psf_convolve_workspace_bytes(...) for the same arguments. */
+JT_API size_t    jt_psf_convolve_workspace_bytes(jt_dtype dtype, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
+                                          jt_conv_method method);
+JT_API jt_status jt_psf_convolve(jt_dtype dtype, int32_t ny, int32_t nx, const void *image,
+                          int32_t ky, int32_t kx, const void *kernel, jt_conv_method method,
+                          void *workspace, size_t workspace_bytes, void *out, void *stream);
+
+/* Steps 1-3 fused on one system: grid G generated in registers, ray-shoot, Sersic,
+ * binning B (image[j][i] = pixel_scale^2/s^2 * sum of the pixel's s*s sub-ray brightnesses, reduced
+ * with warp shuffles), then PSF convolution.  Traced coordinates never leave the chip.
+ * kernel: device [ky][kx] or NULL with ky = kx = 0 to skip the convolution (out = pre-PSF image).
+ * out: device [ny][nx].  workspace >= jt_simulate_image_workspace_bytes(...). */
+JT_API size_t    jt_simulate_image_workspace_bytes(jt_dtype dtype, const jt_grid *grid, int64_t n_tnfw,
+                                            int32_t ky, int32_t kx, jt_conv_method method);
+JT_API jt_status jt_simulate_image(jt_dtype dtype, const jt_grid *grid, const jt_lens *lens, const jt_sources *sources,
+                            int32_t ky, int32_t kx, const void *kernel, jt_conv_method method,
+                            void *workspace, size_t workspace_bytes, void *out, void *stream);
+
+/* B independent systems sharing one grid (PAPER.md:47 training-set generation; BASELINE.json configs[3]).
+ * All pointers are DEVICE arrays of the call's dtype with leading dimension B. */
+typedef struct {
+    const void *sie;                      /* [B][5]  theta_E, e1, e2, cx, cy */
+    const void *shear;                    /* [B][2]  gamma1, gamma2 */
+    int32_t n_tnfw;  const void *tnfw;    /* [B][5][n_tnfw]  rows cx, cy, Rs, alpha_Rs, r_trunc */
+    int32_t n_src;   const void *sersic;  /* [B][n_src][7]   amp, R_sersic, n_sersic, e1, e2, cx, cy */
+    int32_t ky, kx;  const void *psf;     /* [B][ky][kx], odd sizes; ky = kx = 0 and NULL skips the convolution */
+} jt_batch_params;
+
+/* One launch; one thread block per system keeps the pre-PSF image in shared memory and convolves it
+ * in place (direct sum).  out: device [B][ny][nx].  Limits: ny*nx*sizeof(dtype) + tables must fit
+ * 227 KB of shared memory (JT_ERR_UNSUPPORTED otherwise); no workspace. */
+JT_API jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid *grid, const jt_batch_params *params,
+                            void *out, void *stream);
+
+JT_API const char *jt_status_string(jt_status s);
+JT_API int         jt_last_cuda_error(void);     /* cudaError_t of the last JT_ERR_CUDA on this thread, else 0 */
+JT_API int         jt_version(void);             /* JT_VERSION */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* JT_H */

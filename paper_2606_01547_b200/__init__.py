@@ -1,0 +1,21 @@
+"""jt -- B200-native lensed-image simulation (hot path of arxiv/paper_2606_01547).
+
+The product is libjt.so (C ABI in include/jt.h, CUDA kernels in csrc/).  This package is a thin
+ctypes binding with the same names; PyTorch supplies device memory and streams only.
+There is no CPU fallback: calls raise if libjt.so is missing or no sm_100 device is present.
+"""
+from .binding import (  # noqa: F401
+    Grid,
+    JtError,
+    lib,
+    lib_path,
+    psf_convolve,
+    psf_convolve_workspace_bytes,
+    ray_shoot,
+    ray_shoot_workspace_bytes,
+    simulate_batch,
+    simulate_image,
+    simulate_image_workspace_bytes,
+    source_brightness,
+    version,
+)

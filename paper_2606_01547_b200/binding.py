@@ -1,0 +1,290 @@
+"""ctypes binding of include/jt.h -- argument marshalling only; every step runs in libjt's kernels.
+
+Tensors are torch CUDA tensors (float32 -> JT_F32, float64 -> JT_F64), contiguous; the current
+torch stream is passed through.  Names and argument meaning follow include/jt.h one to one.
+"""
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libjt.so")
+_lib = None
+
+JT_F32, JT_F64 = 0, 1
+_METHODS = {"auto": 0, "direct": 1, "fft": 2}
+_STATUS = {0: "JT_OK", 1: "JT_ERR_INVALID_VALUE", 2: "JT_ERR_UNSUPPORTED", 3: "JT_ERR_WORKSPACE", 4: "JT_ERR_CUDA"}
+
+
+class JtError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        extra = ""
+        if self.status == 4 and _lib is not None:
+            extra = " (cudaError %d)" % _lib.jt_last_cuda_error()
+        super().__init__("%s failed: %s%s" % (where, _STATUS.get(self.status, str(status)), extra))
+
+
+class _Grid(ctypes.Structure):
+    _fields_ = [("nx", ctypes.c_int32), ("ny", ctypes.c_int32), ("pixel_scale", ctypes.c_double),
+                ("cx", ctypes.c_double), ("cy", ctypes.c_double), ("supersample", ctypes.c_int32)]
+
+
+class _Lens(ctypes.Structure):
+    _fields_ = [("has_sie", ctypes.c_int32), ("sie_theta_E", ctypes.c_double), ("sie_e1", ctypes.c_double),
+                ("sie_e2", ctypes.c_double), ("sie_cx", ctypes.c_double), ("sie_cy", ctypes.c_double),
+                ("has_shear", ctypes.c_int32), ("shear_gamma1", ctypes.c_double), ("shear_gamma2", ctypes.c_double),
+                ("n_tnfw", ctypes.c_int64), ("tnfw_cx", ctypes.c_void_p), ("tnfw_cy", ctypes.c_void_p),
+                ("tnfw_Rs", ctypes.c_void_p), ("tnfw_alpha_Rs", ctypes.c_void_p), ("tnfw_r_trunc", ctypes.c_void_p)]
+
+
+_dp = ctypes.POINTER(ctypes.c_double)
+
+
+class _Sources(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int32), ("amp", _dp), ("R_sersic", _dp), ("n_sersic", _dp), ("e1", _dp),
+                ("e2", _dp), ("cx", _dp), ("cy", _dp)]
+
+
+class _Batch(ctypes.Structure):
+    _fields_ = [("sie", ctypes.c_void_p), ("shear", ctypes.c_void_p), ("n_tnfw", ctypes.c_int32),
+                ("tnfw", ctypes.c_void_p), ("n_src", ctypes.c_int32), ("sersic", ctypes.c_void_p),
+                ("ky", ctypes.c_int32), ("kx", ctypes.c_int32), ("psf", ctypes.c_void_p)]
+
+
+@dataclass
+class Grid:
+    """Definition G (include/jt.h jt_grid)."""
+    nx: int
+    ny: int
+    pixel_scale: float
+    cx: float = 0.0
+    cy: float = 0.0
+    supersample: int = 1
+
+    def _c(self):
+        return _Grid(self.nx, self.ny, self.pixel_scale, self.cx, self.cy, self.supersample)
+
+
+def lib_path():
+    return _LIB_PATH
+
+
+def lib():
+    """Loads libjt.so; raises (never falls back) when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError("libjt.so is missing: build it with `python -m paper_2606_01547_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(_LIB_PATH)
+        vp, i32, i64, sz = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_size_t
+        L.jt_status_string.restype = ctypes.c_char_p
+        L.jt_status_string.argtypes = [ctypes.c_int]
+        L.jt_last_cuda_error.restype = ctypes.c_int
+        L.jt_version.restype = ctypes.c_int
+        L.jt_ray_shoot_workspace_bytes.restype = sz
+        L.jt_ray_shoot_workspace_bytes.argtypes = [ctypes.c_int, i64, i64]
+        L.jt_ray_shoot.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Lens), vp, sz, vp, vp, vp]
+        L.jt_source_brightness.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Sources), vp, vp]
+        L.jt_psf_convolve_workspace_bytes.restype = sz
+        L.jt_psf_convolve_workspace_bytes.argtypes = [ctypes.c_int, i32, i32, i32, i32, ctypes.c_int]
+        L.jt_psf_convolve.argtypes = [ctypes.c_int, i32, i32, vp, i32, i32, vp, ctypes.c_int, vp, sz, vp, vp]
+        L.jt_simulate_image_workspace_bytes.restype = sz
+        L.jt_simulate_image_workspace_bytes.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), i64, i32, i32, ctypes.c_int]
+        L.jt_simulate_image.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), ctypes.POINTER(_Lens),
+                                        ctypes.POINTER(_Sources), i32, i32, vp, ctypes.c_int, vp, sz, vp, vp]
+        L.jt_simulate_batch.argtypes = [ctypes.c_int, i64, ctypes.POINTER(_Grid), ctypes.POINTER(_Batch), vp, vp]
+        _lib = L
+    return _lib
+
+
+def version():
+    return lib().jt_version()
+
+
+# ------------------------------------------------------------------ marshalling helpers
+def _dt(t):
+    if t.dtype == torch.float32:
+        return JT_F32
+    if t.dtype == torch.float64:
+        return JT_F64
+    raise TypeError("jt tensors must be float32 or float64, got %s" % t.dtype)
+
+
+def _torch_dtype(code):
+    return torch.float32 if code == JT_F32 else torch.float64
+
+
+def _code(dtype):
+    if dtype in (torch.float32, "f32", JT_F32, np.float32):
+        return JT_F32
+    if dtype in (torch.float64, "f64", JT_F64, np.float64):
+        return JT_F64
+    raise TypeError("dtype must be f32 or f64")
+
+
+def _dev(t, what):
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise TypeError("%s must be a contiguous CUDA tensor" % what)
+    return t
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _check(status, where):
+    if status != 0:
+        raise JtError(status, where)
+
+
+def _lens(dtype_code, sie, shear, tnfw):
+    L = _Lens()
+    if sie is not None:
+        L.has_sie = 1
+        L.sie_theta_E, L.sie_e1, L.sie_e2, L.sie_cx, L.sie_cy = [float(v) for v in sie]
+    if shear is not None:
+        L.has_shear = 1
+        L.shear_gamma1, L.shear_gamma2 = [float(v) for v in shear]
+    if tnfw is not None and tnfw.numel() > 0:
+        _dev(tnfw, "tnfw")
+        if tnfw.dim() != 2 or tnfw.shape[0] != 5 or _dt(tnfw) != dtype_code:
+            raise TypeError("tnfw must be a [5][M] tensor of the call's dtype")
+        M = tnfw.shape[1]
+        es = tnfw.element_size()
+        base = tnfw.data_ptr()
+        L.n_tnfw = M
+        L.tnfw_cx, L.tnfw_cy, L.tnfw_Rs, L.tnfw_alpha_Rs, L.tnfw_r_trunc = [base + k * M * es for k in range(5)]
+    return L
+
+
+def _sources(sources):
+    a = np.ascontiguousarray(np.asarray(sources, dtype=np.float64).reshape(-1, 7).T)   # [7][n]
+    S = _Sources()
+    S.n = a.shape[1]
+    ptrs = [a[k].ctypes.data_as(_dp) for k in range(7)]
+    S.amp, S.R_sersic, S.n_sersic, S.e1, S.e2, S.cx, S.cy = ptrs
+    return S, a          # keep `a` alive during the call
+
+
+def _workspace(nbytes, device, workspace):
+    if nbytes == 0:
+        return None, 0
+    if workspace is None:
+        workspace = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    return workspace, workspace.numel() * workspace.element_size()
+
+
+# ------------------------------------------------------------------ the five calls
+def ray_shoot_workspace_bytes(dtype, n_rays, n_tnfw):
+    return int(lib().jt_ray_shoot_workspace_bytes(_code(dtype), n_rays, n_tnfw))
+
+
+def ray_shoot(theta_x, theta_y, sie=None, shear=None, tnfw=None, workspace=None, stream=None):
+    """jt_ray_shoot: beta = theta - alpha(theta).  Returns (beta_x, beta_y)."""
+    _dev(theta_x, "theta_x"), _dev(theta_y, "theta_y")
+    code = _dt(theta_x)
+    n = theta_x.numel()
+    L = _lens(code, sie, shear, tnfw)
+    ws, wsb = _workspace(ray_shoot_workspace_bytes(code, n, L.n_tnfw), theta_x.device, workspace)
+    bx, by = torch.empty_like(theta_x), torch.empty_like(theta_y)
+    _check(lib().jt_ray_shoot(code, n, _ptr(theta_x), _ptr(theta_y), ctypes.byref(L), _ptr(ws), wsb,
+                              _ptr(bx), _ptr(by), _stream(stream)), "jt_ray_shoot")
+    return bx, by
+
+
+def source_brightness(beta_x, beta_y, sources, stream=None):
+    """jt_source_brightness: sum of elliptical Sersic components at (beta_x, beta_y)."""
+    _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y")
+    code = _dt(beta_x)
+    S, keep = _sources(sources)
+    flux = torch.empty_like(beta_x)
+    _check(lib().jt_source_brightness(code, beta_x.numel(), _ptr(beta_x), _ptr(beta_y), ctypes.byref(S),
+                                      _ptr(flux), _stream(stream)), "jt_source_brightness")
+    del keep
+    return flux
+
+
+def psf_convolve_workspace_bytes(dtype, ny, nx, ky, kx, method="auto"):
+    return int(lib().jt_psf_convolve_workspace_bytes(_code(dtype), ny, nx, ky, kx, _METHODS[method]))
+
+
+def psf_convolve(image, kernel, method="auto", workspace=None, out=None, stream=None):
+    """jt_psf_convolve: zero-padded 'same' true convolution of image [ny][nx] with kernel [ky][kx]."""
+    _dev(image, "image"), _dev(kernel, "kernel")
+    code = _dt(image)
+    if _dt(kernel) != code:
+        raise TypeError("image and kernel dtypes differ")
+    ny, nx = image.shape
+    ky, kx = kernel.shape
+    ws, wsb = _workspace(psf_convolve_workspace_bytes(code, ny, nx, ky, kx, method), image.device, workspace)
+    if out is None:
+        out = torch.empty_like(image)
+    _check(lib().jt_psf_convolve(code, ny, nx, _ptr(image), ky, kx, _ptr(kernel), _METHODS[method], _ptr(ws), wsb,
+                                 _ptr(out), _stream(stream)), "jt_psf_convolve")
+    return out
+
+
+def simulate_image_workspace_bytes(dtype, grid, n_tnfw, ky, kx, method="auto"):
+    g = grid._c()
+    return int(lib().jt_simulate_image_workspace_bytes(_code(dtype), ctypes.byref(g), n_tnfw, ky, kx, _METHODS[method]))
+
+
+def simulate_image(grid, sie, shear, tnfw, sources, psf, dtype=None, method="auto", workspace=None, out=None,
+                   stream=None, device="cuda"):
+    """jt_simulate_image: grid -> ray-shoot -> Sersic -> bin -> PSF convolution.  psf=None skips the convolution."""
+    code = _code(dtype) if dtype is not None else (_dt(psf) if psf is not None else _dt(tnfw))
+    g = grid._c()
+    L = _lens(code, sie, shear, tnfw)
+    S, keep = _sources(sources)
+    ky, kx = (0, 0) if psf is None else psf.shape
+    if psf is not None:
+        _dev(psf, "psf")
+        if _dt(psf) != code:
+            raise TypeError("psf dtype differs from the call's dtype")
+        device = psf.device
+    elif tnfw is not None:
+        device = tnfw.device
+    ws, wsb = _workspace(simulate_image_workspace_bytes(code, grid, L.n_tnfw, ky, kx, method), device, workspace)
+    if out is None:
+        out = torch.empty((grid.ny, grid.nx), dtype=_torch_dtype(code), device=device)
+    _check(lib().jt_simulate_image(code, ctypes.byref(g), ctypes.byref(L), ctypes.byref(S), ky, kx, _ptr(psf),
+                                   _METHODS[method], _ptr(ws), wsb, _ptr(out), _stream(stream)), "jt_simulate_image")
+    del keep
+    return out
+
+
+def simulate_batch(grid, sie, shear, tnfw, sersic, psf, out=None, stream=None):
+    """jt_simulate_batch: B independent systems.  sie [B][5], shear [B][2], tnfw [B][5][M], sersic [B][n][7], psf [B][ky][kx]."""
+    _dev(sie, "sie"), _dev(shear, "shear")
+    code = _dt(sie)
+    B = sie.shape[0]
+    P = _Batch()
+    P.sie, P.shear = sie.data_ptr(), shear.data_ptr()
+    if tnfw is not None and tnfw.numel() > 0:
+        _dev(tnfw, "tnfw")
+        P.n_tnfw, P.tnfw = tnfw.shape[2], tnfw.data_ptr()
+    if sersic is not None and sersic.numel() > 0:
+        _dev(sersic, "sersic")
+        P.n_src, P.sersic = sersic.shape[1], sersic.data_ptr()
+    if psf is not None:
+        _dev(psf, "psf")
+        P.ky, P.kx, P.psf = psf.shape[1], psf.shape[2], psf.data_ptr()
+    for t in (shear, tnfw, sersic, psf):
+        if t is not None and t.numel() > 0 and _dt(t) != code:
+            raise TypeError("all batch tensors must share one dtype")
+    g = grid._c()
+    if out is None:
+        out = torch.empty((B, grid.ny, grid.nx), dtype=_torch_dtype(code), device=sie.device)
+    _check(lib().jt_simulate_batch(code, B, ctypes.byref(g), ctypes.byref(P), _ptr(out), _stream(stream)),
+           "jt_simulate_batch")
+    return out

@@ -1,0 +1,187 @@
+// jt_api.cu -- the C ABI declared in include/jt.h: argument validation, workspace layout, launches.
+#include <string.h>
+#include "jt_internal.h"
+
+namespace jt {
+
+static thread_local int g_last_cuda_error = 0;
+void set_last_cuda_error(int e) { g_last_cuda_error = e; }
+
+static jt_status check_device() {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) { set_last_cuda_error((int)e); return JT_ERR_CUDA; }
+    int major = 0;
+    e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+    if (e != cudaSuccess) { set_last_cuda_error((int)e); return JT_ERR_CUDA; }
+    return major == 10 ? JT_OK : JT_ERR_UNSUPPORTED;
+}
+
+static bool valid_dtype(jt_dtype d) { return d == JT_F32 || d == JT_F64; }
+static bool valid_method(jt_conv_method m) { return m == JT_CONV_AUTO || m == JT_CONV_DIRECT || m == JT_CONV_FFT; }
+static bool valid_grid(const jt_grid* g) {
+    return g && g->nx >= 1 && g->ny >= 1 && g->pixel_scale > 0.0 && g->supersample >= 1 &&
+           g->supersample <= JT_MAX_SUPERSAMPLE && (int64_t)g->nx * g->supersample < (1 << 30) &&
+           (int64_t)g->ny * g->supersample < (1 << 30);
+}
+static bool valid_lens(const jt_lens* l) {
+    if (!l || l->n_tnfw < 0) return false;
+    if (l->n_tnfw > 0 && (!l->tnfw_cx || !l->tnfw_cy || !l->tnfw_Rs || !l->tnfw_alpha_Rs || !l->tnfw_r_trunc)) return false;
+    return true;
+}
+static bool valid_kernel_size(int ky, int kx) { return ky >= 1 && kx >= 1 && (ky & 1) && (kx & 1); }
+
+// AUTO: direct while the tap count is small or the halo tile fits; FFT for large kernels
+// (crossover measured on B200).
+jt_conv_method resolve_conv_method(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method m) {
+    if (m == JT_CONV_DIRECT || m == JT_CONV_FFT) return m;
+    if (!conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_CONV_FFT;
+    return ((int64_t)ky * kx > 41 * 41) ? JT_CONV_FFT : JT_CONV_DIRECT;
+}
+
+static size_t conv_ws(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method method) {
+    const jt_conv_method m = resolve_conv_method(dtype, ny, nx, ky, kx, method);
+    return m == JT_CONV_DIRECT ? conv_direct_workspace_bytes(dtype, ky, kx) : fft_conv_workspace_bytes(dtype, ny, nx, ky, kx);
+}
+
+static jt_status conv_dispatch(jt_dtype dtype, int ny, int nx, const void* image, int ky, int kx, const void* kernel,
+                               jt_conv_method method, void* workspace, void* out, cudaStream_t st) {
+    const jt_conv_method m = resolve_conv_method(dtype, ny, nx, ky, kx, method);
+    if (m == JT_CONV_DIRECT) return launch_conv_direct(dtype, ny, nx, image, ky, kx, kernel, workspace, out, st);
+    return launch_conv_fft(dtype, ny, nx, image, ky, kx, kernel, workspace, out, st);
+}
+
+}  // namespace jt
+
+using namespace jt;
+
+extern "C" {
+
+const char* jt_status_string(jt_status s) {
+    switch (s) {
+        case JT_OK: return "JT_OK";
+        case JT_ERR_INVALID_VALUE: return "JT_ERR_INVALID_VALUE";
+        case JT_ERR_UNSUPPORTED: return "JT_ERR_UNSUPPORTED";
+        case JT_ERR_WORKSPACE: return "JT_ERR_WORKSPACE";
+        case JT_ERR_CUDA: return "JT_ERR_CUDA";
+    }
+    return "JT_ERR_UNKNOWN";
+}
+int jt_last_cuda_error(void) { return g_last_cuda_error; }
+int jt_version(void) { return JT_VERSION; }
+
+// ------------------------------------------------------------------ step 1
+size_t jt_ray_shoot_workspace_bytes(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw) {
+    if (!valid_dtype(dtype) || n_rays <= 0 || n_tnfw < 0) return 0;
+    return plan_trace_rays(n_rays, n_tnfw).total_bytes;
+}
+
+jt_status jt_ray_shoot(jt_dtype dtype, int64_t n_rays, const void* theta_x, const void* theta_y, const jt_lens* lens,
+                       void* workspace, size_t workspace_bytes, void* beta_x, void* beta_y, void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (n_rays < 0 || !valid_lens(lens)) return JT_ERR_INVALID_VALUE;
+    if (n_rays == 0) return JT_OK;
+    if (!theta_x || !theta_y || !beta_x || !beta_y) return JT_ERR_INVALID_VALUE;
+    if (theta_x == beta_x || theta_y == beta_y || theta_x == beta_y || theta_y == beta_x) return JT_ERR_INVALID_VALUE;
+    const TracePlan plan = plan_trace_rays(n_rays, lens->n_tnfw);
+    if (plan.total_bytes > 0 && (!workspace || workspace_bytes < plan.total_bytes)) return JT_ERR_WORKSPACE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_trace_rays(dtype, n_rays, theta_x, theta_y, lens, plan, workspace, beta_x, beta_y, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ step 2
+jt_status jt_source_brightness(jt_dtype dtype, int64_t n, const void* beta_x, const void* beta_y,
+                               const jt_sources* sources, void* flux, void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (n < 0) return JT_ERR_INVALID_VALUE;
+    SrcSet S;
+    jt_status s = make_sources(sources, &S);
+    if (s != JT_OK) return s;
+    if (n == 0) return JT_OK;
+    if (!beta_x || !beta_y || !flux || flux == beta_x || flux == beta_y) return JT_ERR_INVALID_VALUE;
+    s = check_device();
+    if (s != JT_OK) return s;
+    return launch_source_brightness(dtype, n, beta_x, beta_y, S, flux, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ step 3
+size_t jt_psf_convolve_workspace_bytes(jt_dtype dtype, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
+                                       jt_conv_method method) {
+    if (!valid_dtype(dtype) || !valid_method(method) || ny < 1 || nx < 1 || !valid_kernel_size(ky, kx)) return 0;
+    return conv_ws(dtype, ny, nx, ky, kx, method);
+}
+
+jt_status jt_psf_convolve(jt_dtype dtype, int32_t ny, int32_t nx, const void* image, int32_t ky, int32_t kx,
+                          const void* kernel, jt_conv_method method, void* workspace, size_t workspace_bytes, void* out,
+                          void* stream) {
+    if (!valid_dtype(dtype) || !valid_method(method)) return JT_ERR_UNSUPPORTED;
+    if (ny < 1 || nx < 1 || !valid_kernel_size(ky, kx) || !image || !kernel || !out || image == out)
+        return JT_ERR_INVALID_VALUE;
+    if (method == JT_CONV_DIRECT && !conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_ERR_UNSUPPORTED;
+    const size_t need = conv_ws(dtype, ny, nx, ky, kx, method);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return conv_dispatch(dtype, ny, nx, image, ky, kx, kernel, method, workspace, out, (cudaStream_t)stream);
+}
+
+// ------------------------------------------------------------------ fused image
+// workspace layout: [trace partials + counters][pre-PSF image][convolution scratch]
+size_t jt_simulate_image_workspace_bytes(jt_dtype dtype, const jt_grid* grid, int64_t n_tnfw, int32_t ky, int32_t kx,
+                                         jt_conv_method method) {
+    if (!valid_dtype(dtype) || !valid_method(method) || !valid_grid(grid) || n_tnfw < 0) return 0;
+    const TracePlan plan = plan_trace_grid(dtype, grid, n_tnfw);
+    size_t total = align_up(plan.total_bytes, 256);
+    if (ky > 0 || kx > 0) {
+        if (!valid_kernel_size(ky, kx)) return 0;
+        total += align_up((size_t)grid->nx * grid->ny * dtype_size(dtype), 256);
+        total += conv_ws(dtype, grid->ny, grid->nx, ky, kx, method);
+    }
+    return total;
+}
+
+jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* lens, const jt_sources* sources,
+                            int32_t ky, int32_t kx, const void* kernel, jt_conv_method method, void* workspace,
+                            size_t workspace_bytes, void* out, void* stream) {
+    if (!valid_dtype(dtype) || !valid_method(method)) return JT_ERR_UNSUPPORTED;
+    if (!valid_grid(grid) || !valid_lens(lens) || !out) return JT_ERR_INVALID_VALUE;
+    SrcSet S;
+    jt_status s = make_sources(sources, &S);
+    if (s != JT_OK) return s;
+    const bool conv = !(ky == 0 && kx == 0 && kernel == nullptr);
+    if (conv && (!valid_kernel_size(ky, kx) || !kernel)) return JT_ERR_INVALID_VALUE;
+    if (conv && method == JT_CONV_DIRECT && !conv_direct_supported(dtype, grid->ny, grid->nx, ky, kx)) return JT_ERR_UNSUPPORTED;
+    const size_t need = jt_simulate_image_workspace_bytes(dtype, grid, lens->n_tnfw, conv ? ky : 0, conv ? kx : 0, method);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
+    s = check_device();
+    if (s != JT_OK) return s;
+    const TracePlan plan = plan_trace_grid(dtype, grid, lens->n_tnfw);
+    char* ws = (char*)workspace;
+    void* trace_ws = ws;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!conv) return launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, out, st);
+    void* pre = ws + align_up(plan.total_bytes, 256);
+    void* conv_ws_ptr = (char*)pre + align_up((size_t)grid->nx * grid->ny * dtype_size(dtype), 256);
+    s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, pre, st);
+    if (s != JT_OK) return s;
+    return conv_dispatch(dtype, grid->ny, grid->nx, pre, ky, kx, kernel, method, conv_ws_ptr, out, st);
+}
+
+// ------------------------------------------------------------------ batch
+jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid* grid, const jt_batch_params* p, void* out,
+                            void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (B < 0 || !valid_grid(grid) || !p) return JT_ERR_INVALID_VALUE;
+    if (B == 0) return JT_OK;
+    if (!out || !p->sie || !p->shear || p->n_tnfw < 0 || (p->n_tnfw > 0 && !p->tnfw) || p->n_src < 0 ||
+        p->n_src > JT_MAX_SOURCES || (p->n_src > 0 && !p->sersic))
+        return JT_ERR_INVALID_VALUE;
+    const bool conv = !(p->ky == 0 && p->kx == 0 && p->psf == nullptr);
+    if (conv && (!valid_kernel_size(p->ky, p->kx) || !p->psf)) return JT_ERR_INVALID_VALUE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_batch(dtype, B, grid, p, out, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,255 @@
+// jt_device.cuh -- device arithmetic of the lensing hot path (sm_100a).
+//
+// Definitions implemented (readings in DESIGN.md; the paper, PAPER.md:55/:80/:85/:87/:103, prints names only):
+//   E ellipticity, S SIE deflection, H external shear, T truncated-NFW deflection, R elliptical Sersic.
+// Shares nothing with oracle/: the formulas are re-derived in the forms the GPU wants
+// (rsqrt-based, polynomial atan/atanh, cancellation-free far field), see DESIGN.md "Kernel arithmetic".
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "jt_poly.h"
+
+namespace jt {
+
+#define JT_PI_D 3.14159265358979323846264338327950288
+#define JT_LN2_D 0.693147180559945309417232121458176568
+
+// ------------------------------------------------------------------------------------------------
+// small numeric helpers
+// ------------------------------------------------------------------------------------------------
+template <typename T, int N>
+__device__ __forceinline__ T horner(const T (&c)[N], T z) {
+    T p = c[0];
+#pragma unroll
+    for (int i = 1; i < N; ++i) p = fma(p, z, c[i]);
+    return p;
+}
+
+// atan(sqrt z)/sqrt z on [0,1/9]  (far field: z = 1/(X^2-1))
+__device__ __forceinline__ float atan_far(float z) { const float c[] = {JT_ATAN_FAR_F32_COEFS}; return horner(c, z); }
+__device__ __forceinline__ double atan_far(double z) { const double c[] = {JT_ATAN_FAR_F64_COEFS}; return horner(c, z); }
+// atan(sqrt z)/sqrt z on [0,1]
+__device__ __forceinline__ float atan_full(float z) { const float c[] = {JT_ATAN_FULL_F32_COEFS}; return horner(c, z); }
+__device__ __forceinline__ double atan_full(double z) { const double c[] = {JT_ATAN_FULL_F64_COEFS}; return horner(c, z); }
+// atanh(sqrt z)/sqrt z on [0,1/4]
+__device__ __forceinline__ float atanh_q(float z) { const float c[] = {JT_ATANH_Q_F32_COEFS}; return horner(c, z); }
+__device__ __forceinline__ double atanh_q(double z) { const double c[] = {JT_ATANH_Q_F64_COEFS}; return horner(c, z); }
+
+// Reciprocal square root / reciprocal: one MUFU seed (~20-22 bits) + one third-order correction.
+__device__ __forceinline__ float fast_rsqrt(float x) { return rsqrtf(x); }                 // MUFU.RSQ
+__device__ __forceinline__ float fast_rcp(float x) { return __frcp_rn(x); }
+__device__ __forceinline__ float approx_rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+__device__ __forceinline__ double fast_rsqrt(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));          // MUFU.RSQ64H, ~20 bits
+    const double e = fma(-x, y * y, 1.0);                             // e = 1 - x y^2  (~2^-19)
+    return fma(y, e * fma(0.375, e, 0.5), y);                         // y (1 + e/2 + 3e^2/8): error O(e^3)
+}
+__device__ __forceinline__ double fast_rcp(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));            // MUFU.RCP64H, ~20 bits
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);                                   // y (1 + e + e^2): error O(e^3)
+}
+__device__ __forceinline__ double approx_rcp(double x) { return fast_rcp(x); }
+
+__device__ __forceinline__ float t_sqrt(float x) { return sqrtf(x); }
+__device__ __forceinline__ double t_sqrt(double x) { return sqrt(x); }
+__device__ __forceinline__ float t_log(float x) { return logf(x); }
+__device__ __forceinline__ double t_log(double x) { return log(x); }
+
+// ------------------------------------------------------------------------------------------------
+// T: truncated NFW.  Per-subhalo record, derived once (in double) when a tile is staged.
+//   alpha = amp * brace(X^2) / R^2 * (dx, dy),   X^2 = R^2 * iRs2,   amp = alpha_Rs/(1-ln2) * Rs * t/(t+1)^2,
+//   brace = (t-1+2X^2) F(X) + c1 + S (c2 L - pi),  t = tau^2, c1 = tau pi + (t-1) ln tau, c2 = (t-1)/tau,
+//   S = sqrt(t+X^2), L = ln(X/(S+tau)).
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+struct alignas(sizeof(T) * 8) SubRec {
+    T cx, cy, iRs2, thr;      // centre, 1/Rs^2, far-field threshold on X^2 (= max(10, 3t))
+    T t, c1, amp, tm1;        // tau^2, c1, amplitude, tau^2 - 1
+};
+
+template <typename T>
+__device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, double aRs, double rt) {
+    const double tau = rt / Rs, t = tau * tau;
+    SubRec<T> r;
+    r.cx = (T)cx;
+    r.cy = (T)cy;
+    r.iRs2 = (T)(1.0 / (Rs * Rs));
+    r.thr = (T)fmax(10.0, 3.0 * t);
+    r.t = (T)t;
+    r.c1 = (T)(tau * JT_PI_D + (t - 1.0) * log(tau));
+    r.amp = (T)(aRs / (1.0 - JT_LN2_D) * Rs * t / ((t + 1.0) * (t + 1.0)));
+    r.tm1 = (T)(t - 1.0);
+    return r;
+}
+// padding record: contributes exactly 0 and always takes the far path
+template <typename T>
+__device__ __forceinline__ SubRec<T> null_rec() {
+    SubRec<T> r;
+    r.cx = (T)1e6; r.cy = (T)1e6; r.iRs2 = (T)1; r.thr = (T)10; r.t = (T)1; r.c1 = (T)0; r.amp = (T)0; r.tm1 = (T)0;
+    return r;
+}
+
+// Far field, X^2 >= max(10, 3t): no logarithm, no cancellation growing with X.
+//   w = 1/sqrt(X^2-1), z = w^2 <= 1/9, y = t/(X^2+t) <= 1/4,  P = atan(w)/w, Q = atanh(sqrt y)/sqrt y
+//   F = (pi/2 - w P) w;   S c2 L = -(t-1) Q;   2 X^2 F - pi S = pi (w + u - S) - 2 (1+z) P
+//   brace = (t-1)(F - Q) + c1 + pi (w + u - S) - 2 (1+z) P
+// Returns f with alpha = f * (dx, dy).
+template <typename T>
+__device__ __forceinline__ T tnfw_far(T R2, const SubRec<T>& s) {
+    const T u2 = fma(R2, s.iRs2, (T)-1);
+    const T S2 = fma(R2, s.iRs2, s.t);
+    const T w = fast_rsqrt(u2);
+    const T rS = fast_rsqrt(S2);
+    const T iR2 = approx_rcp(R2);
+    const T u = u2 * w, S = S2 * rS, z = w * w, y = (s.t * rS) * rS;
+    const T P = atan_far(z);
+    const T Q = atanh_q(y);
+    const T F = fma(-w, P, (T)(JT_PI_D / 2)) * w;
+    T b = fma(s.tm1, F - Q, s.c1);
+    b = fma((T)JT_PI_D, (w + u) - S, b);
+    b = fma((T)-2, fma(z, P, P), b);
+    return (s.amp * b) * iR2;
+}
+
+// Closed form for any X^2 > 0 (float: use only for X^2 >= 1/4; double: X^2 >= 1e-6).
+template <typename T>
+__device__ __noinline__ T tnfw_mid(T R2, T iRs2, T t, T c1, T amp, T tm1) {
+    const T X2 = R2 * iRs2;
+    const T S = t_sqrt(t + X2);
+    const T tau = t_sqrt(t);
+    const T d = S + tau;
+    const T L = (T)0.5 * t_log(X2 / (d * d));
+    T F, G2;                                         // G2 = 2 X^2 F - pi S
+    if (X2 > (T)1) {
+        const T u2 = X2 - (T)1;
+        if (u2 >= (T)1) {
+            const T w = (T)1 / t_sqrt(u2), z = w * w;
+            const T P = atan_full(z);
+            F = fma(-w, P, (T)(JT_PI_D / 2)) * w;
+            G2 = fma((T)JT_PI_D, (w + u2 * w) - S, (T)-2 * fma(z, P, P));
+        } else {
+            F = atan_full(u2);
+            G2 = fma((T)2 * X2, F, -(T)JT_PI_D * S);
+        }
+    } else {
+        const T u2 = (T)1 - X2;
+        if (u2 <= (T)0.25) {
+            F = atanh_q(u2);
+        } else {
+            const T u = t_sqrt(u2);
+            F = (t_log((T)1 + u) - (T)0.5 * t_log(X2)) / u;
+        }
+        G2 = fma((T)2 * X2, F, -(T)JT_PI_D * S);
+    }
+    const T b = fma(tm1, F, c1) + fma((tm1 / tau) * S, L, G2);
+    return amp * b / R2;
+}
+
+// Two-term small-X series of the brace (X < 1e-3 in double), l = ln(2/X), t = tau^2.
+static __device__ __noinline__ double tnfw_series(double R2, double iRs2, double t, double amp) {
+    const double X2 = R2 * iRs2;
+    const double tau = sqrt(t), lt = log(tau), l = 0.5 * log(4.0 / X2);
+    const double it = 1.0 / t;
+    const double c2 = (t + 1.0) * (t + 1.0) * 0.5 * it * l - (t * t - 1.0) * 0.25 * it - (t - 1.0) * 0.5 * it * lt
+                    - JT_PI_D / (2.0 * tau);
+    const double c4 = (0.375 * t + 0.625 + 0.125 * it - 0.125 * it * it) * l - 7.0 * t / 32.0 - 9.0 / 32.0
+                    - it / 32.0 + it * it / 32.0 + lt * 0.125 * (it - it * it) + JT_PI_D / (8.0 * tau * t);
+    const double b = X2 * (c2 + X2 * c4);
+    return amp * b / R2;
+}
+
+// Any R^2 in double from a double record (used by the f64 kernels' generic path and by the f32 near path).
+__device__ __forceinline__ double tnfw_any(double R2, const SubRec<double>& s) {
+    if (R2 == 0.0) return 0.0;
+    const double X2 = R2 * s.iRs2;
+    if (X2 < 1e-6) return tnfw_series(R2, s.iRs2, s.t, s.amp);
+    return tnfw_mid<double>(R2, s.iRs2, s.t, s.c1, s.amp, s.tm1);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S + H: smooth lens, evaluated per ray in double (both modes).  Host precomputes E: (cos phi, sin phi, q).
+//   b = theta_E sqrt q, f = sqrt(1-q^2), psi = sqrt(q^2 x'^2 + y'^2)
+//   a'x = b (x'/psi) A(f x'/psi), a'y = b (y'/psi) Bh(f y'/psi), A = atan(z)/z, Bh = atanh(z)/z.
+// ------------------------------------------------------------------------------------------------
+struct MacroLens {
+    int has_sie, has_shear;
+    double c, s, q, b, f, cx, cy;
+    double g1, g2;
+};
+
+__device__ __forceinline__ double atanh_over(double z2) {      // atanh(z)/z as a function of z^2 in [0,1)
+    if (z2 <= 0.25) return atanh_q(z2);
+    const double z = sqrt(z2);
+    return 0.5 * log((1.0 + z) / (1.0 - z)) / z;
+}
+
+__device__ __forceinline__ void macro_alpha(const MacroLens& m, double x, double y, double& ax, double& ay) {
+    ax = 0.0; ay = 0.0;
+    if (m.has_sie) {
+        const double dx = x - m.cx, dy = y - m.cy;
+        const double xr = m.c * dx + m.s * dy, yr = -m.s * dx + m.c * dy;
+        const double psi2 = m.q * m.q * xr * xr + yr * yr;
+        if (psi2 > 0.0) {
+            const double ipsi = fast_rsqrt(psi2);
+            const double cx_ = xr * ipsi, cy_ = yr * ipsi;        // x'/psi, y'/psi
+            const double zx = m.f * cx_, zy = m.f * cy_;
+            const double A = atan_full(zx * zx);                  // |zx| <= f < 1
+            const double Bh = atanh_over(zy * zy);
+            const double axr = m.b * cx_ * A, ayr = m.b * cy_ * Bh;
+            ax = m.c * axr - m.s * ayr;
+            ay = m.s * axr + m.c * ayr;
+        }
+    }
+    if (m.has_shear) {
+        ax += m.g1 * x + m.g2 * y;
+        ay += m.g2 * x - m.g1 * y;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// R: elliptical Sersic.  Host precomputes per component: cos phi, sin phi, q, 1/q, centre, amp, b_n,
+// p = 1/(2 n), 1/R_sersic^2.   I = amp exp(-b_n ((R^2/Rs^2)^p - 1)),  R^2 = q x'^2 + y'^2/q.
+// ------------------------------------------------------------------------------------------------
+#define JT_MAX_SRC 16
+struct SrcSet {
+    int n;
+    double c[JT_MAX_SRC], s[JT_MAX_SRC], q[JT_MAX_SRC], iq[JT_MAX_SRC], cx[JT_MAX_SRC], cy[JT_MAX_SRC];
+    double amp[JT_MAX_SRC], bn[JT_MAX_SRC], p[JT_MAX_SRC], iRs2[JT_MAX_SRC];
+};
+
+template <typename T>
+__device__ __forceinline__ double sersic_sum(const SrcSet& S, double bx, double by);
+
+template <>
+__device__ __forceinline__ double sersic_sum<double>(const SrcSet& S, double bx, double by) {
+    double acc = 0.0;
+    for (int k = 0; k < S.n; ++k) {
+        const double dx = bx - S.cx[k], dy = by - S.cy[k];
+        const double xr = S.c[k] * dx + S.s[k] * dy, yr = -S.s[k] * dx + S.c[k] * dy;
+        const double a = (S.q[k] * xr * xr + S.iq[k] * yr * yr) * S.iRs2[k];
+        const double pw = (a > 0.0) ? exp(S.p[k] * log(a)) : 0.0;
+        acc += S.amp[k] * exp(-S.bn[k] * (pw - 1.0));
+    }
+    return acc;
+}
+
+// float mode: the subtraction beta - centre stays double (it cancels), the profile itself is float
+// with MUFU lg2/ex2 (error analysis in DESIGN.md "Precision").
+template <>
+__device__ __forceinline__ double sersic_sum<float>(const SrcSet& S, double bx, double by) {
+    float acc = 0.f;
+    for (int k = 0; k < S.n; ++k) {
+        const float dx = (float)(bx - S.cx[k]), dy = (float)(by - S.cy[k]);
+        const float c = (float)S.c[k], s = (float)S.s[k];
+        const float xr = c * dx + s * dy, yr = -s * dx + c * dy;
+        const float a = ((float)S.q[k] * xr * xr + (float)S.iq[k] * yr * yr) * (float)S.iRs2[k];
+        const float pw = (a > 0.f) ? exp2f((float)S.p[k] * __log2f(a)) : 0.f;
+        acc += (float)S.amp[k] * exp2f((float)(-S.bn[k] * 1.4426950408889634) * (pw - 1.f));
+    }
+    return (double)acc;
+}
+
+}  // namespace jt

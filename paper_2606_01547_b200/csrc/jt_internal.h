@@ -1,0 +1,71 @@
+// jt_internal.h -- host-side plumbing shared by the translation units of libjt (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+#include "../../include/jt.h"
+#include "jt_device.cuh"
+
+namespace jt {
+
+constexpr int kNumSMs = 148;            // B200
+constexpr int kTraceThreads = 256;      // 8 warps per CTA in the ray-tracing kernels
+constexpr int kSubTile = 256;           // subhalo records staged per shared-memory tile
+
+// thread-local last CUDA error (jt_last_cuda_error)
+void set_last_cuda_error(int e);
+#define JT_CUDA_TRY(expr)                                                    \
+    do {                                                                     \
+        cudaError_t _e = (expr);                                             \
+        if (_e != cudaSuccess) { jt::set_last_cuda_error((int)_e); return JT_ERR_CUDA; } \
+    } while (0)
+#define JT_LAUNCH_CHECK()                                                    \
+    do {                                                                     \
+        cudaError_t _e = cudaGetLastError();                                 \
+        if (_e != cudaSuccess) { jt::set_last_cuda_error((int)_e); return JT_ERR_CUDA; } \
+    } while (0)
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline size_t dtype_size(jt_dtype d) { return d == JT_F32 ? 4 : 8; }
+
+// ---- host-side derived parameters (definition E and the constants of S, R) ----
+MacroLens make_macro(const jt_lens* lens);
+jt_status make_sources(const jt_sources* src, SrcSet* out);
+
+// ---- ray tracing (jt_trace.cu) ----
+struct TracePlan {
+    int R;                 // rays per thread
+    int cols_per_warp;     // active lanes per warp (grid mode: floor(32/s)*s; ray mode: 32)
+    int tiles_x, tiles_y;  // ray tiles (ray mode: tiles_y = 1)
+    int64_t n_tiles;
+    int n_chunks;          // subhalo list split (1 = no workspace traffic)
+    int64_t chunk_len;     // subhalos per chunk (multiple of kSubTile unless n_chunks == 1)
+    size_t partial_bytes;  // n_chunks > 1: double2 per (chunk, ray slot)
+    size_t counter_bytes;  // one uint32 per tile
+    size_t total_bytes;
+};
+TracePlan plan_trace_grid(jt_dtype dtype, const jt_grid* g, int64_t n_tnfw);
+TracePlan plan_trace_rays(int64_t n_rays, int64_t n_tnfw);
+
+jt_status launch_trace_grid(jt_dtype dtype, const jt_grid* g, const jt_lens* lens, const SrcSet& src,
+                            const TracePlan& plan, void* workspace, void* pre_psf, cudaStream_t st);
+jt_status launch_trace_rays(jt_dtype dtype, int64_t n, const void* tx, const void* ty, const jt_lens* lens,
+                            const TracePlan& plan, void* workspace, void* bx, void* by, cudaStream_t st);
+jt_status launch_source_brightness(jt_dtype dtype, int64_t n, const void* bx, const void* by, const SrcSet& src,
+                                   void* flux, cudaStream_t st);
+
+// ---- convolution (jt_conv.cu, jt_fft.cu) ----
+jt_conv_method resolve_conv_method(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method m);
+bool      conv_direct_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
+size_t    conv_direct_workspace_bytes(jt_dtype dtype, int ky, int kx);
+jt_status launch_conv_direct(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
+                             void* workspace, void* out, cudaStream_t st);
+size_t    fft_conv_workspace_bytes(jt_dtype dtype, int ny, int nx, int ky, int kx);
+jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
+                          void* workspace, void* out, cudaStream_t st);
+
+// ---- batch (jt_batch.cu) ----
+jt_status launch_batch(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
+                       cudaStream_t st);
+
+}  // namespace jt

@@ -1,0 +1,182 @@
+// jt_trace.cu -- host side of the ray-tracing kernels: derived parameters, launch plans, launches;
+// plus the unfused step-2 kernel (jt_source_brightness).
+#include <math.h>
+#include "jt_trace.cuh"
+
+namespace jt {
+
+template <typename T, bool GRID>
+jt_status launch_trace_t(const TraceArgs<T>& a, int R, cudaStream_t st);
+
+// ---- definition E on the host: (e1,e2) -> (cos phi, sin phi, q) ----
+static void ellipticity(double e1, double e2, double* c, double* s, double* q) {
+    double m = sqrt(e1 * e1 + e2 * e2);
+    if (m > 0.9999) m = 0.9999;
+    const double phi = 0.5 * atan2(e2, e1);
+    *c = cos(phi);
+    *s = sin(phi);
+    *q = (1.0 - m) / (1.0 + m);
+}
+
+MacroLens make_macro(const jt_lens* lens) {
+    MacroLens m = {};
+    m.has_sie = lens->has_sie ? 1 : 0;
+    m.has_shear = lens->has_shear ? 1 : 0;
+    if (m.has_sie) {
+        ellipticity(lens->sie_e1, lens->sie_e2, &m.c, &m.s, &m.q);
+        m.b = lens->sie_theta_E * sqrt(m.q);
+        m.f = sqrt(1.0 - m.q * m.q);
+        m.cx = lens->sie_cx;
+        m.cy = lens->sie_cy;
+    }
+    if (m.has_shear) { m.g1 = lens->shear_gamma1; m.g2 = lens->shear_gamma2; }
+    return m;
+}
+
+jt_status make_sources(const jt_sources* src, SrcSet* out) {
+    SrcSet S = {};
+    if (!src || src->n < 0 || src->n > JT_MAX_SOURCES) return JT_ERR_INVALID_VALUE;
+    S.n = src->n;
+    if (S.n > 0 && (!src->amp || !src->R_sersic || !src->n_sersic || !src->e1 || !src->e2 || !src->cx || !src->cy))
+        return JT_ERR_INVALID_VALUE;
+    for (int k = 0; k < S.n; ++k) {
+        ellipticity(src->e1[k], src->e2[k], &S.c[k], &S.s[k], &S.q[k]);
+        S.iq[k] = 1.0 / S.q[k];
+        S.cx[k] = src->cx[k];
+        S.cy[k] = src->cy[k];
+        S.amp[k] = src->amp[k];
+        S.bn[k] = 1.9992 * src->n_sersic[k] - 0.3271;           // reading Q10
+        S.p[k] = 0.5 / src->n_sersic[k];
+        S.iRs2[k] = 1.0 / (src->R_sersic[k] * src->R_sersic[k]);
+    }
+    *out = S;
+    return JT_OK;
+}
+
+// ---- plans ----
+static int rays_per_thread(int s, bool f64) {
+    if (f64) {
+        switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 6; case 5: return 5; default: return s; }
+    }
+    switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 9; case 5: return 10; default: return s; }
+}
+
+static void plan_chunks(TracePlan* p, int64_t M, int R) {
+    // enough (tile, chunk) CTAs for ~10 waves of 2 CTAs per SM; chunks are whole shared-memory tiles
+    const int64_t target = (int64_t)kNumSMs * 2 * 10;
+    int64_t n_sub_tiles = (M + kSubTile - 1) / kSubTile;
+    int64_t want = (p->n_tiles > 0) ? (target + p->n_tiles - 1) / p->n_tiles : 1;
+    if (want < 1) want = 1;
+    if (want > n_sub_tiles) want = n_sub_tiles;
+    if (want < 1) want = 1;
+    int64_t tiles_per_chunk = (n_sub_tiles + want - 1) / want;
+    if (tiles_per_chunk < 1) tiles_per_chunk = 1;
+    p->chunk_len = tiles_per_chunk * kSubTile;
+    p->n_chunks = (int)((M + p->chunk_len - 1) / p->chunk_len);
+    if (p->n_chunks < 1) p->n_chunks = 1;
+    p->partial_bytes = p->n_chunks > 1 ? (size_t)p->n_chunks * p->n_tiles * R * kTraceThreads * sizeof(double2) : 0;
+    p->counter_bytes = p->n_chunks > 1 ? align_up((size_t)p->n_tiles * sizeof(unsigned int), 256) : 0;
+    p->total_bytes = p->partial_bytes + p->counter_bytes;
+}
+
+static TracePlan plan_trace_grid_t(const jt_grid* g, int64_t n_tnfw, bool f64) {
+    TracePlan p = {};
+    const int s = g->supersample;
+    p.R = rays_per_thread(s, f64);
+    p.cols_per_warp = (32 / s) * s;
+    const int NX = g->nx * s, NY = g->ny * s;
+    p.tiles_x = (NX + 2 * p.cols_per_warp - 1) / (2 * p.cols_per_warp);
+    p.tiles_y = (NY + 4 * p.R - 1) / (4 * p.R);
+    p.n_tiles = (int64_t)p.tiles_x * p.tiles_y;
+    plan_chunks(&p, n_tnfw, p.R);
+    return p;
+}
+TracePlan plan_trace_grid(jt_dtype d, const jt_grid* g, int64_t n_tnfw) { return plan_trace_grid_t(g, n_tnfw, d == JT_F64); }
+
+TracePlan plan_trace_rays(int64_t n_rays, int64_t n_tnfw) {
+    TracePlan p = {};
+    p.R = 8;
+    p.cols_per_warp = 32;
+    p.tiles_x = 1; p.tiles_y = 1;
+    p.n_tiles = (n_rays + (int64_t)p.R * kTraceThreads - 1) / ((int64_t)p.R * kTraceThreads);
+    plan_chunks(&p, n_tnfw, p.R);
+    return p;
+}
+
+template <typename T>
+static void fill_lens(TraceArgs<T>& a, const jt_lens* lens, const TracePlan& plan, void* workspace) {
+    a.m = make_macro(lens);
+    a.M = lens->n_tnfw;
+    a.tn[0] = (const T*)lens->tnfw_cx; a.tn[1] = (const T*)lens->tnfw_cy; a.tn[2] = (const T*)lens->tnfw_Rs;
+    a.tn[3] = (const T*)lens->tnfw_alpha_Rs; a.tn[4] = (const T*)lens->tnfw_r_trunc;
+    a.n_chunks = plan.n_chunks;
+    a.chunk_len = plan.chunk_len;
+    a.n_tiles = plan.n_tiles;
+    a.partial = (double2*)workspace;
+    a.counter = (unsigned int*)((char*)workspace + plan.partial_bytes);
+}
+
+template <typename T>
+static jt_status trace_grid_t(const jt_grid* g, const jt_lens* lens, const SrcSet& src, const TracePlan& plan,
+                              void* workspace, void* pre_psf, cudaStream_t st) {
+    TraceArgs<T> a = {};
+    const int s = g->supersample;
+    a.nx = g->nx; a.ny = g->ny; a.s = s; a.NX = g->nx * s; a.NY = g->ny * s;
+    a.h = g->pixel_scale / (double)s;
+    a.x0 = g->cx - 0.5 * (double)(a.NX - 1) * a.h;
+    a.y0 = g->cy - 0.5 * (double)(a.NY - 1) * a.h;
+    a.area_over_s2 = g->pixel_scale * g->pixel_scale / ((double)s * (double)s);
+    a.cols_per_warp = plan.cols_per_warp;
+    a.tiles_x = plan.tiles_x;
+    fill_lens(a, lens, plan, workspace);
+    a.out = (T*)pre_psf;
+    a.src = src;
+    if (plan.n_chunks > 1) JT_CUDA_TRY(cudaMemsetAsync(a.counter, 0, plan.counter_bytes, st));
+    return launch_trace_t<T, true>(a, plan.R, st);
+}
+
+jt_status launch_trace_grid(jt_dtype dtype, const jt_grid* g, const jt_lens* lens, const SrcSet& src,
+                            const TracePlan& plan, void* workspace, void* pre_psf, cudaStream_t st) {
+    return dtype == JT_F32 ? trace_grid_t<float>(g, lens, src, plan, workspace, pre_psf, st)
+                           : trace_grid_t<double>(g, lens, src, plan, workspace, pre_psf, st);
+}
+
+template <typename T>
+static jt_status trace_rays_t(int64_t n, const void* tx, const void* ty, const jt_lens* lens, const TracePlan& plan,
+                              void* workspace, void* bx, void* by, cudaStream_t st) {
+    TraceArgs<T> a = {};
+    a.n_rays = n;
+    a.tx = (const T*)tx; a.ty = (const T*)ty; a.bx = (T*)bx; a.by = (T*)by;
+    fill_lens(a, lens, plan, workspace);
+    if (plan.n_chunks > 1) JT_CUDA_TRY(cudaMemsetAsync(a.counter, 0, plan.counter_bytes, st));
+    return launch_trace_t<T, false>(a, plan.R, st);
+}
+
+jt_status launch_trace_rays(jt_dtype dtype, int64_t n, const void* tx, const void* ty, const jt_lens* lens,
+                            const TracePlan& plan, void* workspace, void* bx, void* by, cudaStream_t st) {
+    return dtype == JT_F32 ? trace_rays_t<float>(n, tx, ty, lens, plan, workspace, bx, by, st)
+                           : trace_rays_t<double>(n, tx, ty, lens, plan, workspace, bx, by, st);
+}
+
+// ---- step 2 on caller arrays ----
+template <typename T>
+__global__ void __launch_bounds__(256) k_source(int64_t n, const T* __restrict__ bx, const T* __restrict__ by,
+                                                const __grid_constant__ SrcSet src, T* __restrict__ flux) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        flux[i] = (T)sersic_sum<T>(src, (double)bx[i], (double)by[i]);
+}
+
+jt_status launch_source_brightness(jt_dtype dtype, int64_t n, const void* bx, const void* by, const SrcSet& src,
+                                   void* flux, cudaStream_t st) {
+    if (n == 0) return JT_OK;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks > (int64_t)kNumSMs * 32) blocks = (int64_t)kNumSMs * 32;
+    if (dtype == JT_F32)
+        k_source<float><<<(unsigned)blocks, 256, 0, st>>>(n, (const float*)bx, (const float*)by, src, (float*)flux);
+    else
+        k_source<double><<<(unsigned)blocks, 256, 0, st>>>(n, (const double*)bx, (const double*)by, src, (double*)flux);
+    JT_LAUNCH_CHECK();
+    return JT_OK;
+}
+
+}  // namespace jt

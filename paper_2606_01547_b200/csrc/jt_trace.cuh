@@ -1,0 +1,275 @@
+// jt_trace.cuh -- the ray-tracing kernel: steps 1-4 of the hot path.
+//
+//   GRID mode  (jt_simulate_image): observer grid G generated in registers -> subhalo sum (definition T)
+//              -> SIE + shear (S, H) -> lens equation -> Sersic (R) -> s x s binning with warp shuffles (B)
+//              -> pre-PSF image.  Traced coordinates never leave the chip (PAPER.md:55 steps 1+2 fused).
+//   RAYS mode  (jt_ray_shoot): same subhalo sum + SIE + shear on caller-supplied ray positions -> beta.
+//
+// N-body-style structure (PAPER.md:47 is where the time goes): 256 threads, each owning R rays whose
+// deflection accumulators live in registers; the subhalo list streams through shared memory in tiles
+// of 256 derived records (SubRec, built in double by the staging threads).  Per record a warp takes the
+// logarithm-free far-field form when all of its rays have X^2 >= max(10, 3 tau^2) (>98 % of the
+// pairs in the paper-shaped workloads) and a per-ray generic form otherwise.
+// When there are too few ray tiles to fill 148 SMs the subhalo list is split into chunks; every
+// (tile, chunk) CTA writes double partial sums to the workspace and the last CTA to arrive for a tile
+// adds them in chunk order (deterministic) and runs the epilogue.
+#pragma once
+#include "jt_internal.h"
+
+namespace jt {
+
+template <typename T>
+struct TraceArgs {
+    // grid mode geometry (definition G)
+    int nx, ny, s, NX, NY;
+    double h, x0, y0, area_over_s2;
+    int cols_per_warp, tiles_x;
+    // ray mode
+    int64_t n_rays;
+    const T *tx, *ty;
+    T *bx, *by;
+    // lens
+    MacroLens m;
+    int64_t M;
+    const T* tn[5];
+    int n_chunks;
+    int64_t chunk_len, n_tiles;
+    double2* partial;
+    unsigned int* counter;
+    // grid mode output
+    T* out;
+    SrcSet src;
+};
+
+// near/mid evaluation for the float kernel: coordinates re-derived in double so that dx, dy are exact
+// where they matter; closed form in float for X^2 >= 1/4, double from the raw parameters below that.
+template <typename T>
+__device__ __noinline__ double2 tnfw_slow_f32(double xd, double yd, float cx, float cy, float iRs2, float t, float c1,
+                                              float amp, float tm1, int64_t j, const T* const* tn) {
+    const double dx = xd - (double)cx, dy = yd - (double)cy;
+    const double R2 = dx * dx + dy * dy;
+    double f;
+    if (R2 * (double)iRs2 >= 0.25) {
+        f = (double)tnfw_mid<float>((float)R2, iRs2, t, c1, amp, tm1);
+    } else {
+        const SubRec<double> s = make_rec<double>((double)tn[0][j], (double)tn[1][j], (double)tn[2][j],
+                                                  (double)tn[3][j], (double)tn[4][j]);
+        f = tnfw_any(R2, s);
+    }
+    return make_double2(f * dx, f * dy);
+}
+
+template <typename T, int R, bool GRID>
+__global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__ TraceArgs<T> a) {
+    __shared__ SubRec<T> recs[kSubTile];
+    __shared__ int s_last;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t tile = (int64_t)blockIdx.x / a.n_chunks;
+    const int chunk = (int)((int64_t)blockIdx.x % a.n_chunks);
+
+    // ---- ray ownership ----
+    int I = 0, J0 = 0;               // grid mode: column and first row of this thread's R rays
+    int64_t idx0 = 0;                // ray mode: first ray index (stride 256)
+    T xs[R], ys[R];
+    if constexpr (GRID) {
+        const int txi = (int)(tile % a.tiles_x), tyi = (int)(tile / a.tiles_x);
+        I = (txi * 2 + (warp & 1)) * a.cols_per_warp + lane;
+        J0 = (tyi * 4 + (warp >> 1)) * R;
+        const int Ic = min(I, a.NX - 1);
+        const T x = (T)fma((double)Ic, a.h, a.x0);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            xs[r] = x;
+            ys[r] = (T)fma((double)min(J0 + r, a.NY - 1), a.h, a.y0);
+        }
+    } else {
+        idx0 = tile * (int64_t)(R * kTraceThreads) + tid;
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = min(idx0 + (int64_t)r * kTraceThreads, a.n_rays - 1);
+            xs[r] = a.tx[i];
+            ys[r] = a.ty[i];
+        }
+    }
+
+    double axd[R], ayd[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
+
+    // ---- subhalo sum over this CTA's chunk ----
+    const int64_t j_begin = (int64_t)chunk * a.chunk_len;
+    const int64_t j_end = min(a.M, j_begin + a.chunk_len);
+    for (int64_t base = j_begin; base < j_end; base += kSubTile) {
+        __syncthreads();
+        {
+            const int64_t j = base + tid;
+            recs[tid] = (j < j_end) ? make_rec<T>((double)a.tn[0][j], (double)a.tn[1][j], (double)a.tn[2][j],
+                                                  (double)a.tn[3][j], (double)a.tn[4][j])
+                                    : null_rec<T>();
+        }
+        __syncthreads();
+        const int count = (int)min((int64_t)kSubTile, j_end - base);
+
+        T ax[R], ay[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) { ax[r] = (T)0; ay[r] = (T)0; }
+
+#pragma unroll 1
+        for (int jj = 0; jj < count; ++jj) {
+            const SubRec<T> s = recs[jj];
+            T dx[R], dy[R], R2[R];
+            T R2min;
+            if constexpr (GRID) {
+                const T d = xs[0] - s.cx, d2 = d * d;
+#pragma unroll
+                for (int r = 0; r < R; ++r) { dx[r] = d; dy[r] = ys[r] - s.cy; R2[r] = fma(dy[r], dy[r], d2); }
+                // rows ascend in y: the closest row bounds the whole column
+                const T m = fmax(fmax(ys[0] - s.cy, s.cy - ys[R - 1]), (T)0);
+                R2min = fma(m, m, d2);
+            } else {
+                R2min = (T)3.0e38;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    dx[r] = xs[r] - s.cx; dy[r] = ys[r] - s.cy;
+                    R2[r] = fma(dy[r], dy[r], dx[r] * dx[r]);
+                    R2min = fmin(R2min, R2[r]);
+                }
+            }
+            const bool far = R2min * s.iRs2 >= s.thr;
+            if (__all_sync(0xffffffffu, far)) {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const T f = tnfw_far<T>(R2[r], s);
+                    ax[r] = fma(f, dx[r], ax[r]);
+                    ay[r] = fma(f, dy[r], ay[r]);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    if constexpr (sizeof(T) == 8) {
+                        const T f = (R2[r] * s.iRs2 >= s.thr) ? tnfw_far<T>(R2[r], s) : (T)tnfw_any((double)R2[r], *(const SubRec<double>*)&s);
+                        ax[r] = fma(f, dx[r], ax[r]);
+                        ay[r] = fma(f, dy[r], ay[r]);
+                    } else {
+                        double xd, yd;
+                        if constexpr (GRID) {
+                            xd = fma((double)min(I, a.NX - 1), a.h, a.x0);
+                            yd = fma((double)min(J0 + r, a.NY - 1), a.h, a.y0);
+                        } else {
+                            xd = (double)xs[r]; yd = (double)ys[r];
+                        }
+                        const double2 c = tnfw_slow_f32<T>(xd, yd, s.cx, s.cy, s.iRs2, s.t, s.c1, s.amp, s.tm1,
+                                                           base + jj, a.tn);
+                        axd[r] += c.x; ayd[r] += c.y;
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) { axd[r] += (double)ax[r]; ayd[r] += (double)ay[r]; }
+    }
+
+    // ---- split subhalo list: publish partial sums; the last CTA of the tile reduces them in chunk order ----
+    if (a.n_chunks > 1) {
+        const int64_t slot0 = ((int64_t)chunk * a.n_tiles + tile) * R;
+#pragma unroll
+        for (int r = 0; r < R; ++r)
+            __stcg(&a.partial[(slot0 + r) * kTraceThreads + tid], make_double2(axd[r], ayd[r]));
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            const unsigned int old = atomicAdd(&a.counter[tile], 1u);
+            s_last = (old == (unsigned int)(a.n_chunks - 1));
+        }
+        __syncthreads();
+        if (!s_last) return;
+        __threadfence();
+#pragma unroll
+        for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
+        for (int c = 0; c < a.n_chunks; ++c) {
+            const int64_t s0 = ((int64_t)c * a.n_tiles + tile) * R;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const double2 v = __ldcg(&a.partial[(s0 + r) * kTraceThreads + tid]);
+                axd[r] += v.x; ayd[r] += v.y;
+            }
+        }
+        if (tid == 0) a.counter[tile] = 0u;     // leave the counter clean for the next call
+    }
+
+    // ---- epilogue: O(rays) work in double ----
+    double sx[R], sy[R];                        // dynamically indexed below -> local memory, once per ray
+#pragma unroll
+    for (int r = 0; r < R; ++r) { sx[r] = axd[r]; sy[r] = ayd[r]; }
+
+    if constexpr (GRID) {
+        const double xd = fma((double)min(I, a.NX - 1), a.h, a.x0);
+        const int seg = lane - lane % a.s;
+        const bool writer = (lane % a.s == 0) && (lane < a.cols_per_warp) && (I < a.NX);
+        const int ip = I / a.s;
+        double acc = 0.0;
+        int sub = 0;
+#pragma unroll 1
+        for (int r = 0; r < R; ++r) {
+            const int J = J0 + r;
+            const double yd = fma((double)min(J, a.NY - 1), a.h, a.y0);
+            double mx, my;
+            macro_alpha(a.m, xd, yd, mx, my);
+            const double bx = xd - mx - sx[r], by = yd - my - sy[r];
+            acc += sersic_sum<T>(a.src, bx, by);
+            if (++sub == a.s) {
+                // B: s adjacent lanes hold the s sub-columns of one pixel -> segmented shuffle sum
+                double tot = 0.0;
+                for (int d = 0; d < a.s; ++d) tot += __shfl_sync(0xffffffffu, acc, seg + d);
+                if (writer && J < a.NY) a.out[(int64_t)(J / a.s) * a.nx + ip] = (T)(tot * a.area_over_s2);
+                acc = 0.0;
+                sub = 0;
+            }
+        }
+    } else {
+#pragma unroll 1
+        for (int r = 0; r < R; ++r) {
+            const int64_t i = idx0 + (int64_t)r * kTraceThreads;
+            if (i < a.n_rays) {
+                const double xd = (double)a.tx[i], yd = (double)a.ty[i];
+                double mx, my;
+                macro_alpha(a.m, xd, yd, mx, my);
+                a.bx[i] = (T)(xd - mx - sx[r]);
+                a.by[i] = (T)(yd - my - sy[r]);
+            }
+        }
+    }
+}
+
+// host launcher for one (T, GRID) pair; instantiated in jt_trace_f32.cu / jt_trace_f64.cu
+template <typename T, bool GRID>
+jt_status launch_trace_t(const TraceArgs<T>& a, int R, cudaStream_t st);
+
+#define JT_TRACE_CASE(RR)                                                                         \
+    case RR:                                                                                      \
+        k_trace<T, RR, GRID><<<(unsigned)grid, kTraceThreads, 0, st>>>(a);                        \
+        break;
+
+template <typename T, bool GRID>
+jt_status launch_trace_impl(const TraceArgs<T>& a, int R, cudaStream_t st) {
+    const int64_t grid = a.n_tiles * a.n_chunks;
+    if (grid <= 0) return JT_OK;
+    if (grid > 0x7fffffffLL) return JT_ERR_UNSUPPORTED;
+    if constexpr (GRID) {
+        switch (R) {
+            JT_TRACE_CASE(5) JT_TRACE_CASE(6) JT_TRACE_CASE(7) JT_TRACE_CASE(8) JT_TRACE_CASE(9) JT_TRACE_CASE(10) JT_TRACE_CASE(11)
+            JT_TRACE_CASE(12) JT_TRACE_CASE(13) JT_TRACE_CASE(14) JT_TRACE_CASE(15) JT_TRACE_CASE(16)
+            default: return JT_ERR_UNSUPPORTED;
+        }
+    } else {
+        switch (R) {
+            JT_TRACE_CASE(8)
+            default: return JT_ERR_UNSUPPORTED;
+        }
+    }
+    JT_LAUNCH_CHECK();
+    return JT_OK;
+}
+
+}  // namespace jt

@@ -1,0 +1,81 @@
+"""Host-side checks that need no GPU: libjt.so builds, loads, exports every symbol include/jt.h declares,
+and rejects bad arguments before touching the device (error behaviour documented in include/jt.h)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "jt.h")).read()
+    return sorted(set(re.findall(r"JT_API[^;(]*?\b(jt_[a-z_]+)\s*\(", src)))
+
+
+def test_header_symbols_exported(jt):
+    names = _declared()
+    assert len(names) == 11, names
+    L = ctypes.CDLL(jt.lib_path())
+    for n in names:
+        assert hasattr(L, n), n
+    assert jt.version() == 100
+
+
+def test_status_strings(jt):
+    L = jt.lib()
+    assert L.jt_status_string(0) == b"JT_OK" and L.jt_status_string(3) == b"JT_ERR_WORKSPACE"
+
+
+def test_argument_validation_without_device(jt):
+    from paper_2606_01547_b200 import binding as b
+    L = jt.lib()
+    g = b._Grid(10, 10, 0.05, 0.0, 0.0, 1)
+    lens = b._Lens()
+    S, keep = b._sources([[1, 0.2, 1.0, 0, 0, 0, 0]])
+    dummy = ctypes.c_void_p(256)
+    # unknown dtype / method
+    assert L.jt_simulate_image(7, ctypes.byref(g), ctypes.byref(lens), ctypes.byref(S), 0, 0, None, 0, None, 0, dummy, None) == 2
+    assert L.jt_psf_convolve(0, 8, 8, dummy, 3, 3, dummy, 9, None, 0, ctypes.c_void_p(512), None) == 2
+    # even kernel, null pointers, aliasing, bad grid
+    assert L.jt_psf_convolve(0, 8, 8, dummy, 4, 3, dummy, 1, None, 0, ctypes.c_void_p(512), None) == 1
+    assert L.jt_psf_convolve(0, 8, 8, None, 3, 3, dummy, 1, None, 0, ctypes.c_void_p(512), None) == 1
+    assert L.jt_psf_convolve(0, 8, 8, dummy, 3, 3, dummy, 1, None, 0, dummy, None) == 1
+    bad = b._Grid(10, 10, -1.0, 0.0, 0.0, 1)
+    assert L.jt_simulate_image(0, ctypes.byref(bad), ctypes.byref(lens), ctypes.byref(S), 0, 0, None, 0, None, 0, dummy, None) == 1
+    bad = b._Grid(10, 10, 0.05, 0.0, 0.0, 17)
+    assert L.jt_simulate_image(0, ctypes.byref(bad), ctypes.byref(lens), ctypes.byref(S), 0, 0, None, 0, None, 0, dummy, None) == 1
+    lens.n_tnfw = 5          # subhalos announced but no arrays
+    assert L.jt_ray_shoot(1, 10, dummy, dummy, ctypes.byref(lens), None, 0, ctypes.c_void_p(512), ctypes.c_void_p(768), None) == 1
+    lens.n_tnfw = 0
+    assert L.jt_ray_shoot(1, -1, dummy, dummy, ctypes.byref(lens), None, 0, ctypes.c_void_p(512), ctypes.c_void_p(768), None) == 1
+    # workspace too small: direct conv needs scratch for the flipped kernel
+    need = L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 1)
+    assert need >= 21 * 21 * 8
+    assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 1, dummy, need - 1, ctypes.c_void_p(512), None) == 3
+    # zero-sized problems are no-ops
+    assert L.jt_ray_shoot(1, 0, None, None, ctypes.byref(lens), None, 0, None, None, None) == 0
+    del keep
+
+
+def test_workspace_queries_are_consistent(jt):
+    g = jt.Grid(200, 200, 0.04, supersample=2)
+    big = jt.simulate_image_workspace_bytes("f32", g, 10000, 21, 21, "direct")
+    small = jt.simulate_image_workspace_bytes("f32", g, 0, 21, 21, "direct")
+    assert big > small >= 200 * 200 * 4
+    assert jt.ray_shoot_workspace_bytes("f64", 10 ** 7, 100) == 0        # enough ray tiles: no split, no scratch
+    assert jt.ray_shoot_workspace_bytes("f64", 1000, 10 ** 5) > 0
+
+
+def test_no_cpu_fallback_without_device(jt):
+    """On a box without a CUDA device a compute call must fail (JT_ERR_CUDA / UNSUPPORTED), never compute."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA device present")
+    from paper_2606_01547_b200 import binding as b
+    L = jt.lib()
+    lens = b._Lens()
+    st = L.jt_ray_shoot(1, 4, ctypes.c_void_p(256), ctypes.c_void_p(512), ctypes.byref(lens), None, 0,
+                        ctypes.c_void_p(768), ctypes.c_void_p(1024), None)
+    assert st in (2, 4)
