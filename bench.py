@@ -1,0 +1,427 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the lensed-image hot path on B200, one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C2-f64] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A step is ONE pass of the whole hot path (grid -> ray-shoot through every deflector -> Sersic -> bin ->
+PSF convolution) through jt_simulate_image (single systems) or
+jt_simulate_batch (C3) on seeded synthetic inputs (workloads/).
+`value` = ray x deflector evaluations per second, inputs resident in HBM (BASELINE.json:metric);
+`e2e`   = the same with the step's inputs copied from pinned host memory and the image copied back,
+          both inside the timed region;
+`roofline` = the dominant kernel (the ray-tracing kernel) against the issue-limited ALU peak derived in
+          DESIGN.md "Rooflines", its duration measured live with CUDA events recorded by the library on
+          the launch stream (jt_profile_enable);
+`cpu_baseline` = the oracle, as it stands, on this box's host cores on a bounded sample of the same workload.
+With N > 1 every rank runs its own replica of the workload (replicas only, no
+collective on the data path); the time is the max over ranks and the value the sum of the units.
+`--impl reference` times the oracle instead (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ray_deflector_evals_per_s"
+UNIT = "evals/s"
+SM_COUNT = 148
+# Instructions per evaluation that the formulation needs on the issue port (DESIGN.md "Rooflines":
+# counted in the SASS of the warp-uniform far-field branch, profiles/r01_sass_counts.md).
+ALG_INSTR_PER_EVAL = {"f32": 37.5, "f64": 63.0}
+WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
+
+
+# ------------------------------------------------------------------ distributed plumbing
+def dist_init(n_gpus, backend=None):
+    """Returns (rank, world, local_rank).  Single process when WORLD_SIZE is unset."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world == 1:
+        return 0, 1, 0
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    if backend is None:
+        import torch
+        backend = "nccl" if torch.cuda.is_available() else "gloo"
+    if not dist.is_initialized():
+        dist.init_process_group(backend=backend)
+    return dist.get_rank(), dist.get_world_size(), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+def aggregate(units_local, ms_local, device=None):
+    """Whole-job numbers: (sum of units over ranks, max of time over ranks).  No data-path collective exists;
+    this is the only communication of the run."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return float(units_local), float(ms_local)
+    dev = device if device is not None else ("cuda" if dist.get_backend() == "nccl" else "cpu")
+    u = torch.tensor([float(units_local)], dtype=torch.float64, device=dev)
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=dev)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(u.item()), float(t.item())
+
+
+def barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.barrier()
+
+
+def shard_range(n, rank, world):
+    """Contiguous, balanced [lo, hi) share of n independent units (systems of a batch) for `rank`."""
+    base, rem = divmod(n, world)
+    lo = rank * base + min(rank, rem)
+    return lo, lo + base + (1 if rank < rem else 0)
+
+
+# ------------------------------------------------------------------ clocks
+class ClockSampler:
+    """nvidia-smi clocks/throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])), mx.append(float(f[1])), pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        # samples under load = upper half of the clock samples (idle samples precede the first launch)
+        return {"sm_mhz": float(np.median(sm)), "sm_mhz_max_seen": float(max(sm)), "sm_max_mhz": float(max(mx)),
+                "power_w_max": float(max(pw)), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------ workloads
+def make_workload(name, rank=0):
+    """BASELINE.json:configs[i] by name ("C2-f64", ...).  Rank r > 0 gets the same recipe with seed + r
+    (an independent replica of the same shape)."""
+    import workloads
+    cfg, dtype = name.split("-")
+    mk = {"C0": workloads.config_c0, "C1": workloads.config_c1, "C2": workloads.config_c2,
+          "C3": workloads.config_c3, "C4": workloads.config_c4}[cfg]
+    return mk(dtype=dtype, seed_offset=7919 * rank)
+
+
+def describe(name, w, world):
+    d = {"workload": name, "grid": "%dx%d" % (w.nx, w.ny), "pixel_scale": w.pixel_scale,
+         "supersample": w.supersample, "n_tnfw": w.n_tnfw, "psf": "%dx%d" % w.psf.shape[-2:],
+         "evals_per_step_per_gpu": int(w.evals), "l2": "256 MiB buffer rewritten between timed steps",
+         "parallelism": "replicas x%d (no data-path collective)" % world}
+    if hasattr(w, "B"):
+        d["batch"] = w.B
+    return d
+
+
+class ImageRunner:
+    """One lens system through jt_simulate_image; device buffers, workspace and output allocated once."""
+
+    def __init__(self, jt, w, method="auto"):
+        import torch
+        self.jt, self.w, self.method = jt, w, method
+        self.tdt = torch.float32 if w.dtype == "f32" else torch.float64
+        self.grid = jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample)
+        # pinned host copies (e2e leg) and resident device copies (device-timed leg)
+        self.h_tnfw = torch.as_tensor(np.ascontiguousarray(w.tnfw), dtype=self.tdt).pin_memory()
+        self.h_psf = torch.as_tensor(np.ascontiguousarray(w.psf), dtype=self.tdt).pin_memory()
+        self.d_tnfw = self.h_tnfw.to("cuda")
+        self.d_psf = self.h_psf.to("cuda")
+        self.out = torch.empty((w.ny, w.nx), dtype=self.tdt, device="cuda")
+        self.h_out = torch.empty((w.ny, w.nx), dtype=self.tdt).pin_memory()
+        nb = jt.simulate_image_workspace_bytes(w.dtype, self.grid, w.n_tnfw, w.psf.shape[0], w.psf.shape[1], method)
+        self.ws = torch.empty(max(nb, 1), dtype=torch.uint8, device="cuda")
+        self.h2d = self.h_tnfw.numel() * self.h_tnfw.element_size() + self.h_psf.numel() * self.h_psf.element_size()
+        self.d2h = self.h_out.numel() * self.h_out.element_size()
+        self.images = 1
+
+    def step(self):
+        tn = self.d_tnfw if self.w.n_tnfw > 0 else None
+        self.jt.simulate_image(self.grid, self.w.sie, self.w.shear, tn, self.w.sources, self.d_psf,
+                               dtype=self.w.dtype, method=self.method, workspace=self.ws, out=self.out)
+
+    def step_e2e(self):
+        self.d_tnfw.copy_(self.h_tnfw, non_blocking=True)
+        self.d_psf.copy_(self.h_psf, non_blocking=True)
+        self.step()
+        self.h_out.copy_(self.out, non_blocking=True)
+
+
+class BatchRunner:
+    """B independent systems through jt_simulate_batch (C3)."""
+
+    def __init__(self, jt, w):
+        import torch
+        self.jt, self.w = jt, w
+        self.tdt = torch.float32 if w.dtype == "f32" else torch.float64
+        self.grid = jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample)
+        pin = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=self.tdt).pin_memory()
+        self.h = [pin(w.sie), pin(w.shear), pin(w.tnfw), pin(w.sources), pin(w.psf)]
+        self.d = [t.to("cuda") for t in self.h]
+        self.out = torch.empty((w.B, w.ny, w.nx), dtype=self.tdt, device="cuda")
+        self.h_out = torch.empty((w.B, w.ny, w.nx), dtype=self.tdt).pin_memory()
+        self.h2d = sum(t.numel() * t.element_size() for t in self.h)
+        self.d2h = self.h_out.numel() * self.h_out.element_size()
+        self.images = w.B
+
+    def step(self):
+        self.jt.simulate_batch(self.grid, *self.d, out=self.out)
+
+    def step_e2e(self):
+        for d, h in zip(self.d, self.h):
+            d.copy_(h, non_blocking=True)
+        self.step()
+        self.h_out.copy_(self.out, non_blocking=True)
+
+
+# ------------------------------------------------------------------ the oracle on the host cores
+def oracle_sample(w, target_evals=2.0e8):
+    """A bounded sample of the workload for the CPU oracle: pixel rows spread evenly over the image (single
+    systems) or the first systems of the batch, sized to about target_evals ray x deflector evaluations."""
+    if hasattr(w, "B"):
+        per = w.n_rays * (w.n_tnfw + 2)
+        n = int(max(1, min(w.B, round(target_evals / per))))
+        return {"kind": "systems", "systems": list(range(n)), "evals": n * per,
+                "text": "first %d of %d systems, whole pipeline" % (n, w.B)}
+    per_row = w.nx * w.supersample ** 2 * w.n_deflectors
+    n = int(max(1, min(w.ny, round(target_evals / per_row))))
+    rows = sorted(set(int(round(x)) for x in np.linspace(0, w.ny - 1, n)))
+    return {"kind": "rows", "rows": rows, "evals": len(rows) * per_row,
+            "text": "%d of %d pixel rows (all %d deflectors, all sub-rays) + one full-size %dx%d direct convolution"
+                    % (len(rows), w.ny, w.n_deflectors, w.psf.shape[0], w.psf.shape[1])}
+
+
+def oracle_step(orc, w, sample):
+    """One pass of the oracle over the sample; returns seconds."""
+    t0 = time.perf_counter()
+    if sample["kind"] == "systems":
+        orc.simulate_batch(w, systems=sample["systems"])
+    else:
+        img = np.zeros((w.ny, w.nx))
+        for j in sample["rows"]:
+            img[j] = orc.prepsf_rows(w, j, j + 1)[0]
+        orc.convolve(img, w.psf)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline(w, target_evals):
+    import oracle as orc
+    orc.build()
+    cores = len(os.sched_getaffinity(0))
+    orc.set_threads(cores)
+    sample = oracle_sample(w, target_evals)
+    sec = oracle_step(orc, w, sample)
+    return {"value": sample["evals"] / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": sample["text"], "seconds": sec}
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle, as it stands, on this box's host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    w = make_workload(args.workload, 0)
+    import oracle as orc
+    orc.build()
+    cores = len(os.sched_getaffinity(0))
+    orc.set_threads(cores)
+    sample = oracle_sample(w, args.ref_evals)
+    for _ in range(args.warmup):
+        oracle_step(orc, w, sample)
+    secs = [oracle_step(orc, w, sample) for _ in range(args.steps)]
+    total = sum(secs)
+    value = sample["evals"] * args.steps / total
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": describe(args.workload, w, 1),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample["text"]},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------ our arm
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    import paper_2606_01547_b200 as jt
+    jt.lib()
+
+    w = make_workload(args.workload, rank)
+    batch = hasattr(w, "B")
+    runner = BatchRunner(jt, w) if batch else ImageRunner(jt, w, args.method)
+    flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")     # 256 MiB > 126 MB L2
+
+    # ---- device-timed leg (inputs resident) ----
+    jt.profile_enable(True)
+    for _ in range(args.warmup):
+        runner.step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
+    if sampler:
+        sampler.start()
+        time.sleep(0.25)
+    barrier()
+    torch.cuda.synchronize()
+    launches0 = jt.kernel_launches()
+
+    phase = []
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for a, b in ev:
+        flush.add_(1)
+        a.record()
+        runner.step()
+        b.record()
+        if not batch:
+            phase.append(jt.profile_read())          # waits for this step's events only
+    torch.cuda.synchronize()
+    barrier()
+    launches = jt.kernel_launches() - launches0
+    ms = [a.elapsed_time(b) for a, b in ev]
+    clocks = sampler.stop() if sampler else None
+    jt.profile_enable(False)
+    ms_total_local = float(sum(ms))
+    units, ms_total = aggregate(w.evals * args.steps, ms_total_local)
+
+    # ---- end-to-end leg (pinned host inputs -> device -> image back on the host), wall clock around a sync ----
+    for _ in range(max(1, args.warmup)):
+        runner.step_e2e()
+    torch.cuda.synchronize()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        runner.step_e2e()
+        torch.cuda.synchronize()
+    e2e_ms_local = 1e3 * (time.perf_counter() - t0)
+    barrier()
+    e2e_units, e2e_ms = aggregate(w.evals * args.steps, e2e_ms_local)
+
+    if rank != 0:
+        return
+    peaks, peak_kind = load_peaks()
+    value = units / (ms_total * 1e-3)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
+            "config": describe(args.workload, w, world),
+            "images_per_s": world * runner.images * args.steps / (ms_total * 1e-3),
+            "clocks": clocks,
+            "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": runner.h2d,
+                    "d2h_bytes_per_step": runner.d2h, "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": int(launches)}
+
+    # ---- roofline of the dominant kernel: the ray-tracing kernel, issue-limited ALU peak ----
+    f_mhz = (clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
+    peak_tinstr = SM_COUNT * 4 * 32 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+    if phase:
+        trace_ms = float(np.mean([p[0] for p in phase]))
+        conv_ms = float(np.mean([p[1] for p in phase]))
+    else:
+        trace_ms, conv_ms = ms_total_local / args.steps, 0.0
+    n_alg = ALG_INSTR_PER_EVAL[w.dtype]
+    achieved = w.evals * n_alg / (trace_ms * 1e-3) / 1e12
+    line["roofline"] = {
+        "bound": "alu", "kernel": "k_batch" if batch else "k_trace", "achieved": achieved, "peak": peak_tinstr,
+        "unit": "Tinstr/s", "frac": achieved / peak_tinstr, "traffic": None,
+        "peak_kind": "derived: 148 SMs x 4 schedulers x 32 lanes x %.0f MHz (max clock, %s)" % (
+            peaks.get("sm_max_mhz", 1965.0), peak_kind),
+        "alg_instr_per_eval": n_alg, "kernel_ms": trace_ms, "conv_ms": conv_ms,
+        "kernel_share_of_step": trace_ms / (ms_total_local / args.steps),
+        "frac_at_observed_clock": achieved / (SM_COUNT * 4 * 32 * f_mhz * 1e6 / 1e12),
+        "evals_per_s_kernel": w.evals / (trace_ms * 1e-3)}
+    if not batch:
+        K = w.psf.shape[0] * w.psf.shape[1]
+        esz = 4 if w.dtype == "f32" else 8
+        lanes = 128 if w.dtype == "f32" else 64
+        fma_peak = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6
+        line["conv"] = {"method": args.method, "ms": conv_ms,
+                        "gbs": (2 * w.nx * w.ny + K) * esz / (conv_ms * 1e-3) / 1e9 if conv_ms > 0 else None,
+                        "fma_frac": w.nx * w.ny * K / (conv_ms * 1e-3) / fma_peak if conv_ms > 0 else None}
+    if not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(w, args.cpu_evals)
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C2-f64", choices=WORKLOADS)
+    ap.add_argument("--method", default="auto", choices=["auto", "direct", "fft"])
+    ap.add_argument("--cpu-evals", type=float, default=1.5e9, help="oracle sample size for cpu_baseline")
+    ap.add_argument("--ref-evals", type=float, default=2.0e8, help="oracle sample size per --impl reference step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank, world, local_rank = dist_init(args.gpus)
+    try:
+        if args.impl == "reference":
+            run_reference(args, rank, world)
+        else:
+            run_ours(args, rank, world, local_rank)
+    finally:
+        import torch.distributed as dist
+        if dist.is_available() and dist.is_initialized():
+            dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

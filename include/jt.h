@@ -144,6 +144,20 @@ typedef struct {
 JT_API jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid *grid, const jt_batch_params *params,
                             void *out, void *stream);
 
+/* Measurement aid (bench.py's roofline leg).  jt_profile_enable(1) makes every following
+ * jt_simulate_image call on this host thread record CUDA events on its stream before the ray-tracing
+ * kernel, between it and the convolution, and after the convolution (three cudaEventRecord calls, no
+ * synchronisation).  jt_profile_read waits for the events of the LAST such call and returns the two
+ * intervals in milliseconds (conv_ms = 0 when the call had no PSF).  JT_ERR_INVALID_VALUE when profiling is
+ * off or no call has been recorded.  The events are the only state the library keeps; jt_profile_enable(0)
+ * destroys them. */
+JT_API jt_status jt_profile_enable(int on);
+JT_API jt_status jt_profile_read(float *trace_ms, float *conv_ms);
+
+/* Number of CUDA kernels this library has launched from the calling host thread since it was loaded
+ * (bench.py's "gpu_launches" claim; memsets and event records are not counted). */
+JT_API uint64_t jt_kernel_launches(void);
+
 JT_API const char *jt_status_string(jt_status s);
 JT_API int         jt_last_cuda_error(void);     /* cudaError_t of the last JT_ERR_CUDA on this thread, else 0 */
 JT_API int         jt_version(void);             /* JT_VERSION */

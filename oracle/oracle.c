@@ -132,9 +132,15 @@ void orc_pointmass_alpha(double x, double y, double theta_E, double cx, double c
 /* ------------------------------------------------------------------ T: truncated NFW
  * rho(r) = rho0 / [x (1+x)^2] * tau^2/(tau^2+x^2), x = r/Rs, tau = r_trunc/Rs.
  * alpha_Rs = deflection at Rs of the UNtruncated NFW with the same rho0: 4 rho0 Rs^2 = alpha_Rs/(1-ln2). */
+/* F(X) = arccosh(1/X)/sqrt(1-X^2) (X<1), 1 (X=1), arccos(1/X)/sqrt(X^2-1) (X>1)   [definition T].
+ * Written with the identities arccosh(1/X) = ln((1+s)/X), s = sqrt((1-X)(1+X)), and
+ * arccos(1/X) = 2 arctan(sqrt((X-1)/(X+1))): the same function, but 1-X is exact in floating point
+ * near X = 1 whereas 1/X rounds to 1 there and the literal form loses every digit for |X-1| < 1e-8
+ * (reading Q9a; pinned against the literal definition in 40-digit mpmath at
+ * X = 1 +- 1e-3 ... 1 ulp and over 1e-6 ... 1e4 in tests/test_oracle_lens.py). */
 double orc_tnfw_F(double X) {
-    if (X < 1.0) return acosh(1.0 / X) / sqrt(1.0 - X * X);
-    if (X > 1.0) return acos(1.0 / X) / sqrt(X * X - 1.0);
+    if (X < 1.0) { const double s = sqrt((1.0 - X) * (1.0 + X)); return (log1p(s) - log(X)) / s; }
+    if (X > 1.0) return 2.0 * atan(sqrt((X - 1.0) / (X + 1.0))) / sqrt((X - 1.0) * (X + 1.0));
     return 1.0;
 }
 

@@ -8,7 +8,10 @@ from .binding import (  # noqa: F401
     Grid,
     JtError,
     lib,
+    kernel_launches,
     lib_path,
+    profile_enable,
+    profile_read,
     psf_convolve,
     psf_convolve_workspace_bytes,
     ray_shoot,

@@ -98,12 +98,32 @@ def lib():
         L.jt_simulate_image.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), ctypes.POINTER(_Lens),
                                         ctypes.POINTER(_Sources), i32, i32, vp, ctypes.c_int, vp, sz, vp, vp]
         L.jt_simulate_batch.argtypes = [ctypes.c_int, i64, ctypes.POINTER(_Grid), ctypes.POINTER(_Batch), vp, vp]
+        L.jt_kernel_launches.restype = ctypes.c_uint64
+        L.jt_profile_enable.argtypes = [ctypes.c_int]
+        L.jt_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
         _lib = L
     return _lib
 
 
 def version():
     return lib().jt_version()
+
+
+def kernel_launches():
+    """jt_kernel_launches: kernels launched by libjt from this host thread so far."""
+    return int(lib().jt_kernel_launches())
+
+
+def profile_enable(on=True):
+    """jt_profile_enable: record events around the ray-tracing and convolution phases of jt_simulate_image."""
+    _check(lib().jt_profile_enable(1 if on else 0), "jt_profile_enable")
+
+
+def profile_read():
+    """jt_profile_read: (trace_ms, conv_ms) of the last profiled jt_simulate_image call."""
+    a, b = ctypes.c_float(), ctypes.c_float()
+    _check(lib().jt_profile_read(ctypes.byref(a), ctypes.byref(b)), "jt_profile_read")
+    return a.value, b.value
 
 
 # ------------------------------------------------------------------ marshalling helpers

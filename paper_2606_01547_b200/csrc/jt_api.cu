@@ -6,6 +6,12 @@ namespace jt {
 
 static thread_local int g_last_cuda_error = 0;
 void set_last_cuda_error(int e) { g_last_cuda_error = e; }
+static thread_local uint64_t g_launches = 0;
+void count_launch() { ++g_launches; }
+
+// ---- profiling events (jt_profile_enable / jt_profile_read) ----
+struct ProfileState { bool on = false, recorded = false, had_conv = false; cudaEvent_t ev[3] = {nullptr, nullptr, nullptr}; };
+static thread_local ProfileState g_prof;
 
 static jt_status check_device() {
     int dev = 0;
@@ -69,6 +75,7 @@ const char* jt_status_string(jt_status s) {
 }
 int jt_last_cuda_error(void) { return g_last_cuda_error; }
 int jt_version(void) { return JT_VERSION; }
+uint64_t jt_kernel_launches(void) { return g_launches; }
 
 // ------------------------------------------------------------------ step 1
 size_t jt_ray_shoot_workspace_bytes(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw) {
@@ -160,12 +167,44 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
     char* ws = (char*)workspace;
     void* trace_ws = ws;
     cudaStream_t st = (cudaStream_t)stream;
-    if (!conv) return launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, out, st);
+    const bool prof = g_prof.on;
+    if (prof) { g_prof.recorded = false; JT_CUDA_TRY(cudaEventRecord(g_prof.ev[0], st)); }
+    if (!conv) {
+        s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, out, st);
+        if (s == JT_OK && prof) { JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st)); g_prof.had_conv = false; g_prof.recorded = true; }
+        return s;
+    }
     void* pre = ws + align_up(plan.total_bytes, 256);
     void* conv_ws_ptr = (char*)pre + align_up((size_t)grid->nx * grid->ny * dtype_size(dtype), 256);
     s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, pre, st);
     if (s != JT_OK) return s;
-    return conv_dispatch(dtype, grid->ny, grid->nx, pre, ky, kx, kernel, method, conv_ws_ptr, out, st);
+    if (prof) JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st));
+    s = conv_dispatch(dtype, grid->ny, grid->nx, pre, ky, kx, kernel, method, conv_ws_ptr, out, st);
+    if (s == JT_OK && prof) { JT_CUDA_TRY(cudaEventRecord(g_prof.ev[2], st)); g_prof.had_conv = true; g_prof.recorded = true; }
+    return s;
+}
+
+// ------------------------------------------------------------------ profiling
+jt_status jt_profile_enable(int on) {
+    if (on && !g_prof.on) {
+        for (int i = 0; i < 3; ++i) JT_CUDA_TRY(cudaEventCreate(&g_prof.ev[i]));
+        g_prof.on = true;
+        g_prof.recorded = false;
+    } else if (!on && g_prof.on) {
+        for (int i = 0; i < 3; ++i) { cudaEventDestroy(g_prof.ev[i]); g_prof.ev[i] = nullptr; }
+        g_prof.on = false;
+        g_prof.recorded = false;
+    }
+    return JT_OK;
+}
+
+jt_status jt_profile_read(float* trace_ms, float* conv_ms) {
+    if (!g_prof.on || !g_prof.recorded || !trace_ms || !conv_ms) return JT_ERR_INVALID_VALUE;
+    JT_CUDA_TRY(cudaEventSynchronize(g_prof.ev[g_prof.had_conv ? 2 : 1]));
+    JT_CUDA_TRY(cudaEventElapsedTime(trace_ms, g_prof.ev[0], g_prof.ev[1]));
+    *conv_ms = 0.f;
+    if (g_prof.had_conv) JT_CUDA_TRY(cudaEventElapsedTime(conv_ms, g_prof.ev[1], g_prof.ev[2]));
+    return JT_OK;
 }
 
 // ------------------------------------------------------------------ batch

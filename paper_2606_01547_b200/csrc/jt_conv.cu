@@ -6,7 +6,7 @@
 // register window of OY tile values down the column, so one shared-memory load (lanes on consecutive
 // addresses: conflict-free) feeds OY FMAs; kernel taps are warp-uniform vector loads from a flipped,
 // column-major copy (Kc[b][a], built by k_flip_kernel in the workspace).  FMA : LDS = OY : 1.25.
-#include "jt_internal.h"
+#include "jt_conv.cuh"
 
 namespace jt {
 
@@ -16,23 +16,6 @@ __global__ void k_flip_kernel(int ky, int kx, int kyp, const T* __restrict__ K, 
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const int b = i / kyp, a = i % kyp;
         Kc[i] = (a < ky) ? K[(size_t)(ky - 1 - a) * kx + (kx - 1 - b)] : (T)0;
-    }
-}
-
-template <typename T, int OY>
-__device__ __forceinline__ void load_taps(const T* __restrict__ p, T (&kv)[OY]) {
-    if constexpr (sizeof(T) == 4) {
-#pragma unroll
-        for (int i = 0; i < OY; i += 4) {
-            const float4 v = __ldg(reinterpret_cast<const float4*>(p + i));
-            kv[i] = v.x; kv[i + 1] = v.y; kv[i + 2] = v.z; kv[i + 3] = v.w;
-        }
-    } else {
-#pragma unroll
-        for (int i = 0; i < OY; i += 2) {
-            const double2 v = __ldg(reinterpret_cast<const double2*>(p + i));
-            kv[i] = v.x; kv[i + 1] = v.y;
-        }
     }
 }
 
@@ -58,37 +41,7 @@ __global__ void __launch_bounds__(TW* NTR) k_conv_direct(int ny, int nx, const T
     T acc[OY];
 #pragma unroll
     for (int r = 0; r < OY; ++r) acc[r] = (T)0;
-
-    for (int b = 0; b < kx; ++b) {
-        const T* tcol = tile + jl0 * tws + il + b;
-        const T* kcol = Kc + (size_t)b * kyp;
-        T win[OY];
-#pragma unroll
-        for (int r = 0; r < OY - 1; ++r) win[r] = tcol[r * tws];
-        int a0 = 0;
-        for (; a0 + OY <= ky; a0 += OY) {
-            T kv[OY];
-            load_taps<T, OY>(kcol + a0, kv);
-#pragma unroll
-            for (int aa = 0; aa < OY; ++aa) {
-                win[(aa + OY - 1) % OY] = tcol[(a0 + aa + OY - 1) * tws];
-#pragma unroll
-                for (int r = 0; r < OY; ++r) acc[r] = fma(kv[aa], win[(aa + r) % OY], acc[r]);
-            }
-        }
-        if (a0 < ky) {
-            T kv[OY];
-            load_taps<T, OY>(kcol + a0, kv);       // zero-padded up to kyp
-#pragma unroll
-            for (int aa = 0; aa < OY; ++aa) {
-                if (a0 + aa < ky) {
-                    win[(aa + OY - 1) % OY] = tcol[(a0 + aa + OY - 1) * tws];
-#pragma unroll
-                    for (int r = 0; r < OY; ++r) acc[r] = fma(kv[aa], win[(aa + r) % OY], acc[r]);
-                }
-            }
-        }
-    }
+    conv_sweep<T, OY, true>(tile + jl0 * tws + il, tws, Kc, ky, kx, kyp, acc);
 
     const int i = i0 + il;
     if (i < nx) {

@@ -180,6 +180,32 @@ struct MacroLens {
     double g1, g2;
 };
 
+// definition E: (e1,e2) -> (cos phi, sin phi, q), |e| clamped to 0.9999
+__host__ __device__ inline void ellipticity(double e1, double e2, double* c, double* s, double* q) {
+    double m = sqrt(e1 * e1 + e2 * e2);
+    if (m > 0.9999) m = 0.9999;
+    const double phi = 0.5 * atan2(e2, e1);
+    *c = cos(phi);
+    *s = sin(phi);
+    *q = (1.0 - m) / (1.0 + m);
+}
+
+__host__ __device__ inline MacroLens derive_macro(int has_sie, double theta_E, double e1, double e2, double cx, double cy,
+                                                  int has_shear, double g1, double g2) {
+    MacroLens m = {};
+    m.has_sie = has_sie ? 1 : 0;
+    m.has_shear = has_shear ? 1 : 0;
+    if (m.has_sie) {
+        ellipticity(e1, e2, &m.c, &m.s, &m.q);
+        m.b = theta_E * sqrt(m.q);
+        m.f = sqrt(1.0 - m.q * m.q);
+        m.cx = cx;
+        m.cy = cy;
+    }
+    if (m.has_shear) { m.g1 = g1; m.g2 = g2; }
+    return m;
+}
+
 __device__ __forceinline__ double atanh_over(double z2) {      // atanh(z)/z as a function of z^2 in [0,1)
     if (z2 <= 0.25) return atanh_q(z2);
     const double z = sqrt(z2);
@@ -219,6 +245,18 @@ struct SrcSet {
     double c[JT_MAX_SRC], s[JT_MAX_SRC], q[JT_MAX_SRC], iq[JT_MAX_SRC], cx[JT_MAX_SRC], cy[JT_MAX_SRC];
     double amp[JT_MAX_SRC], bn[JT_MAX_SRC], p[JT_MAX_SRC], iRs2[JT_MAX_SRC];
 };
+
+__host__ __device__ inline void derive_source(SrcSet& S, int k, double amp, double R_sersic, double n_sersic, double e1,
+                                              double e2, double cx, double cy) {
+    ellipticity(e1, e2, &S.c[k], &S.s[k], &S.q[k]);
+    S.iq[k] = 1.0 / S.q[k];
+    S.cx[k] = cx;
+    S.cy[k] = cy;
+    S.amp[k] = amp;
+    S.bn[k] = 1.9992 * n_sersic - 0.3271;                 // reading Q10
+    S.p[k] = 0.5 / n_sersic;
+    S.iRs2[k] = 1.0 / (R_sersic * R_sersic);
+}
 
 template <typename T>
 __device__ __forceinline__ double sersic_sum(const SrcSet& S, double bx, double by);

@@ -14,6 +14,7 @@ constexpr int kSubTile = 256;           // subhalo records staged per shared-mem
 
 // thread-local last CUDA error (jt_last_cuda_error)
 void set_last_cuda_error(int e);
+void count_launch();
 #define JT_CUDA_TRY(expr)                                                    \
     do {                                                                     \
         cudaError_t _e = (expr);                                             \
@@ -21,6 +22,7 @@ void set_last_cuda_error(int e);
     } while (0)
 #define JT_LAUNCH_CHECK()                                                    \
     do {                                                                     \
+        jt::count_launch();                                                  \
         cudaError_t _e = cudaGetLastError();                                 \
         if (_e != cudaSuccess) { jt::set_last_cuda_error((int)_e); return JT_ERR_CUDA; } \
     } while (0)

@@ -8,29 +8,9 @@ namespace jt {
 template <typename T, bool GRID>
 jt_status launch_trace_t(const TraceArgs<T>& a, int R, cudaStream_t st);
 
-// ---- definition E on the host: (e1,e2) -> (cos phi, sin phi, q) ----
-static void ellipticity(double e1, double e2, double* c, double* s, double* q) {
-    double m = sqrt(e1 * e1 + e2 * e2);
-    if (m > 0.9999) m = 0.9999;
-    const double phi = 0.5 * atan2(e2, e1);
-    *c = cos(phi);
-    *s = sin(phi);
-    *q = (1.0 - m) / (1.0 + m);
-}
-
 MacroLens make_macro(const jt_lens* lens) {
-    MacroLens m = {};
-    m.has_sie = lens->has_sie ? 1 : 0;
-    m.has_shear = lens->has_shear ? 1 : 0;
-    if (m.has_sie) {
-        ellipticity(lens->sie_e1, lens->sie_e2, &m.c, &m.s, &m.q);
-        m.b = lens->sie_theta_E * sqrt(m.q);
-        m.f = sqrt(1.0 - m.q * m.q);
-        m.cx = lens->sie_cx;
-        m.cy = lens->sie_cy;
-    }
-    if (m.has_shear) { m.g1 = lens->shear_gamma1; m.g2 = lens->shear_gamma2; }
-    return m;
+    return derive_macro(lens->has_sie, lens->sie_theta_E, lens->sie_e1, lens->sie_e2, lens->sie_cx, lens->sie_cy,
+                        lens->has_shear, lens->shear_gamma1, lens->shear_gamma2);
 }
 
 jt_status make_sources(const jt_sources* src, SrcSet* out) {
@@ -39,16 +19,8 @@ jt_status make_sources(const jt_sources* src, SrcSet* out) {
     S.n = src->n;
     if (S.n > 0 && (!src->amp || !src->R_sersic || !src->n_sersic || !src->e1 || !src->e2 || !src->cx || !src->cy))
         return JT_ERR_INVALID_VALUE;
-    for (int k = 0; k < S.n; ++k) {
-        ellipticity(src->e1[k], src->e2[k], &S.c[k], &S.s[k], &S.q[k]);
-        S.iq[k] = 1.0 / S.q[k];
-        S.cx[k] = src->cx[k];
-        S.cy[k] = src->cy[k];
-        S.amp[k] = src->amp[k];
-        S.bn[k] = 1.9992 * src->n_sersic[k] - 0.3271;           // reading Q10
-        S.p[k] = 0.5 / src->n_sersic[k];
-        S.iRs2[k] = 1.0 / (src->R_sersic[k] * src->R_sersic[k]);
-    }
+    for (int k = 0; k < S.n; ++k)
+        derive_source(S, k, src->amp[k], src->R_sersic[k], src->n_sersic[k], src->e1[k], src->e2[k], src->cx[k], src->cy[k]);
     *out = S;
     return JT_OK;
 }

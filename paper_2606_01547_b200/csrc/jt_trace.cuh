@@ -41,22 +41,140 @@ struct TraceArgs {
     SrcSet src;
 };
 
+// raw (caller) subhalo arrays of one system: cx, cy, Rs, alpha_Rs, r_trunc
+template <typename T>
+struct RawTn { const T* p[5]; };
+
+// geometry of definition G for one thread: column I, first row J0 of its R vertically adjacent rays
+struct RayGeom {
+    double h, x0, y0;
+    int NX, NY, I, J0;
+    __device__ __forceinline__ double xd() const { return fma((double)min(I, NX - 1), h, x0); }
+    __device__ __forceinline__ double yd(int r) const { return fma((double)min(J0 + r, NY - 1), h, y0); }
+};
+
 // near/mid evaluation for the float kernel: coordinates re-derived in double so that dx, dy are exact
 // where they matter; closed form in float for X^2 >= 1/4, double from the raw parameters below that.
 template <typename T>
 __device__ __noinline__ double2 tnfw_slow_f32(double xd, double yd, float cx, float cy, float iRs2, float t, float c1,
-                                              float amp, float tm1, int64_t j, const T* const* tn) {
+                                              float amp, float tm1, int64_t j, const RawTn<T>* raw) {
     const double dx = xd - (double)cx, dy = yd - (double)cy;
     const double R2 = dx * dx + dy * dy;
     double f;
     if (R2 * (double)iRs2 >= 0.25) {
         f = (double)tnfw_mid<float>((float)R2, iRs2, t, c1, amp, tm1);
     } else {
-        const SubRec<double> s = make_rec<double>((double)tn[0][j], (double)tn[1][j], (double)tn[2][j],
-                                                  (double)tn[3][j], (double)tn[4][j]);
+        const SubRec<double> s = make_rec<double>((double)raw->p[0][j], (double)raw->p[1][j], (double)raw->p[2][j],
+                                                  (double)raw->p[3][j], (double)raw->p[4][j]);
         f = tnfw_any(R2, s);
     }
     return make_double2(f * dx, f * dy);
+}
+
+// One staged tile of `count` subhalo records against this thread's R rays: adds the tile's deflection to
+// (axd, ayd).  GRID: the R rays share one column (xs[0]) and ascend in y.
+template <typename T, int R, bool GRID>
+__device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs, int count, int64_t base,
+                                             const RawTn<T>& raw, const RayGeom& g, const T (&xs)[R], const T (&ys)[R],
+                                             double (&axd)[R], double (&ayd)[R]) {
+    T ax[R], ay[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) { ax[r] = (T)0; ay[r] = (T)0; }
+
+#pragma unroll 1
+    for (int jj = 0; jj < count; ++jj) {
+        const SubRec<T> s = recs[jj];
+        T dx[R], dy[R], R2[R];
+        T R2min;
+        if constexpr (GRID) {
+            const T d = xs[0] - s.cx, d2 = d * d;
+#pragma unroll
+            for (int r = 0; r < R; ++r) { dx[r] = d; dy[r] = ys[r] - s.cy; R2[r] = fma(dy[r], dy[r], d2); }
+            // rows ascend in y: the closest row bounds the whole column
+            const T m = fmax(fmax(ys[0] - s.cy, s.cy - ys[R - 1]), (T)0);
+            R2min = fma(m, m, d2);
+        } else {
+            R2min = (T)3.0e38;
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                dx[r] = xs[r] - s.cx; dy[r] = ys[r] - s.cy;
+                R2[r] = fma(dy[r], dy[r], dx[r] * dx[r]);
+                R2min = fmin(R2min, R2[r]);
+            }
+        }
+        const bool far = R2min * s.iRs2 >= s.thr;
+        if (__all_sync(0xffffffffu, far)) {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const T f = tnfw_far<T>(R2[r], s);
+                ax[r] = fma(f, dx[r], ax[r]);
+                ay[r] = fma(f, dy[r], ay[r]);
+            }
+        } else {
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                if constexpr (sizeof(T) == 8) {
+                    const T f = (R2[r] * s.iRs2 >= s.thr) ? tnfw_far<T>(R2[r], s) : (T)tnfw_any((double)R2[r], *(const SubRec<double>*)&s);
+                    ax[r] = fma(f, dx[r], ax[r]);
+                    ay[r] = fma(f, dy[r], ay[r]);
+                } else {
+                    double xd, yd;
+                    if constexpr (GRID) { xd = g.xd(); yd = g.yd(r); }
+                    else { xd = (double)xs[r]; yd = (double)ys[r]; }
+                    const double2 c = tnfw_slow_f32<T>(xd, yd, s.cx, s.cy, s.iRs2, s.t, s.c1, s.amp, s.tm1, base + jj, &raw);
+                    axd[r] += c.x; ayd[r] += c.y;
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) { axd[r] += (double)ax[r]; ayd[r] += (double)ay[r]; }
+}
+
+// stage one tile of derived records (in double) from the raw arrays; entries past j_end are null records
+template <typename T>
+__device__ __forceinline__ void stage_tile(SubRec<T>* recs, const RawTn<T>& raw, int64_t base, int64_t j_end, int tid,
+                                           int nthreads) {
+    for (int k = tid; k < kSubTile; k += nthreads) {
+        const int64_t j = base + k;
+        recs[k] = (j < j_end) ? make_rec<T>((double)raw.p[0][j], (double)raw.p[1][j], (double)raw.p[2][j],
+                                            (double)raw.p[3][j], (double)raw.p[4][j])
+                              : null_rec<T>();
+    }
+}
+
+// O(rays) epilogue of the grid path in double: SIE + shear, lens equation, Sersic sum, s x s binning (definition B:
+// s adjacent lanes hold the s sub-columns of a pixel -> segmented shuffle sum; each thread's R rows are a whole
+// number of pixels).  store(j_pixel, i_pixel, value) receives pixel_scale^2/s^2 * sum.
+template <typename T, int R, typename Store>
+__device__ __forceinline__ void grid_epilogue(const MacroLens& m, const SrcSet& src, const RayGeom& g, int s,
+                                              int cols_per_warp, double area_over_s2, int lane, const double (&axd)[R],
+                                              const double (&ayd)[R], Store store) {
+    double sx[R], sy[R];                        // dynamically indexed below -> local memory, once per ray
+#pragma unroll
+    for (int r = 0; r < R; ++r) { sx[r] = axd[r]; sy[r] = ayd[r]; }
+    const double xd = g.xd();
+    const int seg = lane - lane % s;
+    const bool writer = (lane % s == 0) && (lane < cols_per_warp) && (g.I < g.NX);
+    const int ip = g.I / s;
+    double acc = 0.0;
+    int sub = 0;
+#pragma unroll 1
+    for (int r = 0; r < R; ++r) {
+        const int J = g.J0 + r;
+        const double yd = g.yd(r);
+        double mx, my;
+        macro_alpha(m, xd, yd, mx, my);
+        const double bx = xd - mx - sx[r], by = yd - my - sy[r];
+        acc += sersic_sum<T>(src, bx, by);
+        if (++sub == s) {
+            double tot = 0.0;
+            for (int d = 0; d < s; ++d) tot += __shfl_sync(0xffffffffu, acc, seg + d);
+            if (writer && J < g.NY) store(J / s, ip, tot * area_over_s2);
+            acc = 0.0;
+            sub = 0;
+        }
+    }
 }
 
 template <typename T, int R, bool GRID>
@@ -69,20 +187,16 @@ __global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__
     const int chunk = (int)((int64_t)blockIdx.x % a.n_chunks);
 
     // ---- ray ownership ----
-    int I = 0, J0 = 0;               // grid mode: column and first row of this thread's R rays
+    RayGeom g = {a.h, a.x0, a.y0, a.NX, a.NY, 0, 0};
     int64_t idx0 = 0;                // ray mode: first ray index (stride 256)
     T xs[R], ys[R];
     if constexpr (GRID) {
         const int txi = (int)(tile % a.tiles_x), tyi = (int)(tile / a.tiles_x);
-        I = (txi * 2 + (warp & 1)) * a.cols_per_warp + lane;
-        J0 = (tyi * 4 + (warp >> 1)) * R;
-        const int Ic = min(I, a.NX - 1);
-        const T x = (T)fma((double)Ic, a.h, a.x0);
+        g.I = (txi * 2 + (warp & 1)) * a.cols_per_warp + lane;
+        g.J0 = (tyi * 4 + (warp >> 1)) * R;
+        const T x = (T)g.xd();
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            xs[r] = x;
-            ys[r] = (T)fma((double)min(J0 + r, a.NY - 1), a.h, a.y0);
-        }
+        for (int r = 0; r < R; ++r) { xs[r] = x; ys[r] = (T)g.yd(r); }
     } else {
         idx0 = tile * (int64_t)(R * kTraceThreads) + tid;
 #pragma unroll
@@ -98,76 +212,15 @@ __global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__
     for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
 
     // ---- subhalo sum over this CTA's chunk ----
+    const RawTn<T> raw = {{a.tn[0], a.tn[1], a.tn[2], a.tn[3], a.tn[4]}};
     const int64_t j_begin = (int64_t)chunk * a.chunk_len;
     const int64_t j_end = min(a.M, j_begin + a.chunk_len);
     for (int64_t base = j_begin; base < j_end; base += kSubTile) {
         __syncthreads();
-        {
-            const int64_t j = base + tid;
-            recs[tid] = (j < j_end) ? make_rec<T>((double)a.tn[0][j], (double)a.tn[1][j], (double)a.tn[2][j],
-                                                  (double)a.tn[3][j], (double)a.tn[4][j])
-                                    : null_rec<T>();
-        }
+        stage_tile<T>(recs, raw, base, j_end, tid, kTraceThreads);
         __syncthreads();
         const int count = (int)min((int64_t)kSubTile, j_end - base);
-
-        T ax[R], ay[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) { ax[r] = (T)0; ay[r] = (T)0; }
-
-#pragma unroll 1
-        for (int jj = 0; jj < count; ++jj) {
-            const SubRec<T> s = recs[jj];
-            T dx[R], dy[R], R2[R];
-            T R2min;
-            if constexpr (GRID) {
-                const T d = xs[0] - s.cx, d2 = d * d;
-#pragma unroll
-                for (int r = 0; r < R; ++r) { dx[r] = d; dy[r] = ys[r] - s.cy; R2[r] = fma(dy[r], dy[r], d2); }
-                // rows ascend in y: the closest row bounds the whole column
-                const T m = fmax(fmax(ys[0] - s.cy, s.cy - ys[R - 1]), (T)0);
-                R2min = fma(m, m, d2);
-            } else {
-                R2min = (T)3.0e38;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    dx[r] = xs[r] - s.cx; dy[r] = ys[r] - s.cy;
-                    R2[r] = fma(dy[r], dy[r], dx[r] * dx[r]);
-                    R2min = fmin(R2min, R2[r]);
-                }
-            }
-            const bool far = R2min * s.iRs2 >= s.thr;
-            if (__all_sync(0xffffffffu, far)) {
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const T f = tnfw_far<T>(R2[r], s);
-                    ax[r] = fma(f, dx[r], ax[r]);
-                    ay[r] = fma(f, dy[r], ay[r]);
-                }
-            } else {
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    if constexpr (sizeof(T) == 8) {
-                        const T f = (R2[r] * s.iRs2 >= s.thr) ? tnfw_far<T>(R2[r], s) : (T)tnfw_any((double)R2[r], *(const SubRec<double>*)&s);
-                        ax[r] = fma(f, dx[r], ax[r]);
-                        ay[r] = fma(f, dy[r], ay[r]);
-                    } else {
-                        double xd, yd;
-                        if constexpr (GRID) {
-                            xd = fma((double)min(I, a.NX - 1), a.h, a.x0);
-                            yd = fma((double)min(J0 + r, a.NY - 1), a.h, a.y0);
-                        } else {
-                            xd = (double)xs[r]; yd = (double)ys[r];
-                        }
-                        const double2 c = tnfw_slow_f32<T>(xd, yd, s.cx, s.cy, s.iRs2, s.t, s.c1, s.amp, s.tm1,
-                                                           base + jj, a.tn);
-                        axd[r] += c.x; ayd[r] += c.y;
-                    }
-                }
-            }
-        }
-#pragma unroll
-        for (int r = 0; r < R; ++r) { axd[r] += (double)ax[r]; ayd[r] += (double)ay[r]; }
+        subhalo_tile<T, R, GRID>(recs, count, base, raw, g, xs, ys, axd, ayd);
     }
 
     // ---- split subhalo list: publish partial sums; the last CTA of the tile reduces them in chunk order ----
@@ -199,35 +252,15 @@ __global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__
     }
 
     // ---- epilogue: O(rays) work in double ----
-    double sx[R], sy[R];                        // dynamically indexed below -> local memory, once per ray
-#pragma unroll
-    for (int r = 0; r < R; ++r) { sx[r] = axd[r]; sy[r] = ayd[r]; }
-
     if constexpr (GRID) {
-        const double xd = fma((double)min(I, a.NX - 1), a.h, a.x0);
-        const int seg = lane - lane % a.s;
-        const bool writer = (lane % a.s == 0) && (lane < a.cols_per_warp) && (I < a.NX);
-        const int ip = I / a.s;
-        double acc = 0.0;
-        int sub = 0;
-#pragma unroll 1
-        for (int r = 0; r < R; ++r) {
-            const int J = J0 + r;
-            const double yd = fma((double)min(J, a.NY - 1), a.h, a.y0);
-            double mx, my;
-            macro_alpha(a.m, xd, yd, mx, my);
-            const double bx = xd - mx - sx[r], by = yd - my - sy[r];
-            acc += sersic_sum<T>(a.src, bx, by);
-            if (++sub == a.s) {
-                // B: s adjacent lanes hold the s sub-columns of one pixel -> segmented shuffle sum
-                double tot = 0.0;
-                for (int d = 0; d < a.s; ++d) tot += __shfl_sync(0xffffffffu, acc, seg + d);
-                if (writer && J < a.NY) a.out[(int64_t)(J / a.s) * a.nx + ip] = (T)(tot * a.area_over_s2);
-                acc = 0.0;
-                sub = 0;
-            }
-        }
+        T* out = a.out;
+        const int nx = a.nx;
+        grid_epilogue<T, R>(a.m, a.src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
+                            [out, nx](int j, int i, double v) { out[(int64_t)j * nx + i] = (T)v; });
     } else {
+        double sx[R], sy[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) { sx[r] = axd[r]; sy[r] = ayd[r]; }
 #pragma unroll 1
         for (int r = 0; r < R; ++r) {
             const int64_t i = idx0 + (int64_t)r * kTraceThreads;

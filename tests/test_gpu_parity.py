@@ -111,7 +111,8 @@ def test_convolve_direct(jt, orc, dtype, ny, nx, ky, kx):
         img, ker = _f32r(img), _f32r(ker)
     got = jt.psf_convolve(to_dev(img, dtype), to_dev(ker, dtype), method="direct").double().cpu().numpy()
     want = orc.convolve(img, ker)
-    assert rel_err(got, want) < (1e-13 if dtype == "f64" else 2e-6)
+    # f32: ky*kx sequential float additions of positive terms, random-walk rounding ~ sqrt(ky kx) 2^-24
+    assert rel_err(got, want) < (1e-13 if dtype == "f64" else max(2e-6, 3.0 * (ky * kx) ** 0.5 * 2.0 ** -24))
 
 
 def test_convolve_delta_and_shift(jt):

@@ -276,6 +276,20 @@ def test_tnfw_at_centre_and_x_equal_one(orc):
     assert abs(orc.tnfw_F(1 - 1e-7) - 1.0) < 1e-6 and abs(orc.tnfw_F(1 + 1e-7) - 1.0) < 1e-6
 
 
+def test_tnfw_F_against_mpmath_literal_definition(orc):
+    """F(X) as literally defined (arccosh(1/X)/sqrt(1-X^2), arccos(1/X)/sqrt(X^2-1)) evaluated with 40 digits,
+    on both sides of X = 1 down to the last representable neighbours, and over the whole range."""
+    mp.mp.dps = 40
+    xs = [1e-6, 1e-3, 0.03, 0.5, 0.9, 1.1, 2.0, 7.0, 50.0, 1e4]
+    for k in range(3, 16):
+        xs += [1.0 - 10.0 ** -k, 1.0 + 10.0 ** -k]
+    xs += [np.nextafter(1.0, 0.0), np.nextafter(1.0, 2.0)]
+    for X in xs:
+        Xm = mp.mpf(float(X))
+        want = mp.acosh(1 / Xm) / mp.sqrt(1 - Xm * Xm) if X < 1 else mp.acos(1 / Xm) / mp.sqrt(Xm * Xm - 1)
+        assert abs(orc.tnfw_F(float(X)) / float(want) - 1.0) < 4e-15, X
+
+
 # ---------------------------------------------------------------- lens equation
 def test_lens_equation_closed_forms(orc):
     # no lens: beta = theta

@@ -148,7 +148,7 @@ def _draw_subhalos(rng, M, half_width):
     return t
 
 
-def config_c0(nx=60, dtype="f64"):
+def config_c0(nx=60, dtype="f64", seed_offset=0):
     """C0: single lens image, 60x60, no supersampling, SIE + shear, one Sersic, 11x11 Gaussian PSF."""
     w = Workload(
         name="C0", dtype="f64", nx=nx, ny=nx, pixel_scale=0.05, supersample=1,
@@ -157,9 +157,9 @@ def config_c0(nx=60, dtype="f64"):
     return w.as_dtype(dtype)
 
 
-def config_c1(nx=100, supersample=3, K=31, dtype="f64"):
+def config_c1(nx=100, supersample=3, K=31, dtype="f64", seed_offset=0):
     """C1: 100x100, supersampling 3, SIE + shear + one TNFW, two Sersics, Mixture3(31) PSF."""
-    rng = np.random.default_rng(SEEDS["C1"])
+    rng = np.random.default_rng(SEEDS["C1"] + seed_offset)
     theta_E = rng.uniform(0.8, 1.5)
     e1 = rng.uniform(-0.2, 0.2)
     e2 = rng.uniform(-0.2, 0.2)
@@ -174,9 +174,9 @@ def config_c1(nx=100, supersample=3, K=31, dtype="f64"):
     return w.as_dtype(dtype)
 
 
-def config_c2(nx=200, supersample=2, n_tnfw=10000, K=21, dtype="f64"):
+def config_c2(nx=200, supersample=2, n_tnfw=10000, K=21, dtype="f64", seed_offset=0):
     """C2: 200x200 @0.04, supersampling 2, C0 macro-lens + 10,000 TNFW in a 4x4 square."""
-    rng = np.random.default_rng(SEEDS["C2"])
+    rng = np.random.default_rng(SEEDS["C2"] + seed_offset)
     tnfw = _draw_subhalos(rng, n_tnfw, 2.0)
     w = Workload(
         name="C2", dtype="f64", nx=nx, ny=nx, pixel_scale=0.04, supersample=supersample,
@@ -185,9 +185,9 @@ def config_c2(nx=200, supersample=2, n_tnfw=10000, K=21, dtype="f64"):
     return w.as_dtype(dtype)
 
 
-def config_c3(B=4096, nx=64, supersample=2, n_tnfw=100, K=21, dtype="f32"):
+def config_c3(B=4096, nx=64, supersample=2, n_tnfw=100, K=21, dtype="f32", seed_offset=0):
     """C3: B independent systems, 64x64 @0.08, supersampling 2, 100 TNFW each, own Mixture3(21) PSF."""
-    rng = np.random.default_rng(SEEDS["C3"])
+    rng = np.random.default_rng(SEEDS["C3"] + seed_offset)
     sie = np.zeros((B, 5), dtype=np.float64)
     sie[:, 0] = rng.uniform(0.8, 1.5, size=B)
     sie[:, 1] = rng.uniform(-0.2, 0.2, size=B)
@@ -216,9 +216,9 @@ def config_c3(B=4096, nx=64, supersample=2, n_tnfw=100, K=21, dtype="f32"):
     return w.as_dtype(dtype)
 
 
-def config_c4(nx=500, supersample=5, n_tnfw=50000, K=101, half_width=5.0, dtype="f64"):
+def config_c4(nx=500, supersample=5, n_tnfw=50000, K=101, half_width=5.0, dtype="f64", seed_offset=0):
     """C4: 500x500 @0.02, supersampling 5, C0 macro-lens + 50,000 TNFW over 10x10, 3 Sersics, AiryMix(101)."""
-    rng = np.random.default_rng(SEEDS["C4"])
+    rng = np.random.default_rng(SEEDS["C4"] + seed_offset)
     tnfw = _draw_subhalos(rng, n_tnfw, half_width)
     sources = _draw_sources(rng, 3)
     psf = airymix_psf(rng, K)
