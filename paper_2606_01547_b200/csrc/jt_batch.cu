@@ -1,4 +1,200 @@
-#include "jt_internal.h"
+// jt_batch.cu -- jt_simulate_batch: B independent lens systems in ONE launch (PAPER.md:47 training-set
+// generation; BASELINE.json configs[3]).
+//
+// One CTA of 256 threads per system runs the whole pipeline on chip:
+//   per-system parameters -> derived once into shared memory (definition E, SubRec records of T, flipped PSF)
+//   for every ray tile of the system's grid: subhalo sum over the staged records (registers), SIE + shear,
+//       lens equation, Sersic, s x s warp-shuffle binning -> pre-PSF pixel into a zero-haloed shared image
+//   direct convolution (definition P) out of that shared image with the register-window sweep of jt_conv.cuh
+//   one coalesced HBM write of the final image.
+// HBM traffic per system is its parameters in and its image out; nothing intermediate leaves the SM.
+#include "jt_conv.cuh"
+#include "jt_trace.cuh"
+
 namespace jt {
-jt_status launch_batch(jt_dtype, int64_t, const jt_grid*, const jt_batch_params*, void*, cudaStream_t) { return JT_ERR_UNSUPPORTED; }
+
+constexpr int kBatchRecCap = 512;            // subhalo records resident per staging round
+constexpr int kBatchTW = 32;                 // convolution: thread block covers kBatchTW columns x 8*OY rows
+constexpr int kBatchOY = 8;
+
+template <typename T>
+struct BatchArgs {
+    int nx, ny, s, NX, NY;
+    double hh, cx, cy, area_over_s2;
+    int cols_per_warp, tiles_x, tiles_y;
+    int M, n_src, ky, kx, kyp;
+    int pw, ph, img_elems;                   // padded shared image: pw columns, ph rows; elements rounded up to 16 B
+    int rec_cap;
+    const T *sie, *shear, *tnfw, *sersic, *psf;
+    T* out;
+};
+
+template <typename T, int R>
+__global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch(const __grid_constant__ BatchArgs<T> a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ MacroLens s_m;
+    __shared__ SrcSet s_src;
+
+    SubRec<T>* recs = reinterpret_cast<SubRec<T>*>(smem_raw);
+    T* img = reinterpret_cast<T*>(smem_raw + (size_t)a.rec_cap * sizeof(SubRec<T>));
+    T* Kc = img + a.img_elems;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t b = blockIdx.x;
+    const bool conv = a.ky > 0;
+    const int hy = a.ky / 2, hx = a.kx / 2;
+
+    // ---- per-system derived parameters ----
+    if (tid == 0) {
+        const T* p = a.sie + b * 5;
+        const T* g = a.shear + b * 2;
+        s_m = derive_macro(1, (double)p[0], (double)p[1], (double)p[2], (double)p[3], (double)p[4], 1, (double)g[0],
+                           (double)g[1]);
+    }
+    if (tid == 32) s_src.n = a.n_src;
+    if (tid >= 32 && tid < 32 + a.n_src) {
+        const int k = tid - 32;
+        const T* q = a.sersic + (b * a.n_src + k) * 7;
+        derive_source(s_src, k, (double)q[0], (double)q[1], (double)q[2], (double)q[3], (double)q[4], (double)q[5],
+                      (double)q[6]);
+    }
+    if (conv) {
+        for (int i = tid; i < a.pw * a.ph; i += kTraceThreads) img[i] = (T)0;
+        const T* K = a.psf + b * (int64_t)a.ky * a.kx;
+        for (int i = tid; i < a.kx * a.kyp; i += kTraceThreads) {
+            const int cb = i / a.kyp, ca = i % a.kyp;
+            Kc[i] = (ca < a.ky) ? K[(a.ky - 1 - ca) * a.kx + (a.kx - 1 - cb)] : (T)0;
+        }
+    }
+    const RawTn<T> raw = {{a.tnfw + (b * 5 + 0) * a.M, a.tnfw + (b * 5 + 1) * a.M, a.tnfw + (b * 5 + 2) * a.M,
+                           a.tnfw + (b * 5 + 3) * a.M, a.tnfw + (b * 5 + 4) * a.M}};
+    const bool resident = a.M <= a.rec_cap;        // the whole subhalo list is staged once
+    if (resident) {
+        for (int k = tid; k < a.M; k += kTraceThreads)
+            recs[k] = make_rec<T>((double)raw.p[0][k], (double)raw.p[1][k], (double)raw.p[2][k], (double)raw.p[3][k],
+                                  (double)raw.p[4][k]);
+    }
+    __syncthreads();
+
+    // ---- ray tiles: steps 1-4 ----
+    T* gout = a.out + b * (int64_t)a.ny * a.nx;
+    const int n_tiles = a.tiles_x * a.tiles_y;
+    for (int tile = 0; tile < n_tiles; ++tile) {
+        const int txi = tile % a.tiles_x, tyi = tile / a.tiles_x;
+        RayGeom g = {a.hh, a.cx, a.cy, a.NX, a.NY, 0, 0};
+        g.I = (txi * 2 + (warp & 1)) * a.cols_per_warp + lane;
+        g.J0 = (tyi * 4 + (warp >> 1)) * R;
+        T xs[R], ys[R];
+        T x = (T)g.xd();
+        pin(x);
+#pragma unroll
+        for (int r = 0; r < R; ++r) { xs[r] = x; ys[r] = (T)g.yd(r); pin(ys[r]); }
+        double axd[R], ayd[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
+
+        if (resident) {
+            subhalo_tile<T, R, true>(recs, a.M, 0, raw, g, xs, ys, axd, ayd);
+        } else {
+            for (int base = 0; base < a.M; base += a.rec_cap) {
+                const int count = min(a.rec_cap, a.M - base);
+                __syncthreads();
+                for (int k = tid; k < count; k += kTraceThreads)
+                    recs[k] = make_rec<T>((double)raw.p[0][base + k], (double)raw.p[1][base + k],
+                                          (double)raw.p[2][base + k], (double)raw.p[3][base + k],
+                                          (double)raw.p[4][base + k]);
+                __syncthreads();
+                subhalo_tile<T, R, true>(recs, count, base, raw, g, xs, ys, axd, ayd);
+            }
+        }
+        if (conv) {
+            const int pw = a.pw;
+            grid_epilogue<T, R>(s_m, s_src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
+                                [img, pw, hy, hx](int j, int i, double v) { img[(j + hy) * pw + (i + hx)] = (T)v; });
+        } else {
+            const int nx = a.nx;
+            grid_epilogue<T, R>(s_m, s_src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
+                                [gout, nx](int j, int i, double v) { gout[(int64_t)j * nx + i] = (T)v; });
+        }
+    }
+    if (!conv) return;
+    __syncthreads();
+
+    // ---- step 5a out of shared memory ----
+    constexpr int TH = (kTraceThreads / kBatchTW) * kBatchOY;
+    const int il = tid % kBatchTW, jl0 = (tid / kBatchTW) * kBatchOY;
+    for (int j0 = 0; j0 < a.ny; j0 += TH) {
+        for (int i0 = 0; i0 < a.nx; i0 += kBatchTW) {
+            const int i = i0 + il;
+            if (i >= a.nx) continue;
+            T acc[kBatchOY];
+#pragma unroll
+            for (int r = 0; r < kBatchOY; ++r) acc[r] = (T)0;
+            conv_sweep<T, kBatchOY, false>(img + (j0 + jl0) * a.pw + i, a.pw, Kc, a.ky, a.kx, a.kyp, acc);
+#pragma unroll
+            for (int r = 0; r < kBatchOY; ++r) {
+                const int j = j0 + jl0 + r;
+                if (j < a.ny) gout[(int64_t)j * a.nx + i] = acc[r];
+            }
+        }
+    }
 }
+
+constexpr size_t kBatchMaxSmem = 227 * 1024 - 4096;      // static MacroLens + SrcSet live beside the dynamic part
+
+template <typename T>
+static size_t batch_smem(const BatchArgs<T>& a) {
+    return (size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)a.kx * a.kyp) * sizeof(T);
+}
+
+#define JT_BATCH_CASE(RR)                                                                              \
+    case RR: {                                                                                         \
+        auto kern = k_batch<T, RR>;                                                                    \
+        JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        kern<<<(unsigned)B, kTraceThreads, smem, st>>>(a);                                             \
+        break;                                                                                         \
+    }
+
+template <typename T>
+static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
+                         cudaStream_t st) {
+    if (B > 0x7fffffffLL) return JT_ERR_UNSUPPORTED;
+    const TracePlan plan = plan_trace_grid(dtype, g, 0);
+    BatchArgs<T> a = {};
+    const int s = g->supersample;
+    a.nx = g->nx; a.ny = g->ny; a.s = s; a.NX = g->nx * s; a.NY = g->ny * s;
+    a.hh = 0.5 * (g->pixel_scale / (double)s);
+    a.cx = g->cx;
+    a.cy = g->cy;
+    a.area_over_s2 = g->pixel_scale * g->pixel_scale / ((double)s * (double)s);
+    a.cols_per_warp = plan.cols_per_warp;
+    a.tiles_x = plan.tiles_x; a.tiles_y = plan.tiles_y;
+    a.M = p->n_tnfw; a.n_src = p->n_src;
+    const bool conv = p->ky > 0;
+    a.ky = conv ? p->ky : 0; a.kx = conv ? p->kx : 0;
+    a.kyp = (a.ky + 7) / 8 * 8;
+    constexpr int TH = (kTraceThreads / kBatchTW) * kBatchOY;
+    a.pw = conv ? g->nx + a.kx - 1 : 0;
+    a.ph = conv ? (g->ny + TH - 1) / TH * TH + a.ky - 1 : 0;
+    a.img_elems = (a.pw * a.ph + 3) / 4 * 4;
+    a.rec_cap = a.M < kBatchRecCap ? (a.M > 0 ? a.M : 1) : kBatchRecCap;
+    a.sie = (const T*)p->sie; a.shear = (const T*)p->shear; a.tnfw = (const T*)p->tnfw;
+    a.sersic = (const T*)p->sersic; a.psf = (const T*)p->psf;
+    a.out = (T*)out;
+    const size_t smem = batch_smem(a);
+    if (smem > kBatchMaxSmem) return JT_ERR_UNSUPPORTED;
+    switch (plan.R) {
+        JT_BATCH_CASE(5) JT_BATCH_CASE(6) JT_BATCH_CASE(7) JT_BATCH_CASE(8) JT_BATCH_CASE(9) JT_BATCH_CASE(10)
+        JT_BATCH_CASE(11) JT_BATCH_CASE(12) JT_BATCH_CASE(13) JT_BATCH_CASE(14) JT_BATCH_CASE(15) JT_BATCH_CASE(16)
+        default: return JT_ERR_UNSUPPORTED;
+    }
+    JT_LAUNCH_CHECK();
+    return JT_OK;
+}
+
+jt_status launch_batch(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
+                       cudaStream_t st) {
+    return dtype == JT_F32 ? batch_t<float>(dtype, B, g, p, out, st) : batch_t<double>(dtype, B, g, p, out, st);
+}
+
+}  // namespace jt

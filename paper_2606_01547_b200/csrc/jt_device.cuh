@@ -36,7 +36,12 @@ __device__ __forceinline__ float atanh_q(float z) { const float c[] = {JT_ATANH_
 __device__ __forceinline__ double atanh_q(double z) { const double c[] = {JT_ATANH_Q_F64_COEFS}; return horner(c, z); }
 
 // Reciprocal square root / reciprocal: one MUFU seed (~20-22 bits) + one third-order correction.
-__device__ __forceinline__ float fast_rsqrt(float x) { return rsqrtf(x); }                 // MUFU.RSQ
+__device__ __forceinline__ float fast_rsqrt(float x) {                                     // bare MUFU.RSQ
+    float r; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r;
+}
+// keeps a value in its register: stops the compiler re-deriving a float from the double it was rounded from
+__device__ __forceinline__ void pin(float& v) { asm volatile("" : "+f"(v)); }
+__device__ __forceinline__ void pin(double& v) { asm volatile("" : "+d"(v)); }
 __device__ __forceinline__ float fast_rcp(float x) { return __frcp_rn(x); }
 __device__ __forceinline__ float approx_rcp(float x) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
 __device__ __forceinline__ double fast_rsqrt(double x) {
@@ -212,6 +217,12 @@ __device__ __forceinline__ double atanh_over(double z2) {      // atanh(z)/z as 
     return 0.5 * log((1.0 + z) / (1.0 - z)) / z;
 }
 
+__device__ __forceinline__ double atan_over(double z2) {       // atan(z)/z as a function of z^2 >= 0
+    if (z2 <= 1.0) return atan_full(z2);
+    const double iz2 = 1.0 / z2, iz = sqrt(iz2);               // atan z = pi/2 - atan(1/z)
+    return fma(JT_PI_D / 2, iz, -atan_full(iz2) * iz2);
+}
+
 __device__ __forceinline__ void macro_alpha(const MacroLens& m, double x, double y, double& ax, double& ay) {
     ax = 0.0; ay = 0.0;
     if (m.has_sie) {
@@ -222,7 +233,7 @@ __device__ __forceinline__ void macro_alpha(const MacroLens& m, double x, double
             const double ipsi = fast_rsqrt(psi2);
             const double cx_ = xr * ipsi, cy_ = yr * ipsi;        // x'/psi, y'/psi
             const double zx = m.f * cx_, zy = m.f * cy_;
-            const double A = atan_full(zx * zx);                  // |zx| <= f < 1
+            const double A = atan_over(zx * zx);                  // |zx| <= f/q, above 1 when q < 0.707
             const double Bh = atanh_over(zy * zy);
             const double axr = m.b * cx_ * A, ayr = m.b * cy_ * Bh;
             ax = m.c * axr - m.s * ayr;

@@ -94,9 +94,9 @@ static jt_status trace_grid_t(const jt_grid* g, const jt_lens* lens, const SrcSe
     TraceArgs<T> a = {};
     const int s = g->supersample;
     a.nx = g->nx; a.ny = g->ny; a.s = s; a.NX = g->nx * s; a.NY = g->ny * s;
-    a.h = g->pixel_scale / (double)s;
-    a.x0 = g->cx - 0.5 * (double)(a.NX - 1) * a.h;
-    a.y0 = g->cy - 0.5 * (double)(a.NY - 1) * a.h;
+    a.hh = 0.5 * (g->pixel_scale / (double)s);
+    a.cx = g->cx;
+    a.cy = g->cy;
     a.area_over_s2 = g->pixel_scale * g->pixel_scale / ((double)s * (double)s);
     a.cols_per_warp = plan.cols_per_warp;
     a.tiles_x = plan.tiles_x;

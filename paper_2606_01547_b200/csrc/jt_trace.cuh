@@ -22,7 +22,7 @@ template <typename T>
 struct TraceArgs {
     // grid mode geometry (definition G)
     int nx, ny, s, NX, NY;
-    double h, x0, y0, area_over_s2;
+    double hh, cx, cy, area_over_s2;      // half ray spacing, grid centre
     int cols_per_warp, tiles_x;
     // ray mode
     int64_t n_rays;
@@ -45,12 +45,14 @@ struct TraceArgs {
 template <typename T>
 struct RawTn { const T* p[5]; };
 
-// geometry of definition G for one thread: column I, first row J0 of its R vertically adjacent rays
+// geometry of definition G for one thread: column I, first row J0 of its R vertically adjacent rays.
+// theta_x(I) = cx + (I - (NX-1)/2) h is evaluated as (2I - (NX-1)) * (h/2) + cx: the integer factor and h/2 are
+// exact, so a centred grid with an odd ray count puts its middle ray exactly on 0 (the SIE centre, alpha = 0).
 struct RayGeom {
-    double h, x0, y0;
+    double hh, cx, cy;          // half ray spacing, grid centre
     int NX, NY, I, J0;
-    __device__ __forceinline__ double xd() const { return fma((double)min(I, NX - 1), h, x0); }
-    __device__ __forceinline__ double yd(int r) const { return fma((double)min(J0 + r, NY - 1), h, y0); }
+    __device__ __forceinline__ double xd() const { return fma((double)(2 * min(I, NX - 1) - (NX - 1)), hh, cx); }
+    __device__ __forceinline__ double yd(int r) const { return fma((double)(2 * min(J0 + r, NY - 1) - (NY - 1)), hh, cy); }
 };
 
 // near/mid evaluation for the float kernel: coordinates re-derived in double so that dx, dy are exact
@@ -187,16 +189,17 @@ __global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__
     const int chunk = (int)((int64_t)blockIdx.x % a.n_chunks);
 
     // ---- ray ownership ----
-    RayGeom g = {a.h, a.x0, a.y0, a.NX, a.NY, 0, 0};
+    RayGeom g = {a.hh, a.cx, a.cy, a.NX, a.NY, 0, 0};
     int64_t idx0 = 0;                // ray mode: first ray index (stride 256)
     T xs[R], ys[R];
     if constexpr (GRID) {
         const int txi = (int)(tile % a.tiles_x), tyi = (int)(tile / a.tiles_x);
         g.I = (txi * 2 + (warp & 1)) * a.cols_per_warp + lane;
         g.J0 = (tyi * 4 + (warp >> 1)) * R;
-        const T x = (T)g.xd();
+        T x = (T)g.xd();
+        pin(x);
 #pragma unroll
-        for (int r = 0; r < R; ++r) { xs[r] = x; ys[r] = (T)g.yd(r); }
+        for (int r = 0; r < R; ++r) { xs[r] = x; ys[r] = (T)g.yd(r); pin(ys[r]); }
     } else {
         idx0 = tile * (int64_t)(R * kTraceThreads) + tid;
 #pragma unroll

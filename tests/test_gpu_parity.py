@@ -74,6 +74,28 @@ def test_ray_shoot_through_subhalo_cores(jt, orc, dtype):
         assert np.max(np.abs(ax - wax)) < 1e-10 * np.max(np.abs(wax))
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("e1,e2", [(-0.3, 0.35), (0.0, 0.0), (1e-9, 0.0), (0.6, -0.5), (0.9, 0.9), (-0.19, -0.12)])
+def test_ray_shoot_sie_ellipticities(jt, orc, dtype, e1, e2):
+    """SIE alone over the full range of definition E: q below 0.707 (f x'/psi above 1), circular, |e| clamped."""
+    rng = np.random.default_rng(21)
+    n = 6000
+    tx, ty = rng.uniform(-2, 2, n), rng.uniform(-2, 2, n)
+    tx[:4], ty[:4] = [0.3, 0.3, 1e-7, -1.5], [0.0, 1e-9, 0.4, 1e-12]        # on and next to the principal axes
+    sie = (1.2, e1, e2, 0.05, -0.02)
+    if dtype == "f32":
+        tx, ty, sie = _f32r(tx), _f32r(ty), tuple(_f32r(sie))
+    bx, by = jt.ray_shoot(to_dev(tx, dtype), to_dev(ty, dtype), sie, None, None)
+    wx, wy = orc.ray_shoot(tx, ty, sie, None, None)
+    tol = 2e-13 if dtype == "f64" else 4e-7
+    if e1 * e1 + e2 * e2 > 0.98:
+        # clamped |e| = 0.9999: q = 5e-5, atanh(z) is evaluated at 1 - z^2 down to q^2 = 2.5e-9, where a 1e-16 relative
+        # error in z moves the result by 1e-16 / 2.5e-9 = 4e-8: both sides are conditioning-limited, not wrong
+        tol = 2e-7
+    assert np.max(np.abs(bx.double().cpu().numpy() - wx)) < tol
+    assert np.max(np.abs(by.double().cpu().numpy() - wy)) < tol
+
+
 def test_ray_shoot_empty(jt):
     import torch
     e = torch.empty(0, dtype=torch.float64, device="cuda")
@@ -188,3 +210,69 @@ def test_c2_full_size_sampled_rows(jt, orc):
         for j in (0, 97, 163):
             want = orc.prepsf_rows(w, j, j + 1)[0]
             assert np.max(np.abs(got[j] - want)) < TOL_IMG[dtype] * scale, (dtype, j)
+
+
+# ------------------------------------------------------------------ batched: jt_simulate_batch
+def _gpu_batch(jt, bw, conv=True):
+    g = jt.Grid(bw.nx, bw.ny, bw.pixel_scale, bw.cx, bw.cy, bw.supersample)
+    d = lambda a: to_dev(a, bw.dtype)
+    tn = d(bw.tnfw) if bw.tnfw.shape[2] > 0 else None
+    out = jt.simulate_batch(g, d(bw.sie), d(bw.shear), tn, d(bw.sources), d(bw.psf) if conv else None)
+    return out.double().cpu().numpy()
+
+
+def _check_batch(jt, orc, bw):
+    want = orc.simulate_batch(bw)
+    got = _gpu_batch(jt, bw)
+    worst = max(rel_err(got[b], want[b]) for b in range(bw.B))          # reading Q20: per image, worst of the batch
+    assert worst < TOL_IMG[bw.dtype], worst
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_batch_c3_reduced(jt, orc, dtype):
+    """C3's recipe, 12 systems of 64x64 (s=2, 100 subhalos, own 21x21 PSF): the launch shape bench.py times."""
+    _check_batch(jt, orc, workloads.config_c3(B=12, dtype=dtype))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("nx,s,M,K", [(20, 1, 0, 5), (33, 3, 7, 9), (17, 5, 600, 13), (40, 2, 1100, 31), (9, 4, 3, 21)])
+def test_batch_shapes(jt, orc, dtype, nx, s, M, K):
+    """Ragged grids, every path of the subhalo staging (none, resident, re-staged in rounds), kernels wider than the image."""
+    _check_batch(jt, orc, workloads.config_c3(B=3, nx=nx, supersample=s, n_tnfw=M, K=K, dtype=dtype))
+
+
+def test_batch_matches_single_image_call(jt):
+    """jt_simulate_batch on one system == jt_simulate_image on the same system (same arithmetic, f64)."""
+    bw = workloads.config_c3(B=2, nx=48, n_tnfw=300, dtype="f64")
+    got = _gpu_batch(jt, bw)
+    g = jt.Grid(bw.nx, bw.ny, bw.pixel_scale, bw.cx, bw.cy, bw.supersample)
+    for b in range(bw.B):
+        one = jt.simulate_image(g, tuple(bw.sie[b]), tuple(bw.shear[b]), to_dev(bw.tnfw[b], "f64"), bw.sources[b],
+                                to_dev(bw.psf[b], "f64"), dtype="f64", method="direct").cpu().numpy()
+        assert rel_err(got[b], one) < 1e-12
+
+
+def test_batch_no_psf_and_empty(jt, orc):
+    import torch
+    bw = workloads.config_c3(B=2, nx=24, n_tnfw=50, dtype="f64")
+    got = _gpu_batch(jt, bw, conv=False)
+    g = jt.Grid(bw.nx, bw.ny, bw.pixel_scale, bw.cx, bw.cy, bw.supersample)
+    for b in range(bw.B):
+        one = jt.simulate_image(g, tuple(bw.sie[b]), tuple(bw.shear[b]), to_dev(bw.tnfw[b], "f64"), bw.sources[b],
+                                None, dtype="f64").cpu().numpy()
+        assert rel_err(got[b], one) < 1e-12
+    e = lambda *s: torch.empty(s, dtype=torch.float64, device="cuda")
+    out = jt.simulate_batch(g, e(0, 5), e(0, 2), None, e(0, 1, 7), None)
+    assert out.shape[0] == 0
+
+
+def test_batch_c3_full_size_sampled(jt, orc):
+    """Full C3 (4,096 systems, f32) in the launch configuration bench.py times; 6 systems spread over the batch
+    against the oracle, and every image finite and non-negative."""
+    bw = workloads.config_c3(dtype="f32")
+    got = _gpu_batch(jt, bw)
+    assert np.isfinite(got).all() and (got >= 0).all()
+    idx = [0, 1, 777, 2048, 3333, 4095]
+    want = orc.simulate_batch(bw, systems=idx)
+    worst = max(rel_err(got[b], want[k]) for k, b in enumerate(idx))
+    assert worst < TOL_IMG["f32"], worst
