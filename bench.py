@@ -36,9 +36,11 @@ if ROOT not in sys.path:
 METRIC = "ray_deflector_evals_per_s"
 UNIT = "evals/s"
 SM_COUNT = 148
-# Instructions per evaluation that the formulation needs on the issue port (DESIGN.md "Rooflines":
-# counted in the SASS of the warp-uniform far-field branch, profiles/r01_sass_counts.md).
-ALG_INSTR_PER_EVAL = {"f32": 37.5, "f64": 63.0}
+# Algorithmic work per evaluation on the binding unit: counted in the SASS of the warp-uniform
+# far-field loop (loop head + far body) divided by its 8 rays.  f32: issue slots (the issue port and the FP32 pipe both
+# run 128 lanes/clk/SM, the port binds); f64: FP64-pipe instructions (64 lanes/clk/SM, the pipe binds).
+ALG_INSTR_PER_EVAL = {"f32": 35.1, "f64": 51.75}
+ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
 
 
@@ -368,7 +370,8 @@ def run_ours(args, rank, world, local_rank):
 
     # ---- roofline of the dominant kernel: the ray-tracing kernel, issue-limited ALU peak ----
     f_mhz = (clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
-    peak_tinstr = SM_COUNT * 4 * 32 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+    lanes = ALU_LANES_PER_SM[w.dtype]
+    peak_tinstr = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
     if phase:
         trace_ms = float(np.mean([p[0] for p in phase]))
         conv_ms = float(np.mean([p[1] for p in phase]))
@@ -378,12 +381,13 @@ def run_ours(args, rank, world, local_rank):
     achieved = w.evals * n_alg / (trace_ms * 1e-3) / 1e12
     line["roofline"] = {
         "bound": "alu", "kernel": "k_batch" if batch else "k_trace", "achieved": achieved, "peak": peak_tinstr,
-        "unit": "Tinstr/s", "frac": achieved / peak_tinstr, "traffic": None,
-        "peak_kind": "derived: 148 SMs x 4 schedulers x 32 lanes x %.0f MHz (max clock, %s)" % (
-            peaks.get("sm_max_mhz", 1965.0), peak_kind),
+        "unit": "Tlaneop/s", "frac": achieved / peak_tinstr, "traffic": None,
+        "peak_kind": "derived: 148 SMs x %d lanes/clk (%s) x %.0f MHz (max clock, %s)" % (
+            lanes, "issue port = FP32 pipe" if w.dtype == "f32" else "FP64 pipe", peaks.get("sm_max_mhz", 1965.0),
+            peak_kind),
         "alg_instr_per_eval": n_alg, "kernel_ms": trace_ms, "conv_ms": conv_ms,
         "kernel_share_of_step": trace_ms / (ms_total_local / args.steps),
-        "frac_at_observed_clock": achieved / (SM_COUNT * 4 * 32 * f_mhz * 1e6 / 1e12),
+        "frac_at_observed_clock": achieved / (SM_COUNT * lanes * f_mhz * 1e6 / 1e12),
         "evals_per_s_kernel": w.evals / (trace_ms * 1e-3)}
     if not batch:
         K = w.psf.shape[0] * w.psf.shape[1]
