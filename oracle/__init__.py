@@ -226,6 +226,24 @@ def prepsf_rows(w, j0=0, j1=None):
     return out
 
 
+def prepsf_pixels(w, j, cols):
+    """Pre-PSF values of the pixels (j, i), i in cols, by composing the oracle's steps on just their sub-rays:
+    definition G for the s x s sub-ray angles, orc_ray_shoot, orc_source_brightness, definition B.
+    Used to sample configs whose full image would take core-hours."""
+    s = int(w.supersample)
+    cols = np.asarray(cols, dtype=np.int64)
+    NX, NY = w.nx * s, w.ny * s
+    h = w.pixel_scale / s
+    shape = (len(cols), s, s)                                                            # [pixel][sub-row][sub-column]
+    I = np.broadcast_to(cols[:, None, None] * s + np.arange(s)[None, None, :], shape).astype(np.float64)
+    J = np.broadcast_to(j * s + np.arange(s)[None, :, None], shape).astype(np.float64)
+    tx = w.cx + (I - 0.5 * (NX - 1)) * h
+    ty = w.cy + (J - 0.5 * (NY - 1)) * h
+    bx, by = ray_shoot(tx.ravel(), ty.ravel(), w.sie, w.shear, w.tnfw)
+    flux = source_brightness(bx, by, w.sources).reshape(len(cols), s * s)
+    return w.pixel_scale ** 2 * flux.sum(axis=1) / float(s * s)
+
+
 def simulate_image(w):
     """Whole pipeline on one system; returns (pre_psf, image)."""
     sie, shear, tnfw = _lens_args(w.sie, w.shear, w.tnfw)

@@ -42,6 +42,7 @@ static bool valid_kernel_size(int ky, int kx) { return ky >= 1 && kx >= 1 && (ky
 jt_conv_method resolve_conv_method(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method m) {
     if (m == JT_CONV_DIRECT || m == JT_CONV_FFT) return m;
     if (!conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_CONV_FFT;
+    if (!conv_fft_supported(dtype, ny, nx, ky, kx)) return JT_CONV_DIRECT;
     return ((int64_t)ky * kx > 41 * 41) ? JT_CONV_FFT : JT_CONV_DIRECT;
 }
 
@@ -80,7 +81,7 @@ uint64_t jt_kernel_launches(void) { return g_launches; }
 // ------------------------------------------------------------------ step 1
 size_t jt_ray_shoot_workspace_bytes(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw) {
     if (!valid_dtype(dtype) || n_rays <= 0 || n_tnfw < 0) return 0;
-    return plan_trace_rays(n_rays, n_tnfw).total_bytes;
+    return plan_trace_rays(dtype, n_rays, n_tnfw).total_bytes;
 }
 
 jt_status jt_ray_shoot(jt_dtype dtype, int64_t n_rays, const void* theta_x, const void* theta_y, const jt_lens* lens,
@@ -90,7 +91,7 @@ jt_status jt_ray_shoot(jt_dtype dtype, int64_t n_rays, const void* theta_x, cons
     if (n_rays == 0) return JT_OK;
     if (!theta_x || !theta_y || !beta_x || !beta_y) return JT_ERR_INVALID_VALUE;
     if (theta_x == beta_x || theta_y == beta_y || theta_x == beta_y || theta_y == beta_x) return JT_ERR_INVALID_VALUE;
-    const TracePlan plan = plan_trace_rays(n_rays, lens->n_tnfw);
+    const TracePlan plan = plan_trace_rays(dtype, n_rays, lens->n_tnfw);
     if (plan.total_bytes > 0 && (!workspace || workspace_bytes < plan.total_bytes)) return JT_ERR_WORKSPACE;
     jt_status s = check_device();
     if (s != JT_OK) return s;
@@ -126,6 +127,8 @@ jt_status jt_psf_convolve(jt_dtype dtype, int32_t ny, int32_t nx, const void* im
     if (ny < 1 || nx < 1 || !valid_kernel_size(ky, kx) || !image || !kernel || !out || image == out)
         return JT_ERR_INVALID_VALUE;
     if (method == JT_CONV_DIRECT && !conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_ERR_UNSUPPORTED;
+    if (resolve_conv_method(dtype, ny, nx, ky, kx, method) == JT_CONV_FFT && !conv_fft_supported(dtype, ny, nx, ky, kx))
+        return JT_ERR_UNSUPPORTED;
     const size_t need = conv_ws(dtype, ny, nx, ky, kx, method);
     if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
     jt_status s = check_device();
@@ -159,6 +162,9 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
     const bool conv = !(ky == 0 && kx == 0 && kernel == nullptr);
     if (conv && (!valid_kernel_size(ky, kx) || !kernel)) return JT_ERR_INVALID_VALUE;
     if (conv && method == JT_CONV_DIRECT && !conv_direct_supported(dtype, grid->ny, grid->nx, ky, kx)) return JT_ERR_UNSUPPORTED;
+    if (conv && resolve_conv_method(dtype, grid->ny, grid->nx, ky, kx, method) == JT_CONV_FFT &&
+        !conv_fft_supported(dtype, grid->ny, grid->nx, ky, kx))
+        return JT_ERR_UNSUPPORTED;
     const size_t need = jt_simulate_image_workspace_bytes(dtype, grid, lens->n_tnfw, conv ? ky : 0, conv ? kx : 0, method);
     if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
     s = check_device();

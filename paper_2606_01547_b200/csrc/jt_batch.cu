@@ -21,10 +21,11 @@ template <typename T>
 struct BatchArgs {
     int nx, ny, s, NX, NY;
     double hh, cx, cy, area_over_s2;
-    int cols_per_warp, tiles_x, tiles_y;
+    int cols_per_warp, wtiles_x, n_wt, n_tiles;
     int M, n_src, ky, kx, kyp;
     int pw, ph, img_elems;                   // padded shared image: pw columns, ph rows; elements rounded up to 16 B
     int rec_cap;
+    int dacc_off;                            // byte offset of the DAcc columns (float mode), 16-byte aligned
     const T *sie, *shear, *tnfw, *sersic, *psf;
     T* out;
 };
@@ -34,10 +35,12 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ MacroLens s_m;
     __shared__ SrcSet s_src;
+    __shared__ unsigned short s_queue[kTraceThreads / 32][kBatchRecCap];
 
     SubRec<T>* recs = reinterpret_cast<SubRec<T>*>(smem_raw);
     T* img = reinterpret_cast<T*>(smem_raw + (size_t)a.rec_cap * sizeof(SubRec<T>));
     T* Kc = img + a.img_elems;
+    double2* dacc = reinterpret_cast<double2*>(smem_raw + a.dacc_off);       // float mode only
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t b = blockIdx.x;
@@ -78,23 +81,23 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
 
     // ---- ray tiles: steps 1-4 ----
     T* gout = a.out + b * (int64_t)a.ny * a.nx;
-    const int n_tiles = a.tiles_x * a.tiles_y;
-    for (int tile = 0; tile < n_tiles; ++tile) {
-        const int txi = tile % a.tiles_x, tyi = tile / a.tiles_x;
-        RayGeom g = {a.hh, a.cx, a.cy, a.NX, a.NY, 0, 0};
-        g.I = (txi * 2 + (warp & 1)) * a.cols_per_warp + lane;
-        g.J0 = (tyi * 4 + (warp >> 1)) * R;
+    for (int tile = 0; tile < a.n_tiles; ++tile) {
+        RayGeom g = {a.hh, a.cx, a.cy, a.NX, a.NY, a.NX, a.NY};     // idle warp: clamped coordinates, no stores
+        const int wt = tile * (kTraceThreads / 32) + warp;
+        if (wt < a.n_wt) {
+            g.I = (wt % a.wtiles_x) * a.cols_per_warp + lane;
+            g.J0 = (wt / a.wtiles_x) * R;
+        }
         T xs[R], ys[R];
         T x = (T)g.xd();
         pin(x);
 #pragma unroll
         for (int r = 0; r < R; ++r) { xs[r] = x; ys[r] = (T)g.yd(r); pin(ys[r]); }
-        double axd[R], ayd[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
+        DAcc<T, R> acc;
+        acc.init(dacc + tid);
 
         if (resident) {
-            subhalo_tile<T, R, true>(recs, a.M, 0, raw, g, xs, ys, axd, ayd);
+            subhalo_tile<T, R, true>(recs, a.M, 0, raw, g, xs, ys, acc, s_queue[warp]);
         } else {
             for (int base = 0; base < a.M; base += a.rec_cap) {
                 const int count = min(a.rec_cap, a.M - base);
@@ -104,9 +107,11 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
                                           (double)raw.p[2][base + k], (double)raw.p[3][base + k],
                                           (double)raw.p[4][base + k]);
                 __syncthreads();
-                subhalo_tile<T, R, true>(recs, count, base, raw, g, xs, ys, axd, ayd);
+                subhalo_tile<T, R, true>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp]);
             }
         }
+        double axd[R], ayd[R];
+        acc.result(axd, ayd);
         if (conv) {
             const int pw = a.pw;
             grid_epilogue<T, R>(s_m, s_src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
@@ -140,11 +145,11 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     }
 }
 
-constexpr size_t kBatchMaxSmem = 227 * 1024 - 4096;      // static MacroLens + SrcSet live beside the dynamic part
+constexpr size_t kBatchMaxSmem = 227 * 1024 - 4096 - 8192;      // static MacroLens + SrcSet live beside the dynamic part
 
 template <typename T>
-static size_t batch_smem(const BatchArgs<T>& a) {
-    return (size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)a.kx * a.kyp) * sizeof(T);
+static size_t batch_smem_front(const BatchArgs<T>& a) {
+    return align_up((size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)a.kx * a.kyp) * sizeof(T), 16);
 }
 
 #define JT_BATCH_CASE(RR)                                                                              \
@@ -168,7 +173,7 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.cy = g->cy;
     a.area_over_s2 = g->pixel_scale * g->pixel_scale / ((double)s * (double)s);
     a.cols_per_warp = plan.cols_per_warp;
-    a.tiles_x = plan.tiles_x; a.tiles_y = plan.tiles_y;
+    a.wtiles_x = plan.tiles_x; a.n_wt = (int)plan.n_wt; a.n_tiles = (int)plan.n_tiles;
     a.M = p->n_tnfw; a.n_src = p->n_src;
     const bool conv = p->ky > 0;
     a.ky = conv ? p->ky : 0; a.kx = conv ? p->kx : 0;
@@ -181,7 +186,8 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.sie = (const T*)p->sie; a.shear = (const T*)p->shear; a.tnfw = (const T*)p->tnfw;
     a.sersic = (const T*)p->sersic; a.psf = (const T*)p->psf;
     a.out = (T*)out;
-    const size_t smem = batch_smem(a);
+    a.dacc_off = (int)batch_smem_front(a);
+    const size_t smem = (size_t)a.dacc_off + (sizeof(T) == 4 ? (size_t)plan.R * kTraceThreads * sizeof(double2) : 0);
     if (smem > kBatchMaxSmem) return JT_ERR_UNSUPPORTED;
     switch (plan.R) {
         JT_BATCH_CASE(5) JT_BATCH_CASE(6) JT_BATCH_CASE(7) JT_BATCH_CASE(8) JT_BATCH_CASE(9) JT_BATCH_CASE(10)

@@ -38,8 +38,9 @@ jt_status make_sources(const jt_sources* src, SrcSet* out);
 struct TracePlan {
     int R;                 // rays per thread
     int cols_per_warp;     // active lanes per warp (grid mode: floor(32/s)*s; ray mode: 32)
-    int tiles_x, tiles_y;  // ray tiles (ray mode: tiles_y = 1)
-    int64_t n_tiles;
+    int tiles_x, tiles_y;  // grid mode: warp tiles (cols_per_warp x R rays) per axis
+    int64_t n_wt;          // grid mode: warp tiles in all
+    int64_t n_tiles;       // CTAs per subhalo chunk (8 warp tiles, or 8 * 32 * R rays in ray mode)
     int n_chunks;          // subhalo list split (1 = no workspace traffic)
     int64_t chunk_len;     // subhalos per chunk (multiple of kSubTile unless n_chunks == 1)
     size_t partial_bytes;  // n_chunks > 1: double2 per (chunk, ray slot)
@@ -47,7 +48,7 @@ struct TracePlan {
     size_t total_bytes;
 };
 TracePlan plan_trace_grid(jt_dtype dtype, const jt_grid* g, int64_t n_tnfw);
-TracePlan plan_trace_rays(int64_t n_rays, int64_t n_tnfw);
+TracePlan plan_trace_rays(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw);
 
 jt_status launch_trace_grid(jt_dtype dtype, const jt_grid* g, const jt_lens* lens, const SrcSet& src,
                             const TracePlan& plan, void* workspace, void* pre_psf, cudaStream_t st);
@@ -62,6 +63,7 @@ bool      conv_direct_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
 size_t    conv_direct_workspace_bytes(jt_dtype dtype, int ky, int kx);
 jt_status launch_conv_direct(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
                              void* workspace, void* out, cudaStream_t st);
+bool      conv_fft_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
 size_t    fft_conv_workspace_bytes(jt_dtype dtype, int ny, int nx, int ky, int kx);
 jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
                           void* workspace, void* out, cudaStream_t st);

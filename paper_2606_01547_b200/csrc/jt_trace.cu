@@ -33,45 +33,58 @@ static int rays_per_thread(int s, bool f64) {
     switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 9; case 5: return 10; default: return s; }
 }
 
-static void plan_chunks(TracePlan* p, int64_t M, int R) {
-    // enough (tile, chunk) CTAs for ~10 waves of 2 CTAs per SM; chunks are whole shared-memory tiles
-    const int64_t target = (int64_t)kNumSMs * 2 * 10;
-    int64_t n_sub_tiles = (M + kSubTile - 1) / kSubTile;
-    int64_t want = (p->n_tiles > 0) ? (target + p->n_tiles - 1) / p->n_tiles : 1;
-    if (want < 1) want = 1;
-    if (want > n_sub_tiles) want = n_sub_tiles;
-    if (want < 1) want = 1;
-    int64_t tiles_per_chunk = (n_sub_tiles + want - 1) / want;
-    if (tiles_per_chunk < 1) tiles_per_chunk = 1;
-    p->chunk_len = tiles_per_chunk * kSubTile;
-    p->n_chunks = (int)((M + p->chunk_len - 1) / p->chunk_len);
+// Split of the subhalo list over CTAs.  All CTAs of a launch do the same work, so the launch runs in waves of
+// `slots` CTAs (148 SMs x resident CTAs per SM); pick the chunk count c that minimises
+//   waves(n_tiles * c) * (records per chunk + fixed per-CTA cost in record units)
+// -- e.g. C2 (91 ray tiles, 10,000 subhalos, float): c = 13 gives 1183 CTAs = 4 full waves of 296.
+static void plan_chunks(TracePlan* p, int64_t M, int R, bool f64) {
+    const int64_t slots = (int64_t)kNumSMs * (f64 ? 1 : 2);
+    const int64_t ovh = 48, ovh_split = 24;          // prologue + epilogue; partial-sum publish + reduce
+    int64_t best_c = 1;
+    if (M > 0 && p->n_tiles > 0) {
+        int64_t c_max = M / 64;                      // at least 64 records per chunk
+        if (c_max > 4096) c_max = 4096;
+        double best = -1.0;
+        for (int64_t c = 1; c <= (c_max < 1 ? 1 : c_max); ++c) {
+            const int64_t len = (M + c - 1) / c;
+            const int64_t nc = (M + len - 1) / len;
+            const int64_t waves = (p->n_tiles * nc + slots - 1) / slots;
+            const double cost = (double)waves * (double)(len + ovh + (nc > 1 ? ovh_split : 0));
+            if (best < 0.0 || cost < best * 0.999) { best = cost; best_c = nc; }
+        }
+    }
+    p->chunk_len = M > 0 ? (M + best_c - 1) / best_c : 1;
+    p->n_chunks = M > 0 ? (int)((M + p->chunk_len - 1) / p->chunk_len) : 1;
     if (p->n_chunks < 1) p->n_chunks = 1;
     p->partial_bytes = p->n_chunks > 1 ? (size_t)p->n_chunks * p->n_tiles * R * kTraceThreads * sizeof(double2) : 0;
     p->counter_bytes = p->n_chunks > 1 ? align_up((size_t)p->n_tiles * sizeof(unsigned int), 256) : 0;
     p->total_bytes = p->partial_bytes + p->counter_bytes;
 }
 
+// Ray ownership: a warp tile is cols_per_warp ray columns x R ray rows; the warp tiles of the grid are numbered
+// row-major and dealt to CTAs eight at a time, so only the last CTA can be partly empty whatever the grid shape.
 static TracePlan plan_trace_grid_t(const jt_grid* g, int64_t n_tnfw, bool f64) {
     TracePlan p = {};
     const int s = g->supersample;
     p.R = rays_per_thread(s, f64);
     p.cols_per_warp = (32 / s) * s;
     const int NX = g->nx * s, NY = g->ny * s;
-    p.tiles_x = (NX + 2 * p.cols_per_warp - 1) / (2 * p.cols_per_warp);
-    p.tiles_y = (NY + 4 * p.R - 1) / (4 * p.R);
-    p.n_tiles = (int64_t)p.tiles_x * p.tiles_y;
-    plan_chunks(&p, n_tnfw, p.R);
+    p.tiles_x = (NX + p.cols_per_warp - 1) / p.cols_per_warp;       // warp tiles per row of warp tiles
+    p.tiles_y = (NY + p.R - 1) / p.R;
+    p.n_wt = (int64_t)p.tiles_x * p.tiles_y;
+    p.n_tiles = (p.n_wt + kTraceThreads / 32 - 1) / (kTraceThreads / 32);
+    plan_chunks(&p, n_tnfw, p.R, f64);
     return p;
 }
 TracePlan plan_trace_grid(jt_dtype d, const jt_grid* g, int64_t n_tnfw) { return plan_trace_grid_t(g, n_tnfw, d == JT_F64); }
 
-TracePlan plan_trace_rays(int64_t n_rays, int64_t n_tnfw) {
+TracePlan plan_trace_rays(jt_dtype d, int64_t n_rays, int64_t n_tnfw) {
     TracePlan p = {};
     p.R = 8;
     p.cols_per_warp = 32;
     p.tiles_x = 1; p.tiles_y = 1;
     p.n_tiles = (n_rays + (int64_t)p.R * kTraceThreads - 1) / ((int64_t)p.R * kTraceThreads);
-    plan_chunks(&p, n_tnfw, p.R);
+    plan_chunks(&p, n_tnfw, p.R, d == JT_F64);
     return p;
 }
 
@@ -99,7 +112,8 @@ static jt_status trace_grid_t(const jt_grid* g, const jt_lens* lens, const SrcSe
     a.cy = g->cy;
     a.area_over_s2 = g->pixel_scale * g->pixel_scale / ((double)s * (double)s);
     a.cols_per_warp = plan.cols_per_warp;
-    a.tiles_x = plan.tiles_x;
+    a.wtiles_x = plan.tiles_x;
+    a.n_wt = plan.n_wt;
     fill_lens(a, lens, plan, workspace);
     a.out = (T*)pre_psf;
     a.src = src;

@@ -23,7 +23,8 @@ struct TraceArgs {
     // grid mode geometry (definition G)
     int nx, ny, s, NX, NY;
     double hh, cx, cy, area_over_s2;      // half ray spacing, grid centre
-    int cols_per_warp, tiles_x;
+    int cols_per_warp, wtiles_x;
+    int64_t n_wt;                         // warp tiles of the grid, dealt to CTAs eight at a time
     // ray mode
     int64_t n_rays;
     const T *tx, *ty;
@@ -44,6 +45,8 @@ struct TraceArgs {
 // raw (caller) subhalo arrays of one system: cx, cy, Rs, alpha_Rs, r_trunc
 template <typename T>
 struct RawTn { const T* p[5]; };
+
+constexpr double kMidX2 = 2.0;          // below this X^2 a ray takes the generic (logarithm, series) form
 
 // geometry of definition G for one thread: column I, first row J0 of its R vertically adjacent rays.
 // theta_x(I) = cx + (I - (NX-1)/2) h is evaluated as (2I - (NX-1)) * (h/2) + cx: the integer factor and h/2 are
@@ -73,15 +76,103 @@ __device__ __noinline__ double2 tnfw_slow_f32(double xd, double yd, float cx, fl
     return make_double2(f * dx, f * dy);
 }
 
-// One staged tile of `count` subhalo records against this thread's R rays: adds the tile's deflection to
-// (axd, ayd).  GRID: the R rays share one column (xs[0]) and ascend in y.
+// Deflection accumulators of one thread's R rays.  double mode: 2R registers, summed directly.  float mode: the hot
+// loop carries only float per-tile sums (tx, ty); the double running sums live in a column of shared memory
+// (p[r * kTraceThreads]) that is touched once per staged tile, which keeps the float kernel at 128 registers
+// (2 CTAs per SM) without spilling the ray coordinates.
+template <typename T, int R> struct DAcc;
+template <int R> struct DAcc<double, R> {
+    double tx[R], ty[R];
+    __device__ __forceinline__ void init(double2*) {
+#pragma unroll
+        for (int r = 0; r < R; ++r) { tx[r] = 0.0; ty[r] = 0.0; }
+    }
+    __device__ __forceinline__ void begin_tile() {}
+    __device__ __forceinline__ void end_tile() {}
+    __device__ __forceinline__ void add_double(int r, double x, double y) { tx[r] += x; ty[r] += y; }
+    __device__ __forceinline__ void result(double (&x)[R], double (&y)[R]) const {
+#pragma unroll
+        for (int r = 0; r < R; ++r) { x[r] = tx[r]; y[r] = ty[r]; }
+    }
+};
+template <int R> struct DAcc<float, R> {
+    float tx[R], ty[R];
+    double2* p;
+    __device__ __forceinline__ void init(double2* base) {
+        p = base;
+#pragma unroll
+        for (int r = 0; r < R; ++r) p[r * kTraceThreads] = make_double2(0.0, 0.0);
+    }
+    __device__ __forceinline__ void begin_tile() {
+#pragma unroll
+        for (int r = 0; r < R; ++r) { tx[r] = 0.f; ty[r] = 0.f; }
+    }
+    __device__ __forceinline__ void end_tile() {
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            double2 v = p[r * kTraceThreads];
+            v.x += (double)tx[r]; v.y += (double)ty[r];
+            p[r * kTraceThreads] = v;
+        }
+    }
+    __device__ __forceinline__ void add_double(int r, double x, double y) {
+        double2 v = p[r * kTraceThreads];
+        v.x += x; v.y += y;
+        p[r * kTraceThreads] = v;
+    }
+    __device__ __forceinline__ void result(double (&x)[R], double (&y)[R]) const {
+#pragma unroll
+        for (int r = 0; r < R; ++r) { const double2 v = p[r * kTraceThreads]; x[r] = v.x; y[r] = v.y; }
+    }
+};
+template <typename T, int R>
+constexpr size_t dacc_smem_bytes() { return sizeof(T) == 4 ? (size_t)R * kTraceThreads * sizeof(double2) : 0; }
+
+// Cold path: one record against this thread's R rays when the warp is not uniformly far or mid.  Out of line, and
+// all per-ray state comes in through memory, so that the hot loop's register allocation never sees it.  Each ray
+// picks its own form: far / mid as in the hot loop, else the generic closed form (series below X = 1e-3) in double.
+// dp: the thread's double accumulator column in shared memory (float mode; nullptr in double mode).
+template <typename T, int R, bool GRID>
+__device__ __noinline__ void subhalo_cold(const SubRec<T>* rec, int64_t j, const RawTn<T>* raw, const RayGeom* g,
+                                          const T* xs, const T* ys, T* ax, T* ay, double2* dp) {
+    const SubRec<T> s = *rec;
+#pragma unroll 1
+    for (int r = 0; r < R; ++r) {
+        const T dx = (GRID ? xs[0] : xs[r]) - s.cx, dy = ys[r] - s.cy;
+        const T R2 = fma(dy, dy, dx * dx);
+        const T X2 = R2 * s.iRs2;
+        if (X2 >= (T)kMidX2) {
+            const T f = (X2 >= s.thr) ? tnfw_far<T>(R2, s) : tnfw_midfast<T>(R2, s);
+            ax[r] = fma(f, dx, ax[r]);
+            ay[r] = fma(f, dy, ay[r]);
+        } else if constexpr (sizeof(T) == 8) {
+            const T f = (T)tnfw_any((double)R2, *(const SubRec<double>*)&s);
+            ax[r] = fma(f, dx, ax[r]);
+            ay[r] = fma(f, dy, ay[r]);
+        } else {
+            double xd, yd;
+            if constexpr (GRID) { xd = g->xd(); yd = g->yd(r); }
+            else { xd = (double)xs[r]; yd = (double)ys[r]; }
+            const double2 c = tnfw_slow_f32<T>(xd, yd, s.cx, s.cy, s.iRs2, s.t, s.c1, s.amp, s.tm1, j, raw);
+            double2 v = dp[r * kTraceThreads];
+            v.x += c.x; v.y += c.y;
+            dp[r * kTraceThreads] = v;
+        }
+    }
+}
+
+// One staged tile of `count` subhalo records against this thread's R rays: adds the tile's deflection to acc.
+// GRID: the R rays share one column (xs[0]) and ascend in y.  Records for which the warp is neither uniformly far
+// nor uniformly mid are queued (wq: this warp's index queue in shared memory, >= count entries) and handled by
+// subhalo_cold after the hot loop.
 template <typename T, int R, bool GRID>
 __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs, int count, int64_t base,
                                              const RawTn<T>& raw, const RayGeom& g, const T (&xs)[R], const T (&ys)[R],
-                                             double (&axd)[R], double (&ayd)[R]) {
-    T ax[R], ay[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) { ax[r] = (T)0; ay[r] = (T)0; }
+                                             DAcc<T, R>& acc, unsigned short* wq) {
+    T (&ax)[R] = acc.tx;
+    T (&ay)[R] = acc.ty;
+    acc.begin_tile();
+    int qn = 0;
 
 #pragma unroll 1
     for (int jj = 0; jj < count; ++jj) {
@@ -104,33 +195,43 @@ __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs,
                 R2min = fmin(R2min, R2[r]);
             }
         }
-        const bool far = R2min * s.iRs2 >= s.thr;
-        if (__all_sync(0xffffffffu, far)) {
+        const T X2min = R2min * s.iRs2;
+        if (__all_sync(0xffffffffu, X2min >= s.thr)) {
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const T f = tnfw_far<T>(R2[r], s);
                 ax[r] = fma(f, dx[r], ax[r]);
                 ay[r] = fma(f, dy[r], ay[r]);
             }
-        } else {
+        } else if (__all_sync(0xffffffffu, X2min >= (T)kMidX2)) {
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                if constexpr (sizeof(T) == 8) {
-                    const T f = (R2[r] * s.iRs2 >= s.thr) ? tnfw_far<T>(R2[r], s) : (T)tnfw_any((double)R2[r], *(const SubRec<double>*)&s);
-                    ax[r] = fma(f, dx[r], ax[r]);
-                    ay[r] = fma(f, dy[r], ay[r]);
-                } else {
-                    double xd, yd;
-                    if constexpr (GRID) { xd = g.xd(); yd = g.yd(r); }
-                    else { xd = (double)xs[r]; yd = (double)ys[r]; }
-                    const double2 c = tnfw_slow_f32<T>(xd, yd, s.cx, s.cy, s.iRs2, s.t, s.c1, s.amp, s.tm1, base + jj, &raw);
-                    axd[r] += c.x; ayd[r] += c.y;
-                }
+                const T f = tnfw_midfast<T>(R2[r], s);
+                ax[r] = fma(f, dx[r], ax[r]);
+                ay[r] = fma(f, dy[r], ay[r]);
             }
+        } else {
+            if ((threadIdx.x & 31) == 0) wq[qn] = (unsigned short)jj;
+            ++qn;
         }
     }
+    if (qn > 0) {                                   // warp-uniform
+        __syncwarp();
+        T lx[R], ly[R], lax[R], lay[R];             // local-memory copies: the cold path indexes them dynamically
 #pragma unroll
-    for (int r = 0; r < R; ++r) { axd[r] += (double)ax[r]; ayd[r] += (double)ay[r]; }
+        for (int r = 0; r < R; ++r) { lx[r] = xs[r]; ly[r] = ys[r]; lax[r] = ax[r]; lay[r] = ay[r]; }
+        double2* dp = nullptr;
+        if constexpr (sizeof(T) == 4) dp = acc.p;
+#pragma unroll 1
+        for (int q = 0; q < qn; ++q) {
+            const int jj = wq[q];
+            subhalo_cold<T, R, GRID>(&recs[jj], base + jj, &raw, &g, lx, ly, lax, lay, dp);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) { ax[r] = lax[r]; ay[r] = lay[r]; }
+        __syncwarp();
+    }
+    acc.end_tile();
 }
 
 // stage one tile of derived records (in double) from the raw arrays; entries past j_end are null records
@@ -180,9 +281,11 @@ __device__ __forceinline__ void grid_epilogue(const MacroLens& m, const SrcSet& 
 }
 
 template <typename T, int R, bool GRID>
-__global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__ TraceArgs<T> a) {
+__global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_trace(const __grid_constant__ TraceArgs<T> a) {
     __shared__ SubRec<T> recs[kSubTile];
     __shared__ int s_last;
+    __shared__ unsigned short s_queue[kTraceThreads / 32][kSubTile];
+    extern __shared__ __align__(16) unsigned char dacc_raw[];      // float mode: DAcc columns, R * 256 double2
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t tile = (int64_t)blockIdx.x / a.n_chunks;
@@ -193,9 +296,14 @@ __global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__
     int64_t idx0 = 0;                // ray mode: first ray index (stride 256)
     T xs[R], ys[R];
     if constexpr (GRID) {
-        const int txi = (int)(tile % a.tiles_x), tyi = (int)(tile / a.tiles_x);
-        g.I = (txi * 2 + (warp & 1)) * a.cols_per_warp + lane;
-        g.J0 = (tyi * 4 + (warp >> 1)) * R;
+        const int64_t wt = tile * (kTraceThreads / 32) + warp;
+        if (wt < a.n_wt) {
+            g.I = (int)(wt % a.wtiles_x) * a.cols_per_warp + lane;
+            g.J0 = (int)(wt / a.wtiles_x) * R;
+        } else {                                   // idle warp of the last CTA: clamped coordinates, no stores
+            g.I = a.NX;
+            g.J0 = a.NY;
+        }
         T x = (T)g.xd();
         pin(x);
 #pragma unroll
@@ -210,9 +318,8 @@ __global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__
         }
     }
 
-    double axd[R], ayd[R];
-#pragma unroll
-    for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
+    DAcc<T, R> acc;
+    acc.init(reinterpret_cast<double2*>(dacc_raw) + tid);
 
     // ---- subhalo sum over this CTA's chunk ----
     const RawTn<T> raw = {{a.tn[0], a.tn[1], a.tn[2], a.tn[3], a.tn[4]}};
@@ -223,8 +330,10 @@ __global__ void __launch_bounds__(kTraceThreads) k_trace(const __grid_constant__
         stage_tile<T>(recs, raw, base, j_end, tid, kTraceThreads);
         __syncthreads();
         const int count = (int)min((int64_t)kSubTile, j_end - base);
-        subhalo_tile<T, R, GRID>(recs, count, base, raw, g, xs, ys, axd, ayd);
+        subhalo_tile<T, R, GRID>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp]);
     }
+    double axd[R], ayd[R];
+    acc.result(axd, ayd);
 
     // ---- split subhalo list: publish partial sums; the last CTA of the tile reduces them in chunk order ----
     if (a.n_chunks > 1) {
@@ -283,9 +392,13 @@ template <typename T, bool GRID>
 jt_status launch_trace_t(const TraceArgs<T>& a, int R, cudaStream_t st);
 
 #define JT_TRACE_CASE(RR)                                                                         \
-    case RR:                                                                                      \
-        k_trace<T, RR, GRID><<<(unsigned)grid, kTraceThreads, 0, st>>>(a);                        \
-        break;
+    case RR: {                                                                                    \
+        auto kern = k_trace<T, RR, GRID>;                                                         \
+        const size_t dsm = dacc_smem_bytes<T, RR>();                                              \
+        if (dsm > 0) JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm)); \
+        kern<<<(unsigned)grid, kTraceThreads, dsm, st>>>(a);                                      \
+        break;                                                                                    \
+    }
 
 template <typename T, bool GRID>
 jt_status launch_trace_impl(const TraceArgs<T>& a, int R, cudaStream_t st) {

@@ -151,6 +151,67 @@ def test_convolve_delta_and_shift(jt):
     assert torch.equal(out[1:, 2:], img[:-1, :-2]) and float(out[0].abs().max()) == 0.0
 
 
+# ------------------------------------------------------------------ step 3: jt_psf_convolve (hand-written FFT)
+FFT_SHAPES = [(8, 8, 3, 3), (8, 8, 5, 3), (60, 60, 11, 11), (100, 100, 31, 31), (64, 64, 21, 21), (37, 91, 7, 13),
+              (130, 75, 45, 45), (5, 7, 11, 9), (200, 200, 21, 21), (33, 31, 1, 1), (180, 180, 135, 135),
+              (60, 60, 45, 45), (300, 420, 101, 101), (17, 1000, 3, 61), (1100, 9, 77, 5)]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("ny,nx,ky,kx", FFT_SHAPES)
+def test_convolve_fft(jt, orc, dtype, ny, nx, ky, kx):
+    """FFT path against the oracle's literal quadruple loop (the FFT reaches the direct result up to rounding)."""
+    rng = np.random.default_rng(ny * 1000 + nx + ky)
+    img = rng.uniform(0, 1, (ny, nx))
+    ker = rng.uniform(0, 1, (ky, kx))
+    ker /= ker.sum()
+    if dtype == "f32":
+        img, ker = _f32r(img), _f32r(ker)
+    got = jt.psf_convolve(to_dev(img, dtype), to_dev(ker, dtype), method="fft").double().cpu().numpy()
+    want = orc.convolve(img, ker)
+    # ~log2(Py Px) <= 24 butterfly levels, each adding one rounding of relative size eps to values of size <= max|img|
+    assert rel_err(got, want) < (1e-12 if dtype == "f64" else 2e-6)     # f32: transforms run in double, output rounding only
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_convolve_fft_vs_direct_vs_cufft(jt, dtype):
+    """Three-way agreement: own FFT path, direct path, and a cuFFT-based convolution (torch.fft; test only)."""
+    import torch
+    rng = np.random.default_rng(77)
+    ny, nx, ky, kx = 150, 170, 41, 37
+    img = to_dev(rng.uniform(0, 1, (ny, nx)), dtype)
+    ker = to_dev(rng.uniform(0, 1, (ky, kx)) / (ky * kx * 0.5), dtype)
+    a = jt.psf_convolve(img, ker, method="fft")
+    b = jt.psf_convolve(img, ker, method="direct")
+    sy, sx = ny + ky - 1, nx + kx - 1
+    full = torch.fft.irfft2(torch.fft.rfft2(img.double(), s=(sy, sx)) * torch.fft.rfft2(ker.double(), s=(sy, sx)), s=(sy, sx))
+    c = full[ky // 2:ky // 2 + ny, kx // 2:kx // 2 + nx]
+    tol = 1e-12 if dtype == "f64" else 2e-5
+    m = float(c.abs().max())
+    assert float((a.double() - c).abs().max()) < tol * m
+    assert float((b.double() - c).abs().max()) < tol * m
+    assert float((a.double() - b.double()).abs().max()) < tol * m
+
+
+def test_convolve_fft_delta_shift_and_auto(jt):
+    """delta kernel = identity and single-tap shift through the FFT path; AUTO resolves to a working method."""
+    import torch
+    rng = np.random.default_rng(6)
+    img = to_dev(rng.uniform(0, 1, (40, 50)), "f64")
+    k = torch.zeros(7, 5, dtype=torch.float64, device="cuda")
+    k[3, 2] = 1.0
+    assert float((jt.psf_convolve(img, k, method="fft") - img).abs().max()) < 1e-13
+    k.zero_()
+    k[3 + 1, 2 + 2] = 1.0
+    out = jt.psf_convolve(img, k, method="fft")
+    assert float((out[1:, 2:] - img[:-1, :-2]).abs().max()) < 1e-13 and float(out[0].abs().max()) < 1e-13
+    big = to_dev(rng.uniform(0, 1, (61, 61)), "f64")
+    big /= big.sum()
+    a = jt.psf_convolve(img, big, method="auto")
+    b = jt.psf_convolve(img, big, method="direct")
+    assert float((a - b).abs().max()) < 1e-13
+
+
 # ------------------------------------------------------------------ fused: jt_simulate_image
 def _check_image(jt, orc, w, method="auto", tol=None):
     pre, want = orc.simulate_image(w)
@@ -210,6 +271,24 @@ def test_c2_full_size_sampled_rows(jt, orc):
         for j in (0, 97, 163):
             want = orc.prepsf_rows(w, j, j + 1)[0]
             assert np.max(np.abs(got[j] - want)) < TOL_IMG[dtype] * scale, (dtype, j)
+
+
+def test_c4_full_size_sampled(jt, orc):
+    """Full-size C4 (500x500, s=5, 50,000 subhalos, f64, 101x101 AiryMix PSF) in the launch configuration bench.py
+    times.  (1) two pixel rows of the pre-PSF image, 40 pixels each spread over the row, against the oracle with all
+    50,002 deflectors; (2) both convolution methods on the FULL image: the oracle's direct convolution of the GPU's
+    pre-PSF image against the GPU's convolved images (SURVEY.md section 8(d) C4 plan)."""
+    w = workloads.config_c4(dtype="f64")
+    pre = gpu_simulate(jt, w, conv=False)
+    scale = np.max(np.abs(pre))
+    cols = np.linspace(0, w.nx - 1, 40).astype(int)
+    for j in (3, 251):
+        want = orc.prepsf_pixels(w, j, cols)
+        assert np.max(np.abs(pre[j, cols] - want)) < TOL_IMG["f64"] * scale, j
+    want = orc.convolve(pre, w.psf)
+    for method in ("direct", "fft"):
+        got = gpu_simulate(jt, w, method=method)
+        assert rel_err(got, want) < TOL_IMG["f64"], method
 
 
 # ------------------------------------------------------------------ batched: jt_simulate_batch

@@ -217,3 +217,13 @@ def test_workload_shapes_and_seeding():
     assert c4.psf.shape == (101, 101) and np.all(c4.psf > 0) and c4.sources.shape == (3, 7)
     full = workloads.config_c2()
     assert full.evals == 1_600_320_000
+
+
+def test_prepsf_pixels_matches_rows(orc):
+    """The pixel sampler used for full-size C4 parity equals the row routine on a small C4-shaped case."""
+    import workloads
+    w = workloads.config_c4(nx=12, n_tnfw=40, K=5, half_width=0.3)
+    rows = orc.prepsf_rows(w, 0, w.ny)
+    cols = np.array([0, 3, 7, 11])
+    for j in (0, 5, 11):
+        np.testing.assert_allclose(orc.prepsf_pixels(w, j, cols), rows[j, cols], rtol=1e-13, atol=0)
