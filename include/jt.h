@@ -154,6 +154,14 @@ JT_API jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid *gri
 JT_API jt_status jt_profile_enable(int on);
 JT_API jt_status jt_profile_read(float *trace_ms, float *conv_ms);
 
+/* Measurement aid: ALU peak microbenchmark (bench.py reports the measured rates beside the derived peaks of
+ * DESIGN.md section 6; MEASURED_PEAKS.json covers only HBM and tensor cores).  Launches `blocks` CTAs of 256
+ * threads, each thread running 8 independent chains of `kind` for iters * 4 rounds; *lane_ops (host, may be NULL)
+ * receives the number of thread-level instructions of that kind the launch executes (an FFMA2 counts once but
+ * performs two FMAs).  sink: device scratch of >= 4 bytes.  Time it with events on `stream`. */
+typedef enum { JT_PROBE_FFMA = 0, JT_PROBE_FFMA2 = 1, JT_PROBE_DFMA = 2, JT_PROBE_MUFU_RSQ = 3 } jt_probe_kind;
+JT_API jt_status jt_probe_alu(int32_t kind, int32_t blocks, int64_t iters, void *sink, int64_t *lane_ops, void *stream);
+
 /* Number of CUDA kernels this library has launched from the calling host thread since it was loaded
  * (bench.py's "gpu_launches" claim; memsets and event records are not counted). */
 JT_API uint64_t jt_kernel_launches(void);

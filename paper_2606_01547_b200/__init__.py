@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     lib,
     kernel_launches,
     lib_path,
+    probe_alu,
     profile_enable,
     profile_read,
     psf_convolve,

@@ -101,6 +101,7 @@ def lib():
         L.jt_kernel_launches.restype = ctypes.c_uint64
         L.jt_profile_enable.argtypes = [ctypes.c_int]
         L.jt_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
+        L.jt_probe_alu.argtypes = [i32, i32, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
     return _lib
 
@@ -124,6 +125,27 @@ def profile_read():
     a, b = ctypes.c_float(), ctypes.c_float()
     _check(lib().jt_profile_read(ctypes.byref(a), ctypes.byref(b)), "jt_profile_read")
     return a.value, b.value
+
+
+PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3}
+
+
+def probe_alu(kind, blocks=148 * 8, iters=4096, repeats=3):
+    """jt_probe_alu timed with CUDA events: returns thread-level instructions of `kind` per second (best of repeats)."""
+    import torch
+    sink = torch.zeros(4, dtype=torch.float32, device="cuda")
+    n = ctypes.c_int64()
+    st = torch.cuda.current_stream()
+    best = 0.0
+    for _ in range(repeats + 1):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(st)
+        _check(lib().jt_probe_alu(PROBE_KINDS[kind], blocks, iters, ctypes.c_void_p(sink.data_ptr()), ctypes.byref(n),
+                                  ctypes.c_void_p(st.cuda_stream)), "jt_probe_alu")
+        b.record(st)
+        b.synchronize()
+        best = max(best, n.value / (a.elapsed_time(b) * 1e-3))
+    return best
 
 
 # ------------------------------------------------------------------ marshalling helpers

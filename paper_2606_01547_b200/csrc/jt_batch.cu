@@ -14,7 +14,7 @@
 namespace jt {
 
 constexpr int kBatchRecCap = 512;            // subhalo records resident per staging round
-constexpr int kBatchTW = 32;                 // convolution: thread block covers kBatchTW columns x 8*OY rows
+constexpr int kBatchTW = 64;                 // convolution pass: 64 columns (32 lanes x 2) x 8 warps * OY rows
 constexpr int kBatchOY = 8;
 
 template <typename T>
@@ -63,11 +63,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     }
     if (conv) {
         for (int i = tid; i < a.pw * a.ph; i += kTraceThreads) img[i] = (T)0;
-        const T* K = a.psf + b * (int64_t)a.ky * a.kx;
-        for (int i = tid; i < a.kx * a.kyp; i += kTraceThreads) {
-            const int cb = i / a.kyp, ca = i % a.kyp;
-            Kc[i] = (ca < a.ky) ? K[(a.ky - 1 - ca) * a.kx + (a.kx - 1 - cb)] : (T)0;
-        }
+        stage_taps<T>(Kc, a.psf + b * (int64_t)a.ky * a.kx, a.ky, a.kx, a.kyp, -1, a.kx + 2, tid, kTraceThreads);
     }
     const RawTn<T> raw = {{a.tnfw + (b * 5 + 0) * a.M, a.tnfw + (b * 5 + 1) * a.M, a.tnfw + (b * 5 + 2) * a.M,
                            a.tnfw + (b * 5 + 3) * a.M, a.tnfw + (b * 5 + 4) * a.M}};
@@ -125,21 +121,23 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     if (!conv) return;
     __syncthreads();
 
-    // ---- step 5a out of shared memory ----
-    constexpr int TH = (kTraceThreads / kBatchTW) * kBatchOY;
-    const int il = tid % kBatchTW, jl0 = (tid / kBatchTW) * kBatchOY;
+    // ---- step 5a out of shared memory: passes of 64 columns x 64 rows, OY x 2 outputs per thread ----
+    constexpr int TH = (kTraceThreads / 32) * kBatchOY;
+    const int npairs = (a.kx + 1) / 2;
     for (int j0 = 0; j0 < a.ny; j0 += TH) {
         for (int i0 = 0; i0 < a.nx; i0 += kBatchTW) {
-            const int i = i0 + il;
-            if (i >= a.nx) continue;
-            T acc[kBatchOY];
+            T acc[kBatchOY][2];
 #pragma unroll
-            for (int r = 0; r < kBatchOY; ++r) acc[r] = (T)0;
-            conv_sweep<T, kBatchOY, false>(img + (j0 + jl0) * a.pw + i, a.pw, Kc, a.ky, a.kx, a.kyp, acc);
+            for (int r = 0; r < kBatchOY; ++r) { acc[r][0] = (T)0; acc[r][1] = (T)0; }
+            conv_sweep2<T, kBatchOY>(img + (size_t)(j0 + warp * kBatchOY) * a.pw + i0 + 2 * lane, a.pw, Kc, a.kyp, npairs, acc);
+            const int i = i0 + 2 * lane;
 #pragma unroll
             for (int r = 0; r < kBatchOY; ++r) {
-                const int j = j0 + jl0 + r;
-                if (j < a.ny) gout[(int64_t)j * a.nx + i] = acc[r];
+                const int j = j0 + warp * kBatchOY + r;
+                if (j < a.ny) {
+                    if (i < a.nx) gout[(int64_t)j * a.nx + i] = acc[r][0];
+                    if (i + 1 < a.nx) gout[(int64_t)j * a.nx + i + 1] = acc[r][1];
+                }
             }
         }
     }
@@ -149,7 +147,7 @@ constexpr size_t kBatchMaxSmem = 227 * 1024 - 4096 - 8192;      // static MacroL
 
 template <typename T>
 static size_t batch_smem_front(const BatchArgs<T>& a) {
-    return align_up((size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)a.kx * a.kyp) * sizeof(T), 16);
+    return align_up((size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)(a.kx + 2) * a.kyp) * sizeof(T), 16);
 }
 
 #define JT_BATCH_CASE(RR)                                                                              \
@@ -178,9 +176,9 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     const bool conv = p->ky > 0;
     a.ky = conv ? p->ky : 0; a.kx = conv ? p->kx : 0;
     a.kyp = (a.ky + 7) / 8 * 8;
-    constexpr int TH = (kTraceThreads / kBatchTW) * kBatchOY;
-    a.pw = conv ? g->nx + a.kx - 1 : 0;
-    a.ph = conv ? (g->ny + TH - 1) / TH * TH + a.ky - 1 : 0;
+    constexpr int TH = (kTraceThreads / 32) * kBatchOY;
+    a.pw = conv ? (g->nx + kBatchTW - 1) / kBatchTW * kBatchTW + a.kx - 1 : 0;        // even: pair loads stay aligned
+    a.ph = conv ? (g->ny + TH - 1) / TH * TH + a.kyp - 1 : 0;
     a.img_elems = (a.pw * a.ph + 3) / 4 * 4;
     a.rec_cap = a.M < kBatchRecCap ? (a.M > 0 ? a.M : 1) : kBatchRecCap;
     a.sie = (const T*)p->sie; a.shear = (const T*)p->shear; a.tnfw = (const T*)p->tnfw;

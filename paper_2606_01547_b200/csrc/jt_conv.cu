@@ -2,73 +2,88 @@
 //
 // out[j][i] = sum_a sum_b Kf[a][b] tile[jl+a][il+b],  Kf = kernel flipped in both axes (true convolution),
 // tile = image window with a (ky-1, kx-1) halo staged in shared memory, zero outside the image.
-// Each thread owns OY vertically adjacent outputs of one column: for a kernel column b it slides a
-// register window of OY tile values down the column, so one shared-memory load (lanes on consecutive
-// addresses: conflict-free) feeds OY FMAs; kernel taps are warp-uniform vector loads from a flipped,
-// column-major copy (Kc[b][a], built by k_flip_kernel in the workspace).  FMA : LDS = OY : 1.25.
+// CTA = NW warps; tile = 64 columns x NW*OY rows; a thread owns OY x 2 outputs (jt_conv.cuh: pair loads, register
+// window, 4 OY FMAs per shared load).  The flipped kernel is staged in shared memory by the CTA itself (no separate
+// flip launch, no workspace), whole when it fits beside the tile, else in bands of kernel-column pairs.
+// The host picks (OY, NW) so that the CTA count fills 148 SMs with the fewest, fullest waves.
 #include "jt_conv.cuh"
 
 namespace jt {
 
-template <typename T>
-__global__ void k_flip_kernel(int ky, int kx, int kyp, const T* __restrict__ K, T* __restrict__ Kc) {
-    const int n = kx * kyp;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const int b = i / kyp, a = i % kyp;
-        Kc[i] = (a < ky) ? K[(size_t)(ky - 1 - a) * kx + (kx - 1 - b)] : (T)0;
-    }
-}
+constexpr int kConvTW = 64;
+constexpr size_t kMaxSmem = 227 * 1024;
 
-template <typename T, int OY, int TW, int NTR>
-__global__ void __launch_bounds__(TW* NTR) k_conv_direct(int ny, int nx, const T* __restrict__ img, int ky, int kx,
-                                                         int kyp, const T* __restrict__ Kc, T* __restrict__ out) {
+template <typename T, int OY>
+__global__ void __launch_bounds__(256) k_conv_direct(int ny, int nx, const T* __restrict__ img, int ky, int kx, int kyp,
+                                                     int band_pairs, const T* __restrict__ K, T* __restrict__ out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nthr = blockDim.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int TH = (nthr >> 5) * OY;
+    const int tws = kConvTW + kx - 1;                 // even (kx odd)
+    const int ths = TH + kyp - 1;                     // rows below TH + ky - 1 only ever meet zero taps: zero-filled
     T* tile = reinterpret_cast<T*>(smem_raw);
-    constexpr int TH = NTR * OY;
-    const int tws = TW + kx - 1, ths = TH + ky - 1;
-    const int i0 = blockIdx.x * TW, j0 = blockIdx.y * TH;
+    T* Kc = reinterpret_cast<T*>(smem_raw + ((size_t)ths * tws * sizeof(T) + 15) / 16 * 16);
+    const int i0 = blockIdx.x * kConvTW, j0 = blockIdx.y * TH;
     const int col0 = i0 - (kx - 1 - kx / 2), row0 = j0 - (ky - 1 - ky / 2);
-    const int tid = threadIdx.x;
 
-    for (int idx = tid; idx < ths * tws; idx += TW * NTR) {
+    for (int idx = tid; idx < ths * tws; idx += nthr) {
         const int r = idx / tws, c = idx - r * tws;
         const int gj = row0 + r, gi = col0 + c;
-        tile[idx] = (gj >= 0 && gj < ny && gi >= 0 && gi < nx) ? __ldg(&img[(size_t)gj * nx + gi]) : (T)0;
+        tile[idx] = (r < TH + ky - 1 && gj >= 0 && gj < ny && gi >= 0 && gi < nx) ? __ldg(&img[(size_t)gj * nx + gi]) : (T)0;
     }
-    __syncthreads();
 
-    const int il = tid % TW, jl0 = (tid / TW) * OY;
-    T acc[OY];
+    T acc[OY][2];
 #pragma unroll
-    for (int r = 0; r < OY; ++r) acc[r] = (T)0;
-    conv_sweep<T, OY, true>(tile + jl0 * tws + il, tws, Kc, ky, kx, kyp, acc);
+    for (int r = 0; r < OY; ++r) { acc[r][0] = (T)0; acc[r][1] = (T)0; }
+    const T* tp0 = tile + (size_t)(warp * OY) * tws + 2 * lane;
+    const int npairs = (kx + 1) / 2;
+    for (int m0 = 0; m0 < npairs; m0 += band_pairs) {
+        const int mb = min(band_pairs, npairs - m0);
+        if (m0 > 0) __syncthreads();                  // every warp is done with the previous band's taps
+        stage_taps<T>(Kc, K, ky, kx, kyp, 2 * m0 - 1, 2 * mb + 1, tid, nthr);
+        __syncthreads();                              // taps (and, first time, the tile) are in place
+        conv_sweep2<T, OY>(tp0 + 2 * m0, tws, Kc, kyp, mb, acc);
+    }
 
-    const int i = i0 + il;
-    if (i < nx) {
+    const int i = i0 + 2 * lane;
 #pragma unroll
-        for (int r = 0; r < OY; ++r) {
-            const int j = j0 + jl0 + r;
-            if (j < ny) out[(size_t)j * nx + i] = acc[r];
+    for (int r = 0; r < OY; ++r) {
+        const int j = j0 + warp * OY + r;
+        if (j < ny) {
+            if (i < nx) out[(size_t)j * nx + i] = acc[r][0];
+            if (i + 1 < nx) out[(size_t)j * nx + i + 1] = acc[r][1];
         }
     }
 }
 
-constexpr size_t kMaxSmem = 227 * 1024;
+struct ConvCfg { int OY, NW, kyp, band_pairs; size_t smem; };
 
-struct ConvCfg { int OY, TW, NTR; size_t smem; };
-
-static bool pick_cfg(jt_dtype d, int ny, int nx, int ky, int kx, ConvCfg* c) {
+// Equal-work CTAs run in waves of 148: cost = waves x rows per CTA (x 1.1 for OY = 4: twice the shared loads per FMA).
+static bool pick_cfg(jt_dtype d, int ny, int nx, int ky, int kx, ConvCfg* best) {
     const size_t sz = dtype_size(d);
-    // wide tile first (better FMA:LDS), narrow tile when the halo would not fit
-    const ConvCfg cands[2] = {{8, 64, 4, 0}, {4, 32, 8, 0}};
-    for (int k = 0; k < 2; ++k) {
-        ConvCfg x = cands[k];
-        if (k == 0 && nx <= 32) continue;
-        x.smem = (size_t)(x.NTR * x.OY + ky - 1) * (size_t)(x.TW + kx - 1) * sz;
-        if (x.smem <= kMaxSmem) { *c = x; return true; }
+    const int npairs = (kx + 1) / 2;
+    double best_cost = -1.0;
+    for (int OY = 8; OY >= 4; OY -= 4) {
+        const int kyp = (ky + OY - 1) / OY * OY;
+        for (int NW = 8; NW >= 4; --NW) {
+            const int TH = NW * OY;
+            const size_t tile = align_up((size_t)(TH + kyp - 1) * (kConvTW + kx - 1) * sz, 16);
+            if (tile + (size_t)3 * kyp * sz > kMaxSmem) continue;
+            // taps: whole kernel if it fits (and stays under 48 KB so that small kernels leave room for several CTAs)
+            int bp = npairs;
+            const size_t tap_budget = kMaxSmem - tile < 48 * 1024 ? kMaxSmem - tile : 48 * 1024;
+            while (bp > 1 && (size_t)(2 * bp + 1) * kyp * sz > tap_budget) --bp;
+            const int64_t tiles = (int64_t)((nx + kConvTW - 1) / kConvTW) * ((ny + TH - 1) / TH);
+            const int64_t waves = (tiles + kNumSMs - 1) / kNumSMs;
+            const int n_bands = (npairs + bp - 1) / bp;
+            const double cost = (double)waves * TH * (OY == 8 ? 1.0 : 1.1) * (1.0 + 0.01 * (n_bands - 1));
+            if (best_cost < 0.0 || cost < best_cost) {
+                best_cost = cost;
+                *best = {OY, NW, kyp, bp, tile + (size_t)(2 * bp + 1) * kyp * sz};
+            }
+        }
     }
-    (void)ny;
-    return false;
+    return best_cost >= 0.0;
 }
 
 bool conv_direct_supported(jt_dtype d, int ny, int nx, int ky, int kx) {
@@ -76,41 +91,31 @@ bool conv_direct_supported(jt_dtype d, int ny, int nx, int ky, int kx) {
     return pick_cfg(d, ny, nx, ky, kx, &c);
 }
 
-size_t conv_direct_workspace_bytes(jt_dtype d, int ky, int kx) {
-    const int kyp = (ky + 7) / 8 * 8;
-    return align_up((size_t)kx * kyp * dtype_size(d), 256);
-}
+size_t conv_direct_workspace_bytes(jt_dtype, int, int) { return 0; }
 
-template <typename T, int OY, int TW, int NTR>
-static jt_status run_cfg(int ny, int nx, const T* img, int ky, int kx, int kyp, const T* Kc, T* out, size_t smem,
-                         cudaStream_t st) {
-    auto kern = k_conv_direct<T, OY, TW, NTR>;
-    JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    dim3 grid((nx + TW - 1) / TW, (ny + NTR * OY - 1) / (NTR * OY));
-    kern<<<grid, TW * NTR, smem, st>>>(ny, nx, img, ky, kx, kyp, Kc, out);
+template <typename T, int OY>
+static jt_status run_cfg(const ConvCfg& c, int ny, int nx, const T* img, int ky, int kx, const T* ker, T* out, cudaStream_t st) {
+    auto kern = k_conv_direct<T, OY>;
+    JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c.smem));
+    dim3 grid((nx + kConvTW - 1) / kConvTW, (ny + c.NW * OY - 1) / (c.NW * OY));
+    kern<<<grid, c.NW * 32, c.smem, st>>>(ny, nx, img, ky, kx, c.kyp, c.band_pairs, ker, out);
     JT_LAUNCH_CHECK();
     return JT_OK;
 }
 
 template <typename T>
-static jt_status conv_direct_t(jt_dtype d, int ny, int nx, const T* img, int ky, int kx, const T* ker, void* workspace,
-                               T* out, cudaStream_t st) {
+static jt_status conv_direct_t(jt_dtype d, int ny, int nx, const T* img, int ky, int kx, const T* ker, T* out, cudaStream_t st) {
     ConvCfg c;
     if (!pick_cfg(d, ny, nx, ky, kx, &c)) return JT_ERR_UNSUPPORTED;
-    const int kyp = (ky + 7) / 8 * 8;
-    T* Kc = (T*)workspace;
-    const int n = kx * kyp;
-    k_flip_kernel<T><<<(n + 255) / 256, 256, 0, st>>>(ky, kx, kyp, ker, Kc);
-    JT_LAUNCH_CHECK();
-    if (c.OY == 8) return run_cfg<T, 8, 64, 4>(ny, nx, img, ky, kx, kyp, Kc, out, c.smem, st);
-    return run_cfg<T, 4, 32, 8>(ny, nx, img, ky, kx, kyp, Kc, out, c.smem, st);
+    if (c.OY == 8) return run_cfg<T, 8>(c, ny, nx, img, ky, kx, ker, out, st);
+    return run_cfg<T, 4>(c, ny, nx, img, ky, kx, ker, out, st);
 }
 
 jt_status launch_conv_direct(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
                              void* workspace, void* out, cudaStream_t st) {
-    return dtype == JT_F32
-               ? conv_direct_t<float>(dtype, ny, nx, (const float*)img, ky, kx, (const float*)ker, workspace, (float*)out, st)
-               : conv_direct_t<double>(dtype, ny, nx, (const double*)img, ky, kx, (const double*)ker, workspace, (double*)out, st);
+    (void)workspace;
+    return dtype == JT_F32 ? conv_direct_t<float>(dtype, ny, nx, (const float*)img, ky, kx, (const float*)ker, (float*)out, st)
+                           : conv_direct_t<double>(dtype, ny, nx, (const double*)img, ky, kx, (const double*)ker, (double*)out, st);
 }
 
 }  // namespace jt

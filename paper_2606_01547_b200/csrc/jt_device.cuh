@@ -261,13 +261,13 @@ __host__ __device__ inline MacroLens derive_macro(int has_sie, double theta_E, d
 
 __device__ __forceinline__ double atanh_over(double z2) {      // atanh(z)/z as a function of z^2 in [0,1)
     if (z2 <= 0.25) return atanh_q(z2);
-    const double z = sqrt(z2);
-    return 0.5 * log((1.0 + z) / (1.0 - z)) / z;
+    const double iz = fast_rsqrt(z2), z = z2 * iz;             // no libdevice sqrt / log / division slow paths
+    return 0.5 * ln_pos((1.0 + z) * fast_rcp(1.0 - z)) * iz;
 }
 
 __device__ __forceinline__ double atan_over(double z2) {       // atan(z)/z as a function of z^2 >= 0
     if (z2 <= 1.0) return atan_full(z2);
-    const double iz2 = 1.0 / z2, iz = sqrt(iz2);               // atan z = pi/2 - atan(1/z)
+    const double iz = fast_rsqrt(z2), iz2 = iz * iz;           // atan z = pi/2 - atan(1/z)
     return fma(JT_PI_D / 2, iz, -atan_full(iz2) * iz2);
 }
 

@@ -16,7 +16,7 @@ def _declared():
 
 def test_header_symbols_exported(jt):
     names = _declared()
-    assert len(names) == 14, names
+    assert len(names) == 15, names
     L = ctypes.CDLL(jt.lib_path())
     for n in names:
         assert hasattr(L, n), n
@@ -50,10 +50,12 @@ def test_argument_validation_without_device(jt):
     assert L.jt_ray_shoot(1, 10, dummy, dummy, ctypes.byref(lens), None, 0, ctypes.c_void_p(512), ctypes.c_void_p(768), None) == 1
     lens.n_tnfw = 0
     assert L.jt_ray_shoot(1, -1, dummy, dummy, ctypes.byref(lens), None, 0, ctypes.c_void_p(512), ctypes.c_void_p(768), None) == 1
-    # workspace too small: direct conv needs scratch for the flipped kernel
-    need = L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 1)
-    assert need >= 21 * 21 * 8
-    assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 1, dummy, need - 1, ctypes.c_void_p(512), None) == 3
+    # workspace too small: the FFT path needs its complex plane (the direct path needs none)
+    assert L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 1) == 0
+    need = L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 2)
+    assert need >= 128 * 128 * 16
+    assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 2, dummy, need - 1, ctypes.c_void_p(512), None) == 3
+    assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 2, None, 0, ctypes.c_void_p(512), None) == 3
     # zero-sized problems are no-ops
     assert L.jt_ray_shoot(1, 0, None, None, ctypes.byref(lens), None, 0, None, None, None) == 0
     del keep
