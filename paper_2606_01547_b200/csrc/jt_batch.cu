@@ -15,7 +15,7 @@ namespace jt {
 
 constexpr int kBatchRecCap = 512;            // subhalo records resident per staging round
 constexpr int kBatchTW = 64;                 // convolution pass: 64 columns (32 lanes x 2) x 8 warps * OY rows
-constexpr int kBatchOY = 8;
+template <typename T> struct BatchOY { static constexpr int value = sizeof(T) == 4 ? 8 : 4; };   // as in jt_conv.cu
 
 template <typename T>
 struct BatchArgs {
@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     }
     if (conv) {
         for (int i = tid; i < a.pw * a.ph; i += kTraceThreads) img[i] = (T)0;
-        stage_taps<T>(Kc, a.psf + b * (int64_t)a.ky * a.kx, a.ky, a.kx, a.kyp, -1, a.kx + 2, tid, kTraceThreads);
+        stage_taps<T>(Kc, a.psf + b * (int64_t)a.ky * a.kx, a.ky, a.kx, a.kyp, 0, (a.kx + 1) / 2, tid, kTraceThreads);
     }
     const RawTn<T> raw = {{a.tnfw + (b * 5 + 0) * a.M, a.tnfw + (b * 5 + 1) * a.M, a.tnfw + (b * 5 + 2) * a.M,
                            a.tnfw + (b * 5 + 3) * a.M, a.tnfw + (b * 5 + 4) * a.M}};
@@ -122,21 +122,21 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     __syncthreads();
 
     // ---- step 5a out of shared memory: passes of 64 columns x 64 rows, OY x 2 outputs per thread ----
+    constexpr int kBatchOY = BatchOY<T>::value;
     constexpr int TH = (kTraceThreads / 32) * kBatchOY;
     const int npairs = (a.kx + 1) / 2;
     for (int j0 = 0; j0 < a.ny; j0 += TH) {
         for (int i0 = 0; i0 < a.nx; i0 += kBatchTW) {
-            T acc[kBatchOY][2];
-#pragma unroll
-            for (int r = 0; r < kBatchOY; ++r) { acc[r][0] = (T)0; acc[r][1] = (T)0; }
-            conv_sweep2<T, kBatchOY>(img + (size_t)(j0 + warp * kBatchOY) * a.pw + i0 + 2 * lane, a.pw, Kc, a.kyp, npairs, acc);
+            ConvAcc<T, kBatchOY> acc;
+            acc.zero();
+            acc.sweep(img + (size_t)(j0 + warp * kBatchOY) * a.pw + i0 + 2 * lane, a.pw, Kc, a.kyp, npairs);
             const int i = i0 + 2 * lane;
 #pragma unroll
             for (int r = 0; r < kBatchOY; ++r) {
                 const int j = j0 + warp * kBatchOY + r;
                 if (j < a.ny) {
-                    if (i < a.nx) gout[(int64_t)j * a.nx + i] = acc[r][0];
-                    if (i + 1 < a.nx) gout[(int64_t)j * a.nx + i + 1] = acc[r][1];
+                    if (i < a.nx) gout[(int64_t)j * a.nx + i] = acc.col0(r);
+                    if (i + 1 < a.nx) gout[(int64_t)j * a.nx + i + 1] = acc.col1(r);
                 }
             }
         }
@@ -147,7 +147,7 @@ constexpr size_t kBatchMaxSmem = 227 * 1024 - 4096 - 8192;      // static MacroL
 
 template <typename T>
 static size_t batch_smem_front(const BatchArgs<T>& a) {
-    return align_up((size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)(a.kx + 2) * a.kyp) * sizeof(T), 16);
+    return align_up((size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)4 * ((a.kx + 1) / 2) * a.kyp) * sizeof(T), 16);
 }
 
 #define JT_BATCH_CASE(RR)                                                                              \
@@ -175,7 +175,8 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.M = p->n_tnfw; a.n_src = p->n_src;
     const bool conv = p->ky > 0;
     a.ky = conv ? p->ky : 0; a.kx = conv ? p->kx : 0;
-    a.kyp = (a.ky + 7) / 8 * 8;
+    constexpr int kBatchOY = BatchOY<T>::value;
+    a.kyp = (a.ky + kBatchOY - 1) / kBatchOY * kBatchOY;
     constexpr int TH = (kTraceThreads / 32) * kBatchOY;
     a.pw = conv ? (g->nx + kBatchTW - 1) / kBatchTW * kBatchTW + a.kx - 1 : 0;        // even: pair loads stay aligned
     a.ph = conv ? (g->ny + TH - 1) / TH * TH + a.kyp - 1 : 0;

@@ -3,7 +3,7 @@
 // out[j][i] = sum_a sum_b Kf[a][b] tile[jl+a][il+b],  Kf = kernel flipped in both axes (true convolution),
 // tile = image window with a (ky-1, kx-1) halo staged in shared memory, zero outside the image.
 // CTA = NW warps; tile = 64 columns x NW*OY rows; a thread owns OY x 2 outputs (jt_conv.cuh: pair loads, register
-// window, 4 OY FMAs per shared load).  The flipped kernel is staged in shared memory by the CTA itself (no separate
+// window, 4 OY FMAs per shared load; float: packed FFMA2).  The flipped kernel is staged in shared memory by the CTA itself (no separate
 // flip launch, no workspace), whole when it fits beside the tile, else in bands of kernel-column pairs.
 // The host picks (OY, NW) so that the CTA count fills 148 SMs with the fewest, fullest waves.
 #include "jt_conv.cuh"
@@ -32,17 +32,16 @@ __global__ void __launch_bounds__(256) k_conv_direct(int ny, int nx, const T* __
         tile[idx] = (r < TH + ky - 1 && gj >= 0 && gj < ny && gi >= 0 && gi < nx) ? __ldg(&img[(size_t)gj * nx + gi]) : (T)0;
     }
 
-    T acc[OY][2];
-#pragma unroll
-    for (int r = 0; r < OY; ++r) { acc[r][0] = (T)0; acc[r][1] = (T)0; }
+    ConvAcc<T, OY> acc;
+    acc.zero();
     const T* tp0 = tile + (size_t)(warp * OY) * tws + 2 * lane;
     const int npairs = (kx + 1) / 2;
     for (int m0 = 0; m0 < npairs; m0 += band_pairs) {
         const int mb = min(band_pairs, npairs - m0);
         if (m0 > 0) __syncthreads();                  // every warp is done with the previous band's taps
-        stage_taps<T>(Kc, K, ky, kx, kyp, 2 * m0 - 1, 2 * mb + 1, tid, nthr);
+        stage_taps<T>(Kc, K, ky, kx, kyp, m0, mb, tid, nthr);
         __syncthreads();                              // taps (and, first time, the tile) are in place
-        conv_sweep2<T, OY>(tp0 + 2 * m0, tws, Kc, kyp, mb, acc);
+        acc.sweep(tp0 + 2 * m0, tws, Kc, kyp, mb);
     }
 
     const int i = i0 + 2 * lane;
@@ -50,8 +49,8 @@ __global__ void __launch_bounds__(256) k_conv_direct(int ny, int nx, const T* __
     for (int r = 0; r < OY; ++r) {
         const int j = j0 + warp * OY + r;
         if (j < ny) {
-            if (i < nx) out[(size_t)j * nx + i] = acc[r][0];
-            if (i + 1 < nx) out[(size_t)j * nx + i + 1] = acc[r][1];
+            if (i < nx) out[(size_t)j * nx + i] = acc.col0(r);
+            if (i + 1 < nx) out[(size_t)j * nx + i + 1] = acc.col1(r);
         }
     }
 }
@@ -63,23 +62,23 @@ static bool pick_cfg(jt_dtype d, int ny, int nx, int ky, int kx, ConvCfg* best) 
     const size_t sz = dtype_size(d);
     const int npairs = (kx + 1) / 2;
     double best_cost = -1.0;
-    for (int OY = 8; OY >= 4; OY -= 4) {
+    for (int OY = (d == JT_F64 ? 4 : 8); OY >= 4; OY -= 4) {       // double: OY = 4 only (register budget of the pipelined sweep)
         const int kyp = (ky + OY - 1) / OY * OY;
         for (int NW = 8; NW >= 4; --NW) {
             const int TH = NW * OY;
             const size_t tile = align_up((size_t)(TH + kyp - 1) * (kConvTW + kx - 1) * sz, 16);
-            if (tile + (size_t)3 * kyp * sz > kMaxSmem) continue;
+            if (tile + (size_t)4 * kyp * sz > kMaxSmem) continue;
             // taps: whole kernel if it fits (and stays under 48 KB so that small kernels leave room for several CTAs)
             int bp = npairs;
             const size_t tap_budget = kMaxSmem - tile < 48 * 1024 ? kMaxSmem - tile : 48 * 1024;
-            while (bp > 1 && (size_t)(2 * bp + 1) * kyp * sz > tap_budget) --bp;
+            while (bp > 1 && (size_t)4 * bp * kyp * sz > tap_budget) --bp;
             const int64_t tiles = (int64_t)((nx + kConvTW - 1) / kConvTW) * ((ny + TH - 1) / TH);
             const int64_t waves = (tiles + kNumSMs - 1) / kNumSMs;
             const int n_bands = (npairs + bp - 1) / bp;
             const double cost = (double)waves * TH * (OY == 8 ? 1.0 : 1.1) * (1.0 + 0.01 * (n_bands - 1));
             if (best_cost < 0.0 || cost < best_cost) {
                 best_cost = cost;
-                *best = {OY, NW, kyp, bp, tile + (size_t)(2 * bp + 1) * kyp * sz};
+                *best = {OY, NW, kyp, bp, tile + (size_t)4 * bp * kyp * sz};
             }
         }
     }
@@ -107,7 +106,9 @@ template <typename T>
 static jt_status conv_direct_t(jt_dtype d, int ny, int nx, const T* img, int ky, int kx, const T* ker, T* out, cudaStream_t st) {
     ConvCfg c;
     if (!pick_cfg(d, ny, nx, ky, kx, &c)) return JT_ERR_UNSUPPORTED;
-    if (c.OY == 8) return run_cfg<T, 8>(c, ny, nx, img, ky, kx, ker, out, st);
+    if constexpr (sizeof(T) == 4) {
+        if (c.OY == 8) return run_cfg<T, 8>(c, ny, nx, img, ky, kx, ker, out, st);
+    }
     return run_cfg<T, 4>(c, ny, nx, img, ky, kx, ker, out, st);
 }
 
