@@ -39,7 +39,7 @@ SM_COUNT = 148
 # Algorithmic work per evaluation on the binding unit: counted in the SASS of the warp-uniform
 # far-field loop (loop head + far body) divided by its 8 rays.  f32: issue slots (the issue port and the FP32 pipe both
 # run 128 lanes/clk/SM, the port binds); f64: FP64-pipe instructions (64 lanes/clk/SM, the pipe binds).
-ALG_INSTR_PER_EVAL = {"f32": 35.1, "f64": 51.75}
+ALG_INSTR_PER_EVAL = {"f32": 34.25, "f64": 51.6}      # 274 / 8 issue slots; 413 / 8 FP64-pipe instructions
 ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
 
@@ -389,14 +389,39 @@ def run_ours(args, rank, world, local_rank):
         "kernel_share_of_step": trace_ms / (ms_total_local / args.steps),
         "frac_at_observed_clock": achieved / (SM_COUNT * lanes * f_mhz * 1e6 / 1e12),
         "evals_per_s_kernel": w.evals / (trace_ms * 1e-3)}
+    # ---- ALU rates measured in this run by the library's microbenchmark (thread-level instructions / s) ----
+    probes = {k: jt.probe_alu(k) for k in ("ffma", "ffma2", "dfma", "mufu_rsq")}
+    line["alu_peaks_measured"] = {k: {"Tlaneinstr_per_s": v / 1e12, "lanes_per_clk_per_sm_at_max_clock":
+                                      v / SM_COUNT / (peaks.get("sm_max_mhz", 1965.0) * 1e6)} for k, v in probes.items()}
+    meas = probes["ffma"] if w.dtype == "f32" else probes["dfma"]
+    line["roofline"]["frac_of_measured_alu_rate"] = achieved * 1e12 / meas
     if not batch:
-        K = w.psf.shape[0] * w.psf.shape[1]
+        ky, kx = w.psf.shape
+        K = ky * kx
         esz = 4 if w.dtype == "f32" else 8
         lanes = 128 if w.dtype == "f32" else 64
         fma_peak = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6
-        line["conv"] = {"method": args.method, "ms": conv_ms,
-                        "gbs": (2 * w.nx * w.ny + K) * esz / (conv_ms * 1e-3) / 1e9 if conv_ms > 0 else None,
-                        "fma_frac": w.nx * w.ny * K / (conv_ms * 1e-3) / fma_peak if conv_ms > 0 else None}
+        method = args.method
+        if method == "auto":
+            method = "fft" if K > 41 * 41 else "direct"          # jt_api.cu resolve_conv_method
+        conv = {"method": method, "ms": conv_ms,
+                "gbs_algorithmic": (2 * w.nx * w.ny + K) * esz / (conv_ms * 1e-3) / 1e9 if conv_ms > 0 else None}
+        if conv_ms > 0 and method == "direct":
+            conv.update({"bound": "alu", "fma_per_s": w.nx * w.ny * K / (conv_ms * 1e-3),
+                         "frac_of_derived_fma_peak": w.nx * w.ny * K / (conv_ms * 1e-3) / fma_peak,
+                         "frac_of_measured_fma_rate": w.nx * w.ny * K / (conv_ms * 1e-3) /
+                                                      (2 * probes["ffma2"] if w.dtype == "f32" else probes["dfma"])})
+        elif conv_ms > 0:
+            # FFT path: image in + image out + kernel in, plus the complex-double plane written by the row pass, read and
+            # written (cropped rows only) by the column pass and read by the inverse row pass
+            p2 = lambda v: 1 << max(4, int(np.ceil(np.log2(v))))
+            Px, Py = p2(w.nx + kx - 1), p2(w.ny + ky - 1)
+            plane = 16 * Px * (2 * max(w.ny, ky) + 2 * w.ny)
+            nbytes = (2 * w.nx * w.ny + K) * esz + plane
+            conv.update({"bound": "hbm", "bytes": nbytes, "gbs": nbytes / (conv_ms * 1e-3) / 1e9,
+                         "frac_of_measured_hbm": nbytes / (conv_ms * 1e-3) / 1e9 / peaks.get("hbm_gbs", 6650.0),
+                         "pad": "%dx%d" % (Py, Px)})
+        line["conv"] = conv
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_evals)
     print(json.dumps(line), flush=True)

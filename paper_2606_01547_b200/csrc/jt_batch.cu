@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
         for (int i0 = 0; i0 < a.nx; i0 += kBatchTW) {
             ConvAcc<T, kBatchOY> acc;
             acc.zero();
-            acc.sweep(img + (size_t)(j0 + warp * kBatchOY) * a.pw + i0 + 2 * lane, a.pw, Kc, a.kyp, npairs);
+            acc.template sweep<false>(img + (size_t)(j0 + warp * kBatchOY) * a.pw + i0 + 2 * lane, a.pw, Kc, a.kyp, npairs);
             const int i = i0 + 2 * lane;
 #pragma unroll
             for (int r = 0; r < kBatchOY; ++r) {

@@ -113,6 +113,9 @@ struct ConvAcc {
             for (int r = 0; r < OY; ++r) O::fma_y(v[r], t[aa], win[(aa + r) % OY]);
         }
     }
+    // PIPE = false: loads issue in program order, one kernel row at a time (enough when >= 4 warps per scheduler are
+    // resident, as in the batch kernel, and much lighter on registers).
+    template <bool PIPE = true>
     __device__ __forceinline__ void sweep(const T* __restrict__ tp0, int tws, const T* __restrict__ Kq, int kyp, int npairs) {
 #pragma unroll 1
         for (int m = 0; m < npairs; ++m) {
@@ -121,6 +124,23 @@ struct ConvAcc {
             typename O::Win win[OY];
 #pragma unroll
             for (int r = 0; r < OY - 1; ++r) { win[r] = *reinterpret_cast<const typename O::Win*>(wp); wp += tws; }
+            if constexpr (!PIPE) {
+#pragma unroll 1
+                for (int a0 = 0; a0 < kyp; a0 += OY) {
+#pragma unroll
+                    for (int aa = 0; aa < OY; ++aa) {
+                        const typename O::Tap t = O::load_tap(kp + 4 * aa);
+                        win[(aa + OY - 1) % OY] = *reinterpret_cast<const typename O::Win*>(wp);
+                        wp += tws;
+#pragma unroll
+                        for (int r = 0; r < OY; ++r) O::fma_x(v[r], t, win[(aa + r) % OY]);
+#pragma unroll
+                        for (int r = 0; r < OY; ++r) O::fma_y(v[r], t, win[(aa + r) % OY]);
+                    }
+                    kp += 4 * OY;
+                }
+                continue;
+            }
             typename O::Tap tA[OY], tB[OY];
             typename O::Win wA[OY], wB[OY];
             load_chunk(tA, wA, kp, wp, tws);
