@@ -69,54 +69,65 @@ __device__ __forceinline__ double t_log(double x) { return log(x); }
 //   brace = (t-1+2X^2) F(X) + c1 + S (c2 L - pi),  t = tau^2, c1 = tau pi + (t-1) ln tau, c2 = (t-1)/tau,
 //   S = sqrt(t+X^2), L = ln(X/(S+tau)).
 // ------------------------------------------------------------------------------------------------
+// The hot loops read the first nine fields (amplitude folded into the brace coefficients: one multiply per evaluation
+// less); the generic near-field forms read amp, tm1, c1.
 template <typename T>
-struct alignas(sizeof(T) * 8) SubRec {
-    T cx, cy, iRs2, thr;      // centre, 1/Rs^2, far-field threshold on X^2 (= max(10, 3t))
-    T t, c1, amp, tm1;        // tau^2, c1, amplitude, tau^2 - 1
+struct alignas(sizeof(T) * 4) SubRec {
+    T cx, cy, iRs2, thr;       // centre, 1/Rs^2, far-field threshold on X^2 (= max(10, 3t))
+    T t, a_tm1, a_c1, a_pi;    // tau^2, amp (t-1), amp c1, amp pi
+    T a_m2, amp, tm1, c1;      // -2 amp, amplitude, tau^2 - 1, c1
 };
 
 template <typename T>
 __device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, double aRs, double rt) {
     const double tau = rt / Rs, t = tau * tau;
+    const double c1 = tau * JT_PI_D + (t - 1.0) * log(tau);
+    const double amp = aRs / (1.0 - JT_LN2_D) * Rs * t / ((t + 1.0) * (t + 1.0));
     SubRec<T> r;
     r.cx = (T)cx;
     r.cy = (T)cy;
     r.iRs2 = (T)(1.0 / (Rs * Rs));
     r.thr = (T)fmax(10.0, 3.0 * t);
     r.t = (T)t;
-    r.c1 = (T)(tau * JT_PI_D + (t - 1.0) * log(tau));
-    r.amp = (T)(aRs / (1.0 - JT_LN2_D) * Rs * t / ((t + 1.0) * (t + 1.0)));
+    r.a_tm1 = (T)(amp * (t - 1.0));
+    r.a_c1 = (T)(amp * c1);
+    r.a_pi = (T)(amp * JT_PI_D);
+    r.a_m2 = (T)(-2.0 * amp);
+    r.amp = (T)amp;
     r.tm1 = (T)(t - 1.0);
+    r.c1 = (T)c1;
     return r;
 }
 // padding record: contributes exactly 0 and always takes the far path
 template <typename T>
 __device__ __forceinline__ SubRec<T> null_rec() {
     SubRec<T> r;
-    r.cx = (T)1e6; r.cy = (T)1e6; r.iRs2 = (T)1; r.thr = (T)10; r.t = (T)1; r.c1 = (T)0; r.amp = (T)0; r.tm1 = (T)0;
+    r.cx = (T)1e6; r.cy = (T)1e6; r.iRs2 = (T)1; r.thr = (T)10; r.t = (T)1;
+    r.a_tm1 = (T)0; r.a_c1 = (T)0; r.a_pi = (T)0; r.a_m2 = (T)0; r.amp = (T)0; r.tm1 = (T)0; r.c1 = (T)0;
     return r;
 }
 
 // Far field, X^2 >= max(10, 3t): no logarithm, no cancellation growing with X.
 //   w = 1/sqrt(X^2-1), z = w^2 <= 1/9, y = t/(X^2+t) <= 1/4,  P = atan(w)/w, Q = atanh(sqrt y)/sqrt y
-//   F = (pi/2 - w P) w;   S c2 L = -(t-1) Q;   2 X^2 F - pi S = pi (w + u - S) - 2 (1+z) P
-//   brace = (t-1)(F - Q) + c1 + pi (w + u - S) - 2 (1+z) P
+//   F = (pi/2 - w P) w;   S c2 L = -(t-1) Q;   2 X^2 F - pi S = pi (w X^2 - S) - 2 (1+z) P      (w + u = w X^2)
+//   amp brace = a_tm1 (F - Q) + a_c1 + a_pi (w X^2 - S) + a_m2 (1+z) P
 // Returns f with alpha = f * (dx, dy).
 template <typename T>
 __device__ __forceinline__ T tnfw_far(T R2, const SubRec<T>& s) {
-    const T u2 = fma(R2, s.iRs2, (T)-1);
-    const T S2 = fma(R2, s.iRs2, s.t);
+    const T X2 = R2 * s.iRs2;
+    const T u2 = X2 - (T)1;
+    const T S2 = X2 + s.t;
     const T w = fast_rsqrt(u2);
     const T rS = fast_rsqrt(S2);
     const T iR2 = approx_rcp(R2);
-    const T u = u2 * w, S = S2 * rS, z = w * w, y = (s.t * rS) * rS;
+    const T S = S2 * rS, z = w * w, y = (s.t * rS) * rS;
     const T P = atan_far(z);
     const T Q = atanh_q(y);
     const T F = fma(-w, P, (T)(JT_PI_D / 2)) * w;
-    T b = fma(s.tm1, F - Q, s.c1);
-    b = fma((T)JT_PI_D, (w + u) - S, b);
-    b = fma((T)-2, fma(z, P, P), b);
-    return (s.amp * b) * iR2;
+    T b = fma(s.a_tm1, F - Q, s.a_c1);
+    b = fma(s.a_pi, fma(w, X2, -S), b);
+    b = fma(s.a_m2, fma(z, P, P), b);
+    return b * iR2;
 }
 
 // ln x for normal positive x.  float: one MUFU.LG2.  double: x = 2^e m, m in (sqrt(1/2), sqrt 2],
@@ -156,15 +167,15 @@ __device__ __forceinline__ T tnfw_midfast(T R2, const SubRec<T>& s) {
     const T rt = fast_rsqrt(s.t);
     const T iR2 = approx_rcp(R2);
     const T iX2 = approx_rcp(X2);
-    const T u = u2 * w, S = S2 * rS, tau = s.t * rt, z = w * w;
+    const T S = S2 * rS, tau = s.t * rt, z = w * w;
     const T P = atan_full(z);
     const T F = fma(-w, P, (T)(JT_PI_D / 2)) * w;
     const T d = S + tau;
     const T Q = (S * rt) * ((T)0.5 * ln_pos((d * d) * iX2));
-    T b = fma(s.tm1, F - Q, s.c1);
-    b = fma((T)JT_PI_D, (w + u) - S, b);
-    b = fma((T)-2, fma(z, P, P), b);
-    return (s.amp * b) * iR2;
+    T b = fma(s.a_tm1, F - Q, s.a_c1);
+    b = fma(s.a_pi, fma(w, X2, -S), b);
+    b = fma(s.a_m2, fma(z, P, P), b);
+    return b * iR2;
 }
 
 // Closed form for any X^2 > 0 (float: use only for X^2 >= 1/4; double: X^2 >= 1e-6).
