@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(256) k_conv_direct(int ny, int nx, const T* __
         if (m0 > 0) __syncthreads();                  // every warp is done with the previous band's taps
         stage_taps<T>(Kc, K, ky, kx, kyp, m0, mb, tid, nthr);
         __syncthreads();                              // taps (and, first time, the tile) are in place
-        acc.sweep(tp0 + 2 * m0, tws, Kc, kyp, mb);
+        acc.template sweep<true>(tp0 + 2 * m0, tws, Kc, kyp, mb);
     }
 
     const int i = i0 + 2 * lane;
@@ -62,7 +62,7 @@ static bool pick_cfg(jt_dtype d, int ny, int nx, int ky, int kx, ConvCfg* best) 
     const size_t sz = dtype_size(d);
     const int npairs = (kx + 1) / 2;
     double best_cost = -1.0;
-    for (int OY = (d == JT_F64 ? 4 : 8); OY >= 4; OY -= 4) {       // double: OY = 4 only (register budget of the pipelined sweep)
+    for (int OY = (d == JT_F64 ? 4 : 8); OY >= 4; OY -= 4) {
         const int kyp = (ky + OY - 1) / OY * OY;
         for (int NW = 8; NW >= 4; --NW) {
             const int TH = NW * OY;

@@ -64,6 +64,32 @@ __global__ void __launch_bounds__(256) k_probe(int64_t iters, float seed, float*
 #pragma unroll
         for (int c = 0; c < kProbeChains; ++c) s += v[c];
         if (s == 123.456) sink[0] = (float)s;
+    } else if constexpr (KIND == JT_PROBE_FFMA2_RF) {
+        // the direct convolution's operand pattern: 8 accumulators x 4 packed taps x 8 broadcast tile values, all in
+        // distinct registers (5 register reads per FFMA2, only the tap reusable)
+        unsigned long long acc[8], t[4];
+        float w[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) { acc[c] = 0ull; w[c] = a0 * (float)(c + 1); }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            const float x = 1e-3f * (float)(c + 1) * seed;
+            t[c] = ((unsigned long long)__float_as_uint(x) << 32) | __float_as_uint(-x);
+        }
+        for (int64_t i = 0; i < iters; ++i) {
+#pragma unroll
+            for (int u = 0; u < kProbeUnroll; ++u)
+#pragma unroll
+                for (int c = 0; c < kProbeChains; ++c) {
+                    unsigned long long wb;
+                    asm volatile("mov.b64 %0, {%1, %1};" : "=l"(wb) : "f"(w[(c + u) % 8]));
+                    asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[c]) : "l"(t[u]), "l"(wb));
+                }
+        }
+        unsigned long long s = 0;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) s ^= acc[c];
+        if (s == 0x123456789abcdefull) sink[0] = 1.f;
     } else {   // JT_PROBE_MUFU_RSQ
         float v[kProbeChains];
 #pragma unroll
@@ -92,6 +118,7 @@ extern "C" jt_status jt_probe_alu(int32_t kind, int32_t blocks, int64_t iters, v
         case JT_PROBE_FFMA: k_probe<JT_PROBE_FFMA><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_FFMA2: k_probe<JT_PROBE_FFMA2><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_DFMA: k_probe<JT_PROBE_DFMA><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
+        case JT_PROBE_FFMA2_RF: k_probe<JT_PROBE_FFMA2_RF><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_MUFU_RSQ: k_probe<JT_PROBE_MUFU_RSQ><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         default: return JT_ERR_UNSUPPORTED;
     }
