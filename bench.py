@@ -402,8 +402,8 @@ def run_ours(args, rank, world, local_rank):
         lanes = 128 if w.dtype == "f32" else 64
         fma_peak = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6
         method = args.method
-        if method == "auto":
-            method = "fft" if K > 41 * 41 else "direct"          # jt_api.cu resolve_conv_method
+        if method == "auto":                                       # what jt_api.cu's resolve_conv_method picked
+            method = "fft" if jt.psf_convolve_workspace_bytes(w.dtype, w.ny, w.nx, ky, kx, "auto") > 0 else "direct"
         conv = {"method": method, "ms": conv_ms,
                 "gbs_algorithmic": (2 * w.nx * w.ny + K) * esz / (conv_ms * 1e-3) / 1e9 if conv_ms > 0 else None}
         if conv_ms > 0 and method == "direct":
@@ -427,6 +427,69 @@ def run_ours(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
 
 
+def run_conv_sweep(args, rank):
+    """--conv-sweep: jt_psf_convolve alone at the paper's E3 shapes (60x60 with K = 3..45, 180x180 with
+    K = 9..135; 100x100 with K = 13) plus the configs' shapes, float32 and float64, DIRECT and FFT.
+    Each case is captured into a CUDA graph of 20 back-to-back calls and the graph replay is timed with CUDA events, so
+    the number is device time per call, not the Python binding's per-call cost.  Prints one JSON line."""
+    if rank != 0:
+        return
+    import torch
+    import paper_2606_01547_b200 as jt
+    import workloads
+    torch.cuda.set_device(0)
+    jt.lib()
+    peaks, _ = load_peaks()
+    rng = np.random.default_rng(workloads.SEEDS["sweep"])
+    shapes = [(60, k) for k in (3, 11, 21, 31, 45)] + [(180, k) for k in (9, 45, 87, 135)] + \
+             [(100, 13), (100, 31), (200, 21), (500, 101), (1000, 31)]
+    reps = 20
+    rows = []
+    side = torch.cuda.Stream()
+    for dtype, tdt, lanes, esz in (("f32", torch.float32, 128, 4), ("f64", torch.float64, 64, 8)):
+        fma_peak = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6
+        for n, k in shapes:
+            img = torch.as_tensor(rng.uniform(0, 1, (n, n)), dtype=tdt, device="cuda")
+            sig = k / 8.0
+            u = np.arange(k) - k // 2
+            ker = np.exp(-(u[:, None] ** 2 + u[None, :] ** 2) / (2 * sig * sig))
+            ker = torch.as_tensor(ker / ker.sum(), dtype=tdt, device="cuda")
+            out = torch.empty_like(img)
+            row = {"dtype": dtype, "n": n, "K": k}
+            for method in ("direct", "fft", "auto"):
+                try:
+                    nb = jt.psf_convolve_workspace_bytes(dtype, n, n, k, k, method)
+                    ws = torch.empty(max(nb, 1), dtype=torch.uint8, device="cuda")
+                    call = lambda: jt.psf_convolve(img, ker, method=method, workspace=ws, out=out)
+                    with torch.cuda.stream(side):
+                        for _ in range(3):
+                            call()
+                        torch.cuda.synchronize()
+                        g = torch.cuda.CUDAGraph()
+                        with torch.cuda.graph(g, stream=side):
+                            for _ in range(reps):
+                                call()
+                    torch.cuda.synchronize()
+                    g.replay()
+                    torch.cuda.synchronize()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    g.replay()
+                    b.record()
+                    b.synchronize()
+                    us = 1e3 * a.elapsed_time(b) / reps
+                    row[method + "_us"] = us
+                    row[method + "_gbs"] = (2 * n * n + k * k) * esz / (us * 1e-6) / 1e9
+                    if method == "direct":
+                        row["direct_frac_of_fma_peak"] = n * n * k * k / (us * 1e-6) / fma_peak
+                except jt.JtError as e:
+                    row[method + "_us"] = None
+                    row[method + "_error"] = str(e)
+            rows.append(row)
+    print(json.dumps({"metric": "psf_convolve_us", "unit": "us per call (CUDA-graph replay of %d calls)" % reps,
+                      "n_gpus": 1, "data": "synthetic", "rows": rows}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -438,11 +501,14 @@ def main():
     ap.add_argument("--cpu-evals", type=float, default=1.5e9, help="oracle sample size for cpu_baseline")
     ap.add_argument("--ref-evals", type=float, default=2.0e8, help="oracle sample size per --impl reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--conv-sweep", action="store_true", help="time jt_psf_convolve alone at the paper's shapes")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank, world, local_rank = dist_init(args.gpus)
     try:
-        if args.impl == "reference":
+        if args.conv_sweep:
+            run_conv_sweep(args, rank)
+        elif args.impl == "reference":
             run_reference(args, rank, world)
         else:
             run_ours(args, rank, world, local_rank)

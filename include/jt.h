@@ -109,7 +109,7 @@ JT_API jt_status jt_source_brightness(jt_dtype dtype, int64_t n, const void *bet
  * (zero padding, 'same' size, true convolution -- kernel flipped relative to correlation).
  * image: device [ny][nx] (in).  kernel: device [ky][kx], ky and kx odd (in); used as given, never
  * renormalised.  out: device [ny][nx].  method: DIRECT = shared-memory tiled sum; FFT = zero-pad
- * to a power of two P >= n+K-1, hand-written shared-memory FFTs; AUTO picks by kernel size.
+ * to a power of two P >= n+K-1, hand-written shared-memory FFTs; AUTO picks the path a time model calibrated on B200 expects to be faster.
  * workspace: device scratch >= jt_psf_convolve_workspace_bytes(...) for the same arguments. */
 JT_API size_t    jt_psf_convolve_workspace_bytes(jt_dtype dtype, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
                                           jt_conv_method method);

@@ -37,13 +37,12 @@ static bool valid_lens(const jt_lens* l) {
 }
 static bool valid_kernel_size(int ky, int kx) { return ky >= 1 && kx >= 1 && (ky & 1) && (kx & 1); }
 
-// AUTO: direct while the tap count is small or the halo tile fits; FFT for large kernels
-// (crossover measured on B200).
+// AUTO: whichever of the two supported paths the calibrated time models expect to be faster.
 jt_conv_method resolve_conv_method(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method m) {
     if (m == JT_CONV_DIRECT || m == JT_CONV_FFT) return m;
     if (!conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_CONV_FFT;
     if (!conv_fft_supported(dtype, ny, nx, ky, kx)) return JT_CONV_DIRECT;
-    return ((int64_t)ky * kx > 41 * 41) ? JT_CONV_FFT : JT_CONV_DIRECT;
+    return conv_fft_estimate_us(dtype, ny, nx, ky, kx) < conv_direct_estimate_us(dtype, ny, nx, ky, kx) ? JT_CONV_FFT : JT_CONV_DIRECT;
 }
 
 static size_t conv_ws(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method method) {

@@ -92,6 +92,19 @@ bool conv_direct_supported(jt_dtype d, int ny, int nx, int ky, int kx) {
 
 size_t conv_direct_workspace_bytes(jt_dtype, int, int) { return 0; }
 
+// Time model behind JT_CONV_AUTO, calibrated on B200 with `bench.py --conv-sweep`: a warp spends
+// 4 OY (float, FFMA2) or 8 OY (double, DFMA) pipe cycles per kernel-column pair and kernel row, the warps of a
+// scheduler share the pipe, the measured pipe efficiency is one half, and CTAs run in waves of 148.
+double conv_direct_estimate_us(jt_dtype d, int ny, int nx, int ky, int kx) {
+    ConvCfg c;
+    if (!pick_cfg(d, ny, nx, ky, kx, &c)) return 1e30;
+    const int64_t tiles = (int64_t)((nx + kConvTW - 1) / kConvTW) * ((ny + c.NW * c.OY - 1) / (c.NW * c.OY));
+    const double waves = (double)((tiles + kNumSMs - 1) / kNumSMs);
+    const double per_warp = (double)((kx + 1) / 2) * c.kyp * (d == JT_F32 ? 4.0 : 8.0) * c.OY;
+    const double share = c.NW > 4 ? c.NW / 4.0 : 1.0;
+    return 3.0 + waves * per_warp * share / 0.5 / 1.9e3;
+}
+
 template <typename T, int OY>
 static jt_status run_cfg(const ConvCfg& c, int ny, int nx, const T* img, int ky, int kx, const T* ker, T* out, cudaStream_t st) {
     auto kern = k_conv_direct<T, OY>;

@@ -264,6 +264,13 @@ static FftPlan plan_fft(jt_dtype d, int ny, int nx, int ky, int kx) {
 
 bool conv_fft_supported(jt_dtype d, int ny, int nx, int ky, int kx) { return plan_fft(d, ny, nx, ky, kx).ok; }
 
+// Time model behind JT_CONV_AUTO (bench.py --conv-sweep on B200: P = 128: 20 us, 256: 29, 512: 44, 1024: 104, 2048: 408)
+double conv_fft_estimate_us(jt_dtype d, int ny, int nx, int ky, int kx) {
+    const FftPlan p = plan_fft(d, ny, nx, ky, kx);
+    if (!p.ok) return 1e30;
+    return 8.0 + 0.9 * (p.logPx + p.logPy) + 90.0 * ((double)p.Px * p.Py / 1048576.0);
+}
+
 size_t fft_conv_workspace_bytes(jt_dtype d, int ny, int nx, int ky, int kx) {
     const FftPlan p = plan_fft(d, ny, nx, ky, kx);
     return p.ok ? align_up(p.plane_bytes, 256) + 2 * kFftSumCtas * sizeof(double) : 0;
