@@ -26,10 +26,23 @@ __global__ void __launch_bounds__(256) k_conv_direct(int ny, int nx, const T* __
     const int i0 = blockIdx.x * kConvTW, j0 = blockIdx.y * TH;
     const int col0 = i0 - (kx - 1 - kx / 2), row0 = j0 - (ky - 1 - ky / 2);
 
-    for (int idx = tid; idx < ths * tws; idx += nthr) {
-        const int r = idx / tws, c = idx - r * tws;
-        const int gj = row0 + r, gi = col0 + c;
-        tile[idx] = (r < TH + ky - 1 && gj >= 0 && gj < ny && gi >= 0 && gi < nx) ? __ldg(&img[(size_t)gj * nx + gi]) : (T)0;
+    // fill with cp.async (LDGSTS): every thread queues all of its elements without waiting on any of them; elements
+    // outside the image (and the padded rows below TH + ky - 1) are zero-filled by a source size of 0
+    {
+        const unsigned tile_s = (unsigned)__cvta_generic_to_shared(tile);
+        for (int idx = tid; idx < ths * tws; idx += nthr) {
+            const int r = idx / tws, c = idx - r * tws;
+            const int gj = row0 + r, gi = col0 + c;
+            const bool ok = r < TH + ky - 1 && gj >= 0 && gj < ny && gi >= 0 && gi < nx;
+            const T* src = img + (ok ? (size_t)gj * nx + gi : 0);
+            const unsigned dst = tile_s + (unsigned)idx * (unsigned)sizeof(T);
+            const int nbytes = ok ? (int)sizeof(T) : 0;
+            if constexpr (sizeof(T) == 4)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(dst), "l"(src), "r"(nbytes) : "memory");
+            else
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(dst), "l"(src), "r"(nbytes) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
     }
 
     ConvAcc<T, OY> acc;
@@ -40,6 +53,7 @@ __global__ void __launch_bounds__(256) k_conv_direct(int ny, int nx, const T* __
         const int mb = min(band_pairs, npairs - m0);
         if (m0 > 0) __syncthreads();                  // every warp is done with the previous band's taps
         stage_taps<T>(Kc, K, ky, kx, kyp, m0, mb, tid, nthr);
+        if (m0 == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
         __syncthreads();                              // taps (and, first time, the tile) are in place
         acc.template sweep<true>(tp0 + 2 * m0, tws, Kc, kyp, mb);
     }

@@ -90,6 +90,24 @@ __global__ void __launch_bounds__(256) k_probe(int64_t iters, float seed, float*
 #pragma unroll
         for (int c = 0; c < 8; ++c) s ^= acc[c];
         if (s == 0x123456789abcdefull) sink[0] = 1.f;
+    } else if constexpr (KIND == JT_PROBE_DFMA_RF) {
+        // DFMA with the direct convolution's operand pattern: 8 accumulators, 4 taps, 8 tile values, all distinct doubles
+        double acc[8], t[4], w[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) { acc[c] = 0.0; w[c] = (double)a0 * (double)(c + 1); }
+#pragma unroll
+        for (int c = 0; c < 4; ++c) t[c] = 1e-3 * (double)(c + 1) * (double)seed;
+        for (int64_t i = 0; i < iters; ++i) {
+#pragma unroll
+            for (int u = 0; u < kProbeUnroll; ++u)
+#pragma unroll
+                for (int c = 0; c < kProbeChains; ++c)
+                    asm volatile("fma.rn.f64 %0, %1, %2, %0;" : "+d"(acc[c]) : "d"(t[u]), "d"(w[(c + u) % 8]));
+        }
+        double s = 0.0;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) s += acc[c];
+        if (s == 123.456) sink[0] = (float)s;
     } else {   // JT_PROBE_MUFU_RSQ
         float v[kProbeChains];
 #pragma unroll
@@ -119,6 +137,7 @@ extern "C" jt_status jt_probe_alu(int32_t kind, int32_t blocks, int64_t iters, v
         case JT_PROBE_FFMA2: k_probe<JT_PROBE_FFMA2><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_DFMA: k_probe<JT_PROBE_DFMA><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_FFMA2_RF: k_probe<JT_PROBE_FFMA2_RF><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
+        case JT_PROBE_DFMA_RF: k_probe<JT_PROBE_DFMA_RF><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_MUFU_RSQ: k_probe<JT_PROBE_MUFU_RSQ><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         default: return JT_ERR_UNSUPPORTED;
     }
