@@ -37,9 +37,10 @@ METRIC = "ray_deflector_evals_per_s"
 UNIT = "evals/s"
 SM_COUNT = 148
 # Algorithmic work per evaluation on the binding unit: counted in the SASS of the warp-uniform
-# far-field loop (loop head + far body) divided by its 8 rays.  f32: issue slots (the issue port and the FP32 pipe both
-# run 128 lanes/clk/SM, the port binds); f64: FP64-pipe instructions (64 lanes/clk/SM, the pipe binds).
-ALG_INSTR_PER_EVAL = {"f32": 34.25, "f64": 51.6}      # 274 / 8 issue slots; 413 / 8 FP64-pipe instructions
+# far-field loop (loop head + far body) divided by its 8 rays.  f32: FP32-pipe lane operations (an FFMA2 / FMUL2 / FADD2
+# counts as two; 237 per 8 rays; the loop needs only 21 issue slots per evaluation, so the 128-lane FP32 pipe binds);
+# f64: FP64-pipe instructions (405 per 8 rays; 64 lanes/clk/SM).
+ALG_INSTR_PER_EVAL = {"f32": 29.6, "f64": 50.6}
 ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
 
@@ -383,7 +384,7 @@ def run_ours(args, rank, world, local_rank):
         "bound": "alu", "kernel": "k_batch" if batch else "k_trace", "achieved": achieved, "peak": peak_tinstr,
         "unit": "Tlaneop/s", "frac": achieved / peak_tinstr, "traffic": None,
         "peak_kind": "derived: 148 SMs x %d lanes/clk (%s) x %.0f MHz (max clock, %s)" % (
-            lanes, "issue port = FP32 pipe" if w.dtype == "f32" else "FP64 pipe", peaks.get("sm_max_mhz", 1965.0),
+            lanes, "FP32 pipe" if w.dtype == "f32" else "FP64 pipe", peaks.get("sm_max_mhz", 1965.0),
             peak_kind),
         "alg_instr_per_eval": n_alg, "kernel_ms": trace_ms, "conv_ms": conv_ms,
         "kernel_share_of_step": trace_ms / (ms_total_local / args.steps),

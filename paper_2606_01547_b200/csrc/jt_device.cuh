@@ -75,7 +75,8 @@ template <typename T>
 struct alignas(sizeof(T) * 4) SubRec {
     T cx, cy, iRs2, thr;       // centre, 1/Rs^2, far-field threshold on X^2 (= max(10, 3t))
     T t, a_tm1, a_c1, a_pi;    // tau^2, amp (t-1), amp c1, amp pi
-    T a_m2, amp, tm1, c1;      // -2 amp, amplitude, tau^2 - 1, c1
+    T c_a, c_b, c_c, amp;      // amp (t-1) pi/2, amp (t+1), 2 amp; amplitude
+    T tm1, c1, pad0, pad1;     // tau^2 - 1, c1 (generic near-field forms)
 };
 
 template <typename T>
@@ -92,7 +93,10 @@ __device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, d
     r.a_tm1 = (T)(amp * (t - 1.0));
     r.a_c1 = (T)(amp * c1);
     r.a_pi = (T)(amp * JT_PI_D);
-    r.a_m2 = (T)(-2.0 * amp);
+    r.c_a = (T)(amp * (t - 1.0) * (JT_PI_D / 2));
+    r.c_b = (T)(amp * (t + 1.0));
+    r.c_c = (T)(2.0 * amp);
+    r.pad0 = (T)0; r.pad1 = (T)0;
     r.amp = (T)amp;
     r.tm1 = (T)(t - 1.0);
     r.c1 = (T)c1;
@@ -103,14 +107,17 @@ template <typename T>
 __device__ __forceinline__ SubRec<T> null_rec() {
     SubRec<T> r;
     r.cx = (T)1e6; r.cy = (T)1e6; r.iRs2 = (T)1; r.thr = (T)10; r.t = (T)1;
-    r.a_tm1 = (T)0; r.a_c1 = (T)0; r.a_pi = (T)0; r.a_m2 = (T)0; r.amp = (T)0; r.tm1 = (T)0; r.c1 = (T)0;
+    r.a_tm1 = (T)0; r.a_c1 = (T)0; r.a_pi = (T)0; r.c_a = (T)0; r.c_b = (T)0; r.c_c = (T)0; r.amp = (T)0;
+    r.tm1 = (T)0; r.c1 = (T)0; r.pad0 = (T)0; r.pad1 = (T)0;
     return r;
 }
 
 // Far field, X^2 >= max(10, 3t): no logarithm, no cancellation growing with X.
 //   w = 1/sqrt(X^2-1), z = w^2 <= 1/9, y = t/(X^2+t) <= 1/4,  P = atan(w)/w, Q = atanh(sqrt y)/sqrt y
 //   F = (pi/2 - w P) w;   S c2 L = -(t-1) Q;   2 X^2 F - pi S = pi (w X^2 - S) - 2 (1+z) P      (w + u = w X^2)
-//   amp brace = a_tm1 (F - Q) + a_c1 + a_pi (w X^2 - S) + a_m2 (1+z) P
+//   amp brace = a_tm1 (F - Q) + a_c1 + a_pi (w X^2 - S) - 2 amp (1+z) P
+//             = (c_a w + a_c1) - P (c_b z + c_c) - a_tm1 Q + a_pi (w X^2 - S)      (F and the (1+z) P term merged:
+//               c_a = amp (t-1) pi/2, c_b = amp (t-1) + 2 amp, c_c = 2 amp; two instructions fewer)
 // Returns f with alpha = f * (dx, dy).
 template <typename T>
 __device__ __forceinline__ T tnfw_far(T R2, const SubRec<T>& s) {
@@ -123,11 +130,77 @@ __device__ __forceinline__ T tnfw_far(T R2, const SubRec<T>& s) {
     const T S = S2 * rS, z = w * w, y = (s.t * rS) * rS;
     const T P = atan_far(z);
     const T Q = atanh_q(y);
-    const T F = fma(-w, P, (T)(JT_PI_D / 2)) * w;
-    T b = fma(s.a_tm1, F - Q, s.a_c1);
+    T b = fma(-P, fma(s.c_b, z, s.c_c), fma(s.c_a, w, s.a_c1));
+    b = fma(-s.a_tm1, Q, b);
     b = fma(s.a_pi, fma(w, X2, -S), b);
-    b = fma(s.a_m2, fma(z, P, P), b);
     return b * iR2;
+}
+
+// Two rays at once in float: the two Horner chains (10 of the 30 FP32 instructions of an evaluation) run as sm_100
+// packed FMAs (fma.rn.f32x2 -> FFMA2, the coefficient as a broadcast operand), which halves their issue slots -- the
+// float far loop is bound by the issue port, not by the FP32 pipe.
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+    unsigned long long d;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(d) : "f"(lo), "f"(hi));
+    return d;
+}
+__device__ __forceinline__ void unpack2(unsigned long long v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long fma2c(unsigned long long p, unsigned long long z, float c) {
+    unsigned long long d;
+    asm("{\n\t.reg .b64 cc;\n\tmov.b64 cc, {%3, %3};\n\tfma.rn.f32x2 %0, %1, %2, cc;\n\t}" : "=l"(d) : "l"(p), "l"(z), "f"(c));
+    return d;
+}
+template <int N>
+__device__ __forceinline__ unsigned long long horner2(const float (&c)[N], unsigned long long z) {
+    unsigned long long p = pack2(c[0], c[0]);
+#pragma unroll
+    for (int i = 1; i < N; ++i) p = fma2c(p, z, c[i]);
+    return p;
+}
+typedef unsigned long long f32x2;                         // two floats in one 64-bit register (lo, hi)
+__device__ __forceinline__ f32x2 bc2(float x) { return pack2(x, x); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+// The whole far-field form on two rays at once (same algebra as tnfw_far<float>; MUFU on the halves).
+__device__ __forceinline__ void tnfw_far_pair(float R2a, float R2b, const SubRec<float>& s, float& fa, float& fb) {
+    const f32x2 R2 = pack2(R2a, R2b);
+    const f32x2 X2 = mul2(R2, bc2(s.iRs2));
+    const f32x2 u2 = add2(X2, bc2(-1.f));
+    const f32x2 S2 = add2(X2, bc2(s.t));
+    float u2a, u2b, S2a, S2b;
+    unpack2(u2, u2a, u2b);
+    unpack2(S2, S2a, S2b);
+    const f32x2 w = pack2(fast_rsqrt(u2a), fast_rsqrt(u2b));
+    const f32x2 rS = pack2(fast_rsqrt(S2a), fast_rsqrt(S2b));
+    const f32x2 iR2 = pack2(approx_rcp(R2a), approx_rcp(R2b));
+    const f32x2 z = mul2(w, w);
+    const f32x2 y = mul2(mul2(bc2(s.t), rS), rS);
+    const float cp[] = {JT_ATAN_FAR_F32_COEFS};
+    const float cq[] = {JT_ATANH_Q_F32_COEFS};
+    const f32x2 P = horner2(cp, z);
+    const f32x2 Q = horner2(cq, y);
+    // amp brace = (c_a w + a_c1) - P (c_b z + c_c) - a_tm1 Q + a_pi (w X2 - S2 rS)
+    const f32x2 g = fma2(bc2(-s.c_b), z, bc2(-s.c_c));                 // -(c_b z + c_c)
+    f32x2 b = fma2(P, g, fma2(bc2(s.c_a), w, bc2(s.a_c1)));
+    b = fma2(bc2(-s.a_tm1), Q, b);
+    b = fma2(bc2(s.a_pi), mul2(w, X2), b);
+    b = fma2(bc2(-s.a_pi), mul2(S2, rS), b);
+    unpack2(mul2(b, iR2), fa, fb);
 }
 
 // ln x for normal positive x.  float: one MUFU.LG2.  double: x = 2^e m, m in (sqrt(1/2), sqrt 2],
@@ -169,12 +242,11 @@ __device__ __forceinline__ T tnfw_midfast(T R2, const SubRec<T>& s) {
     const T iX2 = approx_rcp(X2);
     const T S = S2 * rS, tau = s.t * rt, z = w * w;
     const T P = atan_full(z);
-    const T F = fma(-w, P, (T)(JT_PI_D / 2)) * w;
     const T d = S + tau;
     const T Q = (S * rt) * ((T)0.5 * ln_pos((d * d) * iX2));
-    T b = fma(s.a_tm1, F - Q, s.a_c1);
+    T b = fma(-P, fma(s.c_b, z, s.c_c), fma(s.c_a, w, s.a_c1));
+    b = fma(-s.a_tm1, Q, b);
     b = fma(s.a_pi, fma(w, X2, -S), b);
-    b = fma(s.a_m2, fma(z, P, P), b);
     return b * iR2;
 }
 

@@ -197,11 +197,23 @@ __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs,
         }
         const T X2min = R2min * s.iRs2;
         if (__all_sync(0xffffffffu, X2min >= s.thr)) {
+            if constexpr (sizeof(T) == 4 && R % 2 == 0) {
 #pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const T f = tnfw_far<T>(R2[r], s);
-                ax[r] = fma(f, dx[r], ax[r]);
-                ay[r] = fma(f, dy[r], ay[r]);
+                for (int r = 0; r < R; r += 2) {
+                    float f0, f1;
+                    tnfw_far_pair(R2[r], R2[r + 1], s, f0, f1);
+                    ax[r] = fma(f0, dx[r], ax[r]);
+                    ay[r] = fma(f0, dy[r], ay[r]);
+                    ax[r + 1] = fma(f1, dx[r + 1], ax[r + 1]);
+                    ay[r + 1] = fma(f1, dy[r + 1], ay[r + 1]);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const T f = tnfw_far<T>(R2[r], s);
+                    ax[r] = fma(f, dx[r], ax[r]);
+                    ay[r] = fma(f, dy[r], ay[r]);
+                }
             }
         } else if (__all_sync(0xffffffffu, X2min >= (T)kMidX2)) {
 #pragma unroll
