@@ -160,7 +160,8 @@ JT_API jt_status jt_profile_read(float *trace_ms, float *conv_ms);
  * receives the number of thread-level instructions of that kind the launch executes (an FFMA2 counts once but
  * performs two FMAs).  sink: device scratch of >= 4 bytes.  Time it with events on `stream`. */
 typedef enum { JT_PROBE_FFMA = 0, JT_PROBE_FFMA2 = 1, JT_PROBE_DFMA = 2, JT_PROBE_MUFU_RSQ = 3,
-               JT_PROBE_FFMA2_RF = 4, JT_PROBE_DFMA_RF = 5 /* FFMA2 / DFMA with the direct convolution's operand pattern */ } jt_probe_kind;
+               JT_PROBE_FFMA2_RF = 4, JT_PROBE_DFMA_RF = 5, /* FFMA2 / DFMA with the direct convolution's operand pattern */
+               JT_PROBE_FFMA2_LDS = 6 /* the same with one tap and one window shared-memory load per 8 FFMA2 */ } jt_probe_kind;
 JT_API jt_status jt_probe_alu(int32_t kind, int32_t blocks, int64_t iters, void *sink, int64_t *lane_ops, void *stream);
 
 /* Number of CUDA kernels this library has launched from the calling host thread since it was loaded

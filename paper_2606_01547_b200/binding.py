@@ -127,7 +127,7 @@ def profile_read():
     return a.value, b.value
 
 
-PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "ffma2_rf": 4, "dfma_rf": 5}
+PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "ffma2_rf": 4, "dfma_rf": 5, "ffma2_lds": 6}
 
 
 def probe_alu(kind, blocks=148 * 8, iters=4096, repeats=3):

@@ -108,6 +108,46 @@ __global__ void __launch_bounds__(256) k_probe(int64_t iters, float seed, float*
 #pragma unroll
         for (int c = 0; c < 8; ++c) s += acc[c];
         if (s == 123.456) sink[0] = (float)s;
+    } else if constexpr (KIND == JT_PROBE_FFMA2_LDS) {
+        // the direct convolution's inner loop with its shared-memory traffic: per kernel row one broadcast 128-bit tap
+        // load and one 64-bit window load feed 16 FFMA2 (8 accumulators x two products), window rotating in registers
+        __shared__ __align__(16) float smem[8 * 16 * 4 + 72 * 64];
+        for (int i = threadIdx.x; i < 8 * 16 * 4 + 72 * 64; i += 256) smem[i] = 1e-3f * (float)(i % 17) * seed;
+        __syncthreads();
+        const float* taps = smem;
+        const float* tile = smem + 8 * 16 * 4 + 2 * (threadIdx.x & 31);
+        unsigned long long acc[8];
+        float2 win[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) { acc[c] = 0ull; win[c] = make_float2(a0, a0 * (float)c); }
+        for (int64_t i = 0; i < iters; ++i) {
+            const float* kp = taps + (i & 7) * 64;
+            const float* wp = tile + (i & 7) * 8 * 64;
+#pragma unroll
+            for (int u = 0; u < kProbeUnroll; ++u) {        // 4 kernel rows x 8 accumulators = 32 FFMA2 ... x2 products below
+                const ulonglong2 t = *reinterpret_cast<const ulonglong2*>(kp + 4 * u);
+                win[(u + 7) % 8] = *reinterpret_cast<const float2*>(wp + u * 64);
+                if (u & 1) {                                 // count stays 8 per (u): alternate x and y products
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        unsigned long long wb;
+                        asm volatile("mov.b64 %0, {%1, %1};" : "=l"(wb) : "f"(win[(c + u) % 8].y));
+                        asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[c]) : "l"(t.y), "l"(wb));
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 8; ++c) {
+                        unsigned long long wb;
+                        asm volatile("mov.b64 %0, {%1, %1};" : "=l"(wb) : "f"(win[(c + u) % 8].x));
+                        asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[c]) : "l"(t.x), "l"(wb));
+                    }
+                }
+            }
+        }
+        unsigned long long s2 = 0;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) s2 ^= acc[c];
+        if (s2 == 0x123456789abcdefull) sink[0] = 1.f;
     } else {   // JT_PROBE_MUFU_RSQ
         float v[kProbeChains];
 #pragma unroll
@@ -138,6 +178,7 @@ extern "C" jt_status jt_probe_alu(int32_t kind, int32_t blocks, int64_t iters, v
         case JT_PROBE_DFMA: k_probe<JT_PROBE_DFMA><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_FFMA2_RF: k_probe<JT_PROBE_FFMA2_RF><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_DFMA_RF: k_probe<JT_PROBE_DFMA_RF><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
+        case JT_PROBE_FFMA2_LDS: k_probe<JT_PROBE_FFMA2_LDS><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         case JT_PROBE_MUFU_RSQ: k_probe<JT_PROBE_MUFU_RSQ><<<blocks, 256, 0, st>>>(iters, 1.0f, (float*)sink); break;
         default: return JT_ERR_UNSUPPORTED;
     }

@@ -261,6 +261,38 @@ def test_no_lens_constant_source_invariant(jt):
     assert np.allclose(img, 2.0 * np.exp(b) * 0.05 ** 2, rtol=1e-5)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_image_edge_cases(jt, orc, dtype):
+    """Degenerate shapes of jt_simulate_image: no sources (image = 0), 16 sources (JT_MAX_SOURCES), a 1 x 1 grid,
+    s = 16 on a 3 x 2 grid, a non-square PSF through both convolution paths, one subhalo list entry."""
+    import torch
+    rng = np.random.default_rng(31)
+    w = workloads.config_c1(nx=21, supersample=2, K=9, dtype=dtype)
+    # no sources
+    g = jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample)
+    img = jt.simulate_image(g, w.sie, w.shear, to_dev(w.tnfw, dtype), np.zeros((0, 7)), to_dev(w.psf, dtype), dtype=dtype)
+    assert float(img.abs().max()) == 0.0
+    # 16 sources
+    src = np.tile(w.sources[:1], (16, 1))
+    src[:, 0] = rng.uniform(1, 3, 16)
+    src[:, 5:7] = rng.uniform(-0.3, 0.3, (16, 2))
+    w16 = workloads.config_c1(nx=21, supersample=2, K=9, dtype=dtype)
+    w16.sources = _f32r(src) if dtype == "f32" else src
+    _check_image(jt, orc, w16, method="direct")
+    # 1 x 1 grid and s = 16
+    for nx, ny, s in ((1, 1, 1), (3, 2, 16)):
+        we = workloads.config_c1(nx=nx, supersample=s, K=3, dtype=dtype)
+        we.ny = ny
+        _check_image(jt, orc, we, method="direct")
+    # non-square PSF, both paths
+    wn = workloads.config_c1(nx=40, supersample=1, K=9, dtype=dtype)
+    psf = rng.uniform(0, 1, (5, 13))
+    wn.psf = _f32r(psf / psf.sum()) if dtype == "f32" else psf / psf.sum()
+    _check_image(jt, orc, wn, method="direct")
+    _check_image(jt, orc, wn, method="fft")
+    _check_image(jt, orc, wn, method="auto")
+
+
 def test_c2_full_size_sampled_rows(jt, orc):
     """Full-size C2 (200x200, s=2, 10,000 subhalos) in the launch configuration bench.py times:
     three pixel rows of the pre-PSF image against the oracle, f64 and f32."""
