@@ -153,6 +153,11 @@ JT_API jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid *gri
  * destroys them. */
 JT_API jt_status jt_profile_enable(int on);
 JT_API jt_status jt_profile_read(float *trace_ms, float *conv_ms);
+/* After jt_profile_read semantics: copies the four counters of the LAST profiled jt_simulate_image call to host
+ * memory counts[4]: (warp, subhalo-record) pairs evaluated by the far-far series, the far form, the mid form and the
+ * per-ray cold path.  The counters live in the call's workspace, which must still be allocated;
+ * the call synchronises on the profiling events. */
+JT_API jt_status jt_profile_tiers(uint64_t *counts);
 
 /* Measurement aid: ALU peak microbenchmark (bench.py reports the measured rates beside the derived peaks of
  * DESIGN.md section 6; MEASURED_PEAKS.json covers only HBM and tensor cores).  Launches `blocks` CTAs of 256

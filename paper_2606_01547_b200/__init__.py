@@ -13,6 +13,7 @@ from .binding import (  # noqa: F401
     probe_alu,
     profile_enable,
     profile_read,
+    profile_tiers,
     psf_convolve,
     psf_convolve_workspace_bytes,
     ray_shoot,

@@ -101,6 +101,7 @@ def lib():
         L.jt_kernel_launches.restype = ctypes.c_uint64
         L.jt_profile_enable.argtypes = [ctypes.c_int]
         L.jt_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
+        L.jt_profile_tiers.argtypes = [ctypes.POINTER(ctypes.c_uint64)]
         L.jt_probe_alu.argtypes = [i32, i32, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
     return _lib
@@ -125,6 +126,13 @@ def profile_read():
     a, b = ctypes.c_float(), ctypes.c_float()
     _check(lib().jt_profile_read(ctypes.byref(a), ctypes.byref(b)), "jt_profile_read")
     return a.value, b.value
+
+
+def profile_tiers():
+    """jt_profile_tiers: (far-far, far, mid, cold) counts of (warp, subhalo record) pairs of the last profiled call."""
+    c = (ctypes.c_uint64 * 4)()
+    _check(lib().jt_profile_tiers(c), "jt_profile_tiers")
+    return tuple(int(x) for x in c)
 
 
 PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "ffma2_rf": 4, "dfma_rf": 5, "ffma2_lds": 6}

@@ -10,7 +10,11 @@ static thread_local uint64_t g_launches = 0;
 void count_launch() { ++g_launches; }
 
 // ---- profiling events (jt_profile_enable / jt_profile_read) ----
-struct ProfileState { bool on = false, recorded = false, had_conv = false; cudaEvent_t ev[3] = {nullptr, nullptr, nullptr}; };
+struct ProfileState {
+    bool on = false, recorded = false, had_conv = false;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    void* tiers = nullptr;             // device: four uint64 counters in the last profiled call's workspace
+};
 static thread_local ProfileState g_prof;
 
 static jt_status check_device() {
@@ -175,13 +179,15 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
     const bool prof = g_prof.on;
     if (prof) { g_prof.recorded = false; JT_CUDA_TRY(cudaEventRecord(g_prof.ev[0], st)); }
     if (!conv) {
-        s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, out, st);
+        if (prof) g_prof.tiers = trace_tier_counters(plan, trace_ws);
+        s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, out, prof, st);
         if (s == JT_OK && prof) { JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st)); g_prof.had_conv = false; g_prof.recorded = true; }
         return s;
     }
     void* pre = ws + align_up(plan.total_bytes, 256);
     void* conv_ws_ptr = (char*)pre + align_up((size_t)grid->nx * grid->ny * dtype_size(dtype), 256);
-    s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, pre, st);
+    if (prof) g_prof.tiers = trace_tier_counters(plan, trace_ws);
+    s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, pre, prof, st);
     if (s != JT_OK) return s;
     if (prof) JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st));
     s = conv_dispatch(dtype, grid->ny, grid->nx, pre, ky, kx, kernel, method, conv_ws_ptr, out, st);
@@ -199,6 +205,7 @@ jt_status jt_profile_enable(int on) {
         for (int i = 0; i < 3; ++i) { cudaEventDestroy(g_prof.ev[i]); g_prof.ev[i] = nullptr; }
         g_prof.on = false;
         g_prof.recorded = false;
+        g_prof.tiers = nullptr;
     }
     return JT_OK;
 }
@@ -209,6 +216,13 @@ jt_status jt_profile_read(float* trace_ms, float* conv_ms) {
     JT_CUDA_TRY(cudaEventElapsedTime(trace_ms, g_prof.ev[0], g_prof.ev[1]));
     *conv_ms = 0.f;
     if (g_prof.had_conv) JT_CUDA_TRY(cudaEventElapsedTime(conv_ms, g_prof.ev[1], g_prof.ev[2]));
+    return JT_OK;
+}
+
+jt_status jt_profile_tiers(uint64_t* counts) {
+    if (!g_prof.on || !g_prof.recorded || !g_prof.tiers || !counts) return JT_ERR_INVALID_VALUE;
+    JT_CUDA_TRY(cudaEventSynchronize(g_prof.ev[g_prof.had_conv ? 2 : 1]));
+    JT_CUDA_TRY(cudaMemcpy(counts, g_prof.tiers, 4 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
     return JT_OK;
 }
 

@@ -13,7 +13,8 @@
 
 namespace jt {
 
-constexpr int kBatchRecCap = 512;            // subhalo records resident per staging round
+constexpr int kBatchRecCap = 512;            // subhalo records resident per staging round (float; 256 in double)
+template <typename T> struct BatchRecCap { static constexpr int value = sizeof(T) == 8 ? 256 : 512; };
 constexpr int kBatchTW = 64;                 // convolution pass: 64 columns (32 lanes x 2) x 8 warps * OY rows
 template <typename T> struct BatchOY { static constexpr int value = sizeof(T) == 4 ? 8 : 4; };   // as in jt_conv.cu
 
@@ -91,9 +92,10 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
         for (int r = 0; r < R; ++r) { xs[r] = x; ys[r] = (T)g.yd(r); pin(ys[r]); }
         DAcc<T, R> acc;
         acc.init(dacc + tid);
+        TierCount tiers = {{0u, 0u, 0u, 0u}};
 
         if (resident) {
-            subhalo_tile<T, R, true>(recs, a.M, 0, raw, g, xs, ys, acc, s_queue[warp]);
+            subhalo_tile<T, R, true>(recs, a.M, 0, raw, g, xs, ys, acc, s_queue[warp], tiers);
         } else {
             for (int base = 0; base < a.M; base += a.rec_cap) {
                 const int count = min(a.rec_cap, a.M - base);
@@ -103,7 +105,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
                                           (double)raw.p[2][base + k], (double)raw.p[3][base + k],
                                           (double)raw.p[4][base + k]);
                 __syncthreads();
-                subhalo_tile<T, R, true>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp]);
+                subhalo_tile<T, R, true>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp], tiers);
             }
         }
         double axd[R], ayd[R];
@@ -181,7 +183,7 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.pw = conv ? (g->nx + kBatchTW - 1) / kBatchTW * kBatchTW + a.kx - 1 : 0;        // even: pair loads stay aligned
     a.ph = conv ? (g->ny + TH - 1) / TH * TH + a.kyp - 1 : 0;
     a.img_elems = (a.pw * a.ph + 3) / 4 * 4;
-    a.rec_cap = a.M < kBatchRecCap ? (a.M > 0 ? a.M : 1) : kBatchRecCap;
+    a.rec_cap = a.M < BatchRecCap<T>::value ? (a.M > 0 ? a.M : 1) : BatchRecCap<T>::value;
     a.sie = (const T*)p->sie; a.shear = (const T*)p->shear; a.tnfw = (const T*)p->tnfw;
     a.sersic = (const T*)p->sersic; a.psf = (const T*)p->psf;
     a.out = (T*)out;

@@ -71,23 +71,57 @@ __device__ __forceinline__ double t_log(double x) { return log(x); }
 // ------------------------------------------------------------------------------------------------
 // The hot loops read the first nine fields (amplitude folded into the brace coefficients: one multiply per evaluation
 // less); the generic near-field forms read amp, tm1, c1.
+// Far-far field: for X >= 9 max(1, tau) (double; 8 max(1, tau) in float) the brace is summed from its expansion in
+// v = 1/X, derived with sympy from the closed form (every coefficient carries the factor (t+1)^2; the v^1 term vanishes):
+//   brace = b0 + b2 v^2 + b3 v^3 + ... ,   b0 = (t-1) ln tau - t + pi tau - 1 (the total-mass limit),
+//   b2 = -(t+1)^2/3, b3 = pi (t+1)^2/8, b4 = 2 (t+1)^2 (t-3)/15, b5 = -pi (t+1)^2 (t-2)/16, ...
+// Truncated after v^13 (double) / v^8 (float) the relative error is <= 1e-13 / 2e-8 beyond those radii for
+// tau = 0.3 ... 20 (checked against the closed form at 50 digits).  alpha = f (dx, dy), f = v^2 (a0 + v^2 (a2 + a3 v +
+// ...)), a_k = amp b_k / Rs^2: one MUFU and K + 1 multiply-adds instead of three MUFU and two polynomials.
+template <typename T> struct FarFar;
+template <> struct FarFar<double> { static constexpr int K = 13; static constexpr double kRadius = 9.0; };
+template <> struct FarFar<float> { static constexpr int K = 8; static constexpr double kRadius = 8.0; };
+
 template <typename T>
 struct alignas(sizeof(T) * 4) SubRec {
     T cx, cy, iRs2, thr;       // centre, 1/Rs^2, far-field threshold on X^2 (= max(10, 3t))
     T t, a_tm1, a_c1, a_pi;    // tau^2, amp (t-1), amp c1, amp pi
     T c_a, c_b, c_c, amp;      // amp (t-1) pi/2, amp (t+1), 2 amp; amplitude
-    T tm1, c1, pad0, pad1;     // tau^2 - 1, c1 (generic near-field forms)
+    T tm1, c1, thr2, a0;       // tau^2 - 1, c1 (generic near-field forms); far-far threshold on X^2; a_0
+    T ak[(FarFar<T>::K - 1 + 3) / 4 * 4];      // a_2 ... a_K, zero-padded to a multiple of 4
 };
+
+// b_k / (t+1)^2 for k = 2 ... 14 as polynomials in t (sympy series of the closed form)
+__host__ __device__ inline double farfar_coef(int k, double t) {
+    const double pi = JT_PI_D;
+    switch (k) {
+        case 2: return -1.0 / 3.0;
+        case 3: return pi / 8.0;
+        case 4: return 2.0 / 15.0 * (t - 3.0);
+        case 5: return -pi / 16.0 * (t - 2.0);
+        case 6: return -8.0 / 105.0 * ((t - 3.0) * t + 5.0);
+        case 7: return 5.0 * pi / 128.0 * ((t - 2.0) * t + 3.0);
+        case 8: return 16.0 / 315.0 * (((t - 3.0) * t + 5.0) * t - 7.0);
+        case 9: return -7.0 * pi / 256.0 * (((t - 2.0) * t + 3.0) * t - 4.0);
+        case 10: return -128.0 / 3465.0 * ((((t - 3.0) * t + 5.0) * t - 7.0) * t + 9.0);
+        case 11: return 21.0 * pi / 1024.0 * ((((t - 2.0) * t + 3.0) * t - 4.0) * t + 5.0);
+        case 12: return 256.0 / 9009.0 * (((((t - 3.0) * t + 5.0) * t - 7.0) * t + 9.0) * t - 11.0);
+        case 13: return -33.0 * pi / 2048.0 * (((((t - 2.0) * t + 3.0) * t - 4.0) * t + 5.0) * t - 6.0);
+        default: return 0.0;
+    }
+}
 
 template <typename T>
 __device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, double aRs, double rt) {
     const double tau = rt / Rs, t = tau * tau;
-    const double c1 = tau * JT_PI_D + (t - 1.0) * log(tau);
+    const double lt = log(tau);
+    const double c1 = tau * JT_PI_D + (t - 1.0) * lt;
     const double amp = aRs / (1.0 - JT_LN2_D) * Rs * t / ((t + 1.0) * (t + 1.0));
+    const double iRs2 = 1.0 / (Rs * Rs);
     SubRec<T> r;
     r.cx = (T)cx;
     r.cy = (T)cy;
-    r.iRs2 = (T)(1.0 / (Rs * Rs));
+    r.iRs2 = (T)iRs2;
     r.thr = (T)fmax(10.0, 3.0 * t);
     r.t = (T)t;
     r.a_tm1 = (T)(amp * (t - 1.0));
@@ -96,10 +130,18 @@ __device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, d
     r.c_a = (T)(amp * (t - 1.0) * (JT_PI_D / 2));
     r.c_b = (T)(amp * (t + 1.0));
     r.c_c = (T)(2.0 * amp);
-    r.pad0 = (T)0; r.pad1 = (T)0;
     r.amp = (T)amp;
     r.tm1 = (T)(t - 1.0);
     r.c1 = (T)c1;
+    const double rad = FarFar<T>::kRadius * fmax(1.0, tau);
+    r.thr2 = (T)(rad * rad);
+    const double sc = amp * iRs2;
+    r.a0 = (T)(sc * ((t - 1.0) * lt - t + JT_PI_D * tau - 1.0));
+    const double f = sc * (t + 1.0) * (t + 1.0);
+#pragma unroll
+    for (int k = 2; k <= FarFar<T>::K; ++k) r.ak[k - 2] = (T)(f * farfar_coef(k, t));
+#pragma unroll
+    for (int k = FarFar<T>::K - 1; k < (int)(sizeof(r.ak) / sizeof(T)); ++k) r.ak[k] = (T)0;
     return r;
 }
 // padding record: contributes exactly 0 and always takes the far path
@@ -108,8 +150,21 @@ __device__ __forceinline__ SubRec<T> null_rec() {
     SubRec<T> r;
     r.cx = (T)1e6; r.cy = (T)1e6; r.iRs2 = (T)1; r.thr = (T)10; r.t = (T)1;
     r.a_tm1 = (T)0; r.a_c1 = (T)0; r.a_pi = (T)0; r.c_a = (T)0; r.c_b = (T)0; r.c_c = (T)0; r.amp = (T)0;
-    r.tm1 = (T)0; r.c1 = (T)0; r.pad0 = (T)0; r.pad1 = (T)0;
+    r.tm1 = (T)0; r.c1 = (T)0; r.thr2 = (T)81; r.a0 = (T)0;
+#pragma unroll
+    for (int k = 0; k < (int)(sizeof(r.ak) / sizeof(T)); ++k) r.ak[k] = (T)0;
     return r;
+}
+
+// Far-far field (see FarFar above).  Returns f with alpha = f * (dx, dy).
+template <typename T>
+__device__ __forceinline__ T tnfw_farfar(T R2, const SubRec<T>& s) {
+    const T v = fast_rsqrt(R2 * s.iRs2);
+    const T v2 = v * v;
+    T p = s.ak[FarFar<T>::K - 2];
+#pragma unroll
+    for (int k = FarFar<T>::K - 3; k >= 0; --k) p = fma(p, v, s.ak[k]);
+    return v2 * fma(p, v2, s.a0);
 }
 
 // Far field, X^2 >= max(10, 3t): no logarithm, no cancellation growing with X.
@@ -176,6 +231,19 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
+// far-far field on two rays at once (float)
+__device__ __forceinline__ void tnfw_farfar_pair(float R2a, float R2b, const SubRec<float>& s, float& fa, float& fb) {
+    const f32x2 X2 = mul2(pack2(R2a, R2b), bc2(s.iRs2));
+    float xa, xb;
+    unpack2(X2, xa, xb);
+    const f32x2 v = pack2(fast_rsqrt(xa), fast_rsqrt(xb));
+    const f32x2 v2 = mul2(v, v);
+    f32x2 p = bc2(s.ak[FarFar<float>::K - 2]);
+#pragma unroll
+    for (int k = FarFar<float>::K - 3; k >= 0; --k) p = fma2(p, v, bc2(s.ak[k]));
+    unpack2(mul2(v2, fma2(p, v2, bc2(s.a0))), fa, fb);
+}
+
 // The whole far-field form on two rays at once (same algebra as tnfw_far<float>; MUFU on the halves).
 __device__ __forceinline__ void tnfw_far_pair(float R2a, float R2b, const SubRec<float>& s, float& fa, float& fb) {
     const f32x2 R2 = pack2(R2a, R2b);

@@ -10,7 +10,7 @@ namespace jt {
 
 constexpr int kNumSMs = 148;            // B200
 constexpr int kTraceThreads = 256;      // 8 warps per CTA in the ray-tracing kernels
-constexpr int kSubTile = 256;           // subhalo records staged per shared-memory tile
+template <typename T> struct SubTile { static constexpr int value = sizeof(T) == 8 ? 128 : 256; };   // records staged per shared-memory tile (224 B / 96 B each)
 
 // thread-local last CUDA error (jt_last_cuda_error)
 void set_last_cuda_error(int e);
@@ -45,13 +45,15 @@ struct TracePlan {
     int64_t chunk_len;     // subhalos per chunk (multiple of kSubTile unless n_chunks == 1)
     size_t partial_bytes;  // n_chunks > 1: double2 per (chunk, ray slot)
     size_t counter_bytes;  // one uint32 per tile
+    size_t tier_bytes;     // grid mode: four uint64 tier counters (jt_profile_tiers), always reserved
     size_t total_bytes;
 };
 TracePlan plan_trace_grid(jt_dtype dtype, const jt_grid* g, int64_t n_tnfw);
 TracePlan plan_trace_rays(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw);
 
 jt_status launch_trace_grid(jt_dtype dtype, const jt_grid* g, const jt_lens* lens, const SrcSet& src,
-                            const TracePlan& plan, void* workspace, void* pre_psf, cudaStream_t st);
+                            const TracePlan& plan, void* workspace, void* pre_psf, bool count_tiers, cudaStream_t st);
+void*     trace_tier_counters(const TracePlan& plan, void* workspace);
 jt_status launch_trace_rays(jt_dtype dtype, int64_t n, const void* tx, const void* ty, const jt_lens* lens,
                             const TracePlan& plan, void* workspace, void* bx, void* by, cudaStream_t st);
 jt_status launch_source_brightness(jt_dtype dtype, int64_t n, const void* bx, const void* by, const SrcSet& src,

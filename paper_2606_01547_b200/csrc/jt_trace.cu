@@ -58,7 +58,7 @@ static void plan_chunks(TracePlan* p, int64_t M, int R, bool f64) {
     if (p->n_chunks < 1) p->n_chunks = 1;
     p->partial_bytes = p->n_chunks > 1 ? (size_t)p->n_chunks * p->n_tiles * R * kTraceThreads * sizeof(double2) : 0;
     p->counter_bytes = p->n_chunks > 1 ? align_up((size_t)p->n_tiles * sizeof(unsigned int), 256) : 0;
-    p->total_bytes = p->partial_bytes + p->counter_bytes;
+    p->total_bytes = p->partial_bytes + p->counter_bytes + p->tier_bytes;
 }
 
 // Ray ownership: a warp tile is cols_per_warp ray columns x R ray rows; the warp tiles of the grid are numbered
@@ -73,6 +73,7 @@ static TracePlan plan_trace_grid_t(const jt_grid* g, int64_t n_tnfw, bool f64) {
     p.tiles_y = (NY + p.R - 1) / p.R;
     p.n_wt = (int64_t)p.tiles_x * p.tiles_y;
     p.n_tiles = (p.n_wt + kTraceThreads / 32 - 1) / (kTraceThreads / 32);
+    p.tier_bytes = 64;
     plan_chunks(&p, n_tnfw, p.R, f64);
     return p;
 }
@@ -103,7 +104,7 @@ static void fill_lens(TraceArgs<T>& a, const jt_lens* lens, const TracePlan& pla
 
 template <typename T>
 static jt_status trace_grid_t(const jt_grid* g, const jt_lens* lens, const SrcSet& src, const TracePlan& plan,
-                              void* workspace, void* pre_psf, cudaStream_t st) {
+                              void* workspace, void* pre_psf, bool count_tiers, cudaStream_t st) {
     TraceArgs<T> a = {};
     const int s = g->supersample;
     a.nx = g->nx; a.ny = g->ny; a.s = s; a.NX = g->nx * s; a.NY = g->ny * s;
@@ -118,13 +119,21 @@ static jt_status trace_grid_t(const jt_grid* g, const jt_lens* lens, const SrcSe
     a.out = (T*)pre_psf;
     a.src = src;
     if (plan.n_chunks > 1) JT_CUDA_TRY(cudaMemsetAsync(a.counter, 0, plan.counter_bytes, st));
+    if (count_tiers) {
+        a.tier_counts = (unsigned long long*)trace_tier_counters(plan, workspace);
+        JT_CUDA_TRY(cudaMemsetAsync(a.tier_counts, 0, 4 * sizeof(unsigned long long), st));
+    }
     return launch_trace_t<T, true>(a, plan.R, st);
 }
 
+void* trace_tier_counters(const TracePlan& plan, void* workspace) {
+    return (char*)workspace + plan.partial_bytes + plan.counter_bytes;
+}
+
 jt_status launch_trace_grid(jt_dtype dtype, const jt_grid* g, const jt_lens* lens, const SrcSet& src,
-                            const TracePlan& plan, void* workspace, void* pre_psf, cudaStream_t st) {
-    return dtype == JT_F32 ? trace_grid_t<float>(g, lens, src, plan, workspace, pre_psf, st)
-                           : trace_grid_t<double>(g, lens, src, plan, workspace, pre_psf, st);
+                            const TracePlan& plan, void* workspace, void* pre_psf, bool count_tiers, cudaStream_t st) {
+    return dtype == JT_F32 ? trace_grid_t<float>(g, lens, src, plan, workspace, pre_psf, count_tiers, st)
+                           : trace_grid_t<double>(g, lens, src, plan, workspace, pre_psf, count_tiers, st);
 }
 
 template <typename T>

@@ -37,6 +37,7 @@ struct TraceArgs {
     int64_t chunk_len, n_tiles;
     double2* partial;
     unsigned int* counter;
+    unsigned long long* tier_counts;       // 4 counters or nullptr (profiling off)
     // grid mode output
     T* out;
     SrcSet src;
@@ -80,6 +81,9 @@ __device__ __noinline__ double2 tnfw_slow_f32(double xd, double yd, float cx, fl
 // loop carries only float per-tile sums (tx, ty); the double running sums live in a column of shared memory
 // (p[r * kTraceThreads]) that is touched once per staged tile, which keeps the float kernel at 128 registers
 // (2 CTAs per SM) without spilling the ray coordinates.
+// (warp, record) pairs handled by each form: far-far series, far, mid, queued for the per-ray cold path
+struct TierCount { unsigned int n[4]; };
+
 template <typename T, int R> struct DAcc;
 template <int R> struct DAcc<double, R> {
     double tx[R], ty[R];
@@ -168,7 +172,7 @@ __device__ __noinline__ void subhalo_cold(const SubRec<T>* rec, int64_t j, const
 template <typename T, int R, bool GRID>
 __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs, int count, int64_t base,
                                              const RawTn<T>& raw, const RayGeom& g, const T (&xs)[R], const T (&ys)[R],
-                                             DAcc<T, R>& acc, unsigned short* wq) {
+                                             DAcc<T, R>& acc, unsigned short* wq, TierCount& tiers) {
     T (&ax)[R] = acc.tx;
     T (&ay)[R] = acc.ty;
     acc.begin_tile();
@@ -196,7 +200,28 @@ __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs,
             }
         }
         const T X2min = R2min * s.iRs2;
-        if (__all_sync(0xffffffffu, X2min >= s.thr)) {
+        if (__all_sync(0xffffffffu, X2min >= s.thr2)) {
+            ++tiers.n[0];
+            if constexpr (sizeof(T) == 4 && R % 2 == 0) {
+#pragma unroll
+                for (int r = 0; r < R; r += 2) {
+                    float f0, f1;
+                    tnfw_farfar_pair(R2[r], R2[r + 1], s, f0, f1);
+                    ax[r] = fma(f0, dx[r], ax[r]);
+                    ay[r] = fma(f0, dy[r], ay[r]);
+                    ax[r + 1] = fma(f1, dx[r + 1], ax[r + 1]);
+                    ay[r + 1] = fma(f1, dy[r + 1], ay[r + 1]);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const T f = tnfw_farfar<T>(R2[r], s);
+                    ax[r] = fma(f, dx[r], ax[r]);
+                    ay[r] = fma(f, dy[r], ay[r]);
+                }
+            }
+        } else if (__all_sync(0xffffffffu, X2min >= s.thr)) {
+            ++tiers.n[1];
             if constexpr (sizeof(T) == 4 && R % 2 == 0) {
 #pragma unroll
                 for (int r = 0; r < R; r += 2) {
@@ -216,6 +241,7 @@ __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs,
                 }
             }
         } else if (__all_sync(0xffffffffu, X2min >= (T)kMidX2)) {
+            ++tiers.n[2];
 #pragma unroll
             for (int r = 0; r < R; ++r) {
                 const T f = tnfw_midfast<T>(R2[r], s);
@@ -225,6 +251,7 @@ __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs,
         } else {
             if ((threadIdx.x & 31) == 0) wq[qn] = (unsigned short)jj;
             ++qn;
+            ++tiers.n[3];
         }
     }
     if (qn > 0) {                                   // warp-uniform
@@ -250,7 +277,7 @@ __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs,
 template <typename T>
 __device__ __forceinline__ void stage_tile(SubRec<T>* recs, const RawTn<T>& raw, int64_t base, int64_t j_end, int tid,
                                            int nthreads) {
-    for (int k = tid; k < kSubTile; k += nthreads) {
+    for (int k = tid; k < SubTile<T>::value; k += nthreads) {
         const int64_t j = base + k;
         recs[k] = (j < j_end) ? make_rec<T>((double)raw.p[0][j], (double)raw.p[1][j], (double)raw.p[2][j],
                                             (double)raw.p[3][j], (double)raw.p[4][j])
@@ -294,9 +321,9 @@ __device__ __forceinline__ void grid_epilogue(const MacroLens& m, const SrcSet& 
 
 template <typename T, int R, bool GRID>
 __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_trace(const __grid_constant__ TraceArgs<T> a) {
-    __shared__ SubRec<T> recs[kSubTile];
+    __shared__ SubRec<T> recs[SubTile<T>::value];
     __shared__ int s_last;
-    __shared__ unsigned short s_queue[kTraceThreads / 32][kSubTile];
+    __shared__ unsigned short s_queue[kTraceThreads / 32][SubTile<T>::value];
     extern __shared__ __align__(16) unsigned char dacc_raw[];      // float mode: DAcc columns, R * 256 double2
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -332,20 +359,25 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_trace
 
     DAcc<T, R> acc;
     acc.init(reinterpret_cast<double2*>(dacc_raw) + tid);
+    TierCount tiers = {{0u, 0u, 0u, 0u}};
 
     // ---- subhalo sum over this CTA's chunk ----
     const RawTn<T> raw = {{a.tn[0], a.tn[1], a.tn[2], a.tn[3], a.tn[4]}};
     const int64_t j_begin = (int64_t)chunk * a.chunk_len;
     const int64_t j_end = min(a.M, j_begin + a.chunk_len);
-    for (int64_t base = j_begin; base < j_end; base += kSubTile) {
+    for (int64_t base = j_begin; base < j_end; base += SubTile<T>::value) {
         __syncthreads();
         stage_tile<T>(recs, raw, base, j_end, tid, kTraceThreads);
         __syncthreads();
-        const int count = (int)min((int64_t)kSubTile, j_end - base);
-        subhalo_tile<T, R, GRID>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp]);
+        const int count = (int)min((int64_t)SubTile<T>::value, j_end - base);
+        subhalo_tile<T, R, GRID>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp], tiers);
     }
     double axd[R], ayd[R];
     acc.result(axd, ayd);
+    if (a.tier_counts != nullptr && lane == 0) {          // measurement aid (jt_profile_tiers): four atomics per warp
+#pragma unroll
+        for (int k = 0; k < 4; ++k) atomicAdd(&a.tier_counts[k], (unsigned long long)tiers.n[k]);
+    }
 
     // ---- split subhalo list: publish partial sums; the last CTA of the tile reduces them in chunk order ----
     if (a.n_chunks > 1) {

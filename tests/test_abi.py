@@ -16,7 +16,7 @@ def _declared():
 
 def test_header_symbols_exported(jt):
     names = _declared()
-    assert len(names) == 15, names
+    assert len(names) == 16, names
     L = ctypes.CDLL(jt.lib_path())
     for n in names:
         assert hasattr(L, n), n
