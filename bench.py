@@ -36,11 +36,11 @@ if ROOT not in sys.path:
 METRIC = "ray_deflector_evals_per_s"
 UNIT = "evals/s"
 SM_COUNT = 148
-# Algorithmic work per evaluation on the binding unit: counted in the SASS of the warp-uniform
-# far-field loop (loop head + far body) divided by its 8 rays.  f32: FP32-pipe lane operations (an FFMA2 / FMUL2 / FADD2
-# counts as two; 237 per 8 rays; the loop needs only 21 issue slots per evaluation, so the 128-lane FP32 pipe binds);
-# f64: FP64-pipe instructions (405 per 8 rays; 64 lanes/clk/SM).
-ALG_INSTR_PER_EVAL = {"f32": 29.6, "f64": 50.6}
+# Algorithmic work per evaluation on the binding unit, counted in the SASS of each warp-uniform
+# tier loop (loop head + body) divided by its 8 rays; f32: FP32-pipe lane operations (a packed FFMA2 / FMUL2 / FADD2
+# counts as two); f64: FP64-pipe instructions.  Order: far-far series, far form, mid form, cold path (counted as far).
+# The mix of tiers is measured per run with jt_profile_tiers.
+TIER_COST = {"f32": (14.6, 29.6, 47.0, 29.6), "f64": (24.5, 50.6, 80.0, 50.6)}
 ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
 
@@ -325,6 +325,7 @@ def run_ours(args, rank, world, local_rank):
     launches0 = jt.kernel_launches()
 
     phase = []
+    tier_counts = (0, 0, 0, 0)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     for a, b in ev:
         flush.add_(1)
@@ -333,6 +334,7 @@ def run_ours(args, rank, world, local_rank):
         b.record()
         if not batch:
             phase.append(jt.profile_read())          # waits for this step's events only
+            tier_counts = jt.profile_tiers()
     torch.cuda.synchronize()
     barrier()
     launches = jt.kernel_launches() - launches0
@@ -378,7 +380,21 @@ def run_ours(args, rank, world, local_rank):
         conv_ms = float(np.mean([p[1] for p in phase]))
     else:
         trace_ms, conv_ms = ms_total_local / args.steps, 0.0
-    n_alg = ALG_INSTR_PER_EVAL[w.dtype]
+    # tier mix of the (warp, subhalo record) pairs: counters of the last timed jt_simulate_image call; for the batch
+    # kernel (no workspace, no counters) the same warp tiling is sampled through jt_simulate_image on 4 of its systems
+    if batch:
+        tiers = np.zeros(4)
+        jt.profile_enable(True)
+        for b in range(min(4, w.B)):
+            one = ImageRunner(jt, w.system(b), "direct")
+            one.step()
+            jt.profile_read()
+            tiers += np.array(jt.profile_tiers(), dtype=np.float64)
+        jt.profile_enable(False)
+    else:
+        tiers = np.array(tier_counts, dtype=np.float64)
+    mix = tiers / tiers.sum() if tiers.sum() > 0 else np.array([0.0, 1.0, 0.0, 0.0])
+    n_alg = float(np.dot(mix, TIER_COST[w.dtype]))
     achieved = w.evals * n_alg / (trace_ms * 1e-3) / 1e12
     line["roofline"] = {
         "bound": "alu", "kernel": "k_batch" if batch else "k_trace", "achieved": achieved, "peak": peak_tinstr,
@@ -386,7 +402,8 @@ def run_ours(args, rank, world, local_rank):
         "peak_kind": "derived: 148 SMs x %d lanes/clk (%s) x %.0f MHz (max clock, %s)" % (
             lanes, "FP32 pipe" if w.dtype == "f32" else "FP64 pipe", peaks.get("sm_max_mhz", 1965.0),
             peak_kind),
-        "alg_instr_per_eval": n_alg, "kernel_ms": trace_ms, "conv_ms": conv_ms,
+        "alg_instr_per_eval": n_alg, "tier_mix": {"far_far": mix[0], "far": mix[1], "mid": mix[2], "cold": mix[3]},
+        "tier_cost_per_eval": dict(zip(("far_far", "far", "mid", "cold"), TIER_COST[w.dtype])), "kernel_ms": trace_ms, "conv_ms": conv_ms,
         "kernel_share_of_step": trace_ms / (ms_total_local / args.steps),
         "frac_at_observed_clock": achieved / (SM_COUNT * lanes * f_mhz * 1e6 / 1e12),
         "evals_per_s_kernel": w.evals / (trace_ms * 1e-3)}

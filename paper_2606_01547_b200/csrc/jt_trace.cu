@@ -97,6 +97,12 @@ static void fill_lens(TraceArgs<T>& a, const jt_lens* lens, const TracePlan& pla
     a.tn[3] = (const T*)lens->tnfw_alpha_Rs; a.tn[4] = (const T*)lens->tnfw_r_trunc;
     a.n_chunks = plan.n_chunks;
     a.chunk_len = plan.chunk_len;
+    // records per staging round: the whole chunk when it fits (one barrier pair per CTA), else the largest tile that
+    // leaves room for 2 CTAs/SM (float: 96 B records + 32-64 KB of double sums) or 1 CTA/SM (double: 224 B records)
+    const int64_t cap = sizeof(T) == 8 ? 768 : 512;
+    int64_t tr = plan.chunk_len < cap ? plan.chunk_len : cap;
+    if (a.M < tr) tr = a.M;
+    a.tile_recs = (int)((tr < 1 ? 1 : tr) + 31) / 32 * 32;
     a.n_tiles = plan.n_tiles;
     a.partial = (double2*)workspace;
     a.counter = (unsigned int*)((char*)workspace + plan.partial_bytes);

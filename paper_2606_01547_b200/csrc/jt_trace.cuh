@@ -34,6 +34,7 @@ struct TraceArgs {
     int64_t M;
     const T* tn[5];
     int n_chunks;
+    int tile_recs;                         // subhalo records staged per shared-memory round
     int64_t chunk_len, n_tiles;
     double2* partial;
     unsigned int* counter;
@@ -130,7 +131,7 @@ template <int R> struct DAcc<float, R> {
     }
 };
 template <typename T, int R>
-constexpr size_t dacc_smem_bytes() { return sizeof(T) == 4 ? (size_t)R * kTraceThreads * sizeof(double2) : 0; }
+__host__ __device__ constexpr size_t dacc_smem_bytes() { return sizeof(T) == 4 ? (size_t)R * kTraceThreads * sizeof(double2) : 0; }
 
 // Cold path: one record against this thread's R rays when the warp is not uniformly far or mid.  Out of line, and
 // all per-ray state comes in through memory, so that the hot loop's register allocation never sees it.  Each ray
@@ -273,15 +274,14 @@ __device__ __forceinline__ void subhalo_tile(const SubRec<T>* __restrict__ recs,
     acc.end_tile();
 }
 
-// stage one tile of derived records (in double) from the raw arrays; entries past j_end are null records
+// stage `count` derived records (built in double) from the raw arrays starting at `base`
 template <typename T>
-__device__ __forceinline__ void stage_tile(SubRec<T>* recs, const RawTn<T>& raw, int64_t base, int64_t j_end, int tid,
+__device__ __forceinline__ void stage_tile(SubRec<T>* recs, const RawTn<T>& raw, int64_t base, int count, int tid,
                                            int nthreads) {
-    for (int k = tid; k < SubTile<T>::value; k += nthreads) {
+    for (int k = tid; k < count; k += nthreads) {
         const int64_t j = base + k;
-        recs[k] = (j < j_end) ? make_rec<T>((double)raw.p[0][j], (double)raw.p[1][j], (double)raw.p[2][j],
-                                            (double)raw.p[3][j], (double)raw.p[4][j])
-                              : null_rec<T>();
+        recs[k] = make_rec<T>((double)raw.p[0][j], (double)raw.p[1][j], (double)raw.p[2][j], (double)raw.p[3][j],
+                              (double)raw.p[4][j]);
     }
 }
 
@@ -321,10 +321,11 @@ __device__ __forceinline__ void grid_epilogue(const MacroLens& m, const SrcSet& 
 
 template <typename T, int R, bool GRID>
 __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_trace(const __grid_constant__ TraceArgs<T> a) {
-    __shared__ SubRec<T> recs[SubTile<T>::value];
     __shared__ int s_last;
-    __shared__ unsigned short s_queue[kTraceThreads / 32][SubTile<T>::value];
-    extern __shared__ __align__(16) unsigned char dacc_raw[];      // float mode: DAcc columns, R * 256 double2
+    // dynamic shared memory: [float mode: DAcc columns, R * 256 double2][tile_recs records][8 warp queues of tile_recs]
+    extern __shared__ __align__(32) unsigned char dacc_raw[];
+    SubRec<T>* recs = reinterpret_cast<SubRec<T>*>(dacc_raw + dacc_smem_bytes<T, R>());
+    unsigned short* s_queue = reinterpret_cast<unsigned short*>(recs + a.tile_recs);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int64_t tile = (int64_t)blockIdx.x / a.n_chunks;
@@ -365,12 +366,12 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_trace
     const RawTn<T> raw = {{a.tn[0], a.tn[1], a.tn[2], a.tn[3], a.tn[4]}};
     const int64_t j_begin = (int64_t)chunk * a.chunk_len;
     const int64_t j_end = min(a.M, j_begin + a.chunk_len);
-    for (int64_t base = j_begin; base < j_end; base += SubTile<T>::value) {
+    for (int64_t base = j_begin; base < j_end; base += a.tile_recs) {
+        const int count = (int)min((int64_t)a.tile_recs, j_end - base);
         __syncthreads();
-        stage_tile<T>(recs, raw, base, j_end, tid, kTraceThreads);
+        stage_tile<T>(recs, raw, base, count, tid, kTraceThreads);
         __syncthreads();
-        const int count = (int)min((int64_t)SubTile<T>::value, j_end - base);
-        subhalo_tile<T, R, GRID>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp], tiers);
+        subhalo_tile<T, R, GRID>(recs, count, base, raw, g, xs, ys, acc, s_queue + warp * a.tile_recs, tiers);
     }
     double axd[R], ayd[R];
     acc.result(axd, ayd);
@@ -438,8 +439,8 @@ jt_status launch_trace_t(const TraceArgs<T>& a, int R, cudaStream_t st);
 #define JT_TRACE_CASE(RR)                                                                         \
     case RR: {                                                                                    \
         auto kern = k_trace<T, RR, GRID>;                                                         \
-        const size_t dsm = dacc_smem_bytes<T, RR>();                                              \
-        if (dsm > 0) JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm)); \
+        const size_t dsm = dacc_smem_bytes<T, RR>() + (size_t)a.tile_recs * (sizeof(SubRec<T>) + (kTraceThreads / 32) * 2); \
+        JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));   \
         kern<<<(unsigned)grid, kTraceThreads, dsm, st>>>(a);                                      \
         break;                                                                                    \
     }
