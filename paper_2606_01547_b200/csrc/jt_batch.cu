@@ -95,7 +95,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
         TierCount tiers = {{0u, 0u, 0u, 0u}};
 
         if (resident) {
-            subhalo_tile<T, R, true>(recs, a.M, 0, raw, g, xs, ys, acc, s_queue[warp], tiers);
+            subhalo_tile<T, R, true, false>(recs, a.M, 0, raw, g, xs, ys, acc, s_queue[warp], tiers);
         } else {
             for (int base = 0; base < a.M; base += a.rec_cap) {
                 const int count = min(a.rec_cap, a.M - base);
@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
                                           (double)raw.p[2][base + k], (double)raw.p[3][base + k],
                                           (double)raw.p[4][base + k]);
                 __syncthreads();
-                subhalo_tile<T, R, true>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp], tiers);
+                subhalo_tile<T, R, true, false>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp], tiers);
             }
         }
         double axd[R], ayd[R];
