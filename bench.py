@@ -40,7 +40,7 @@ SM_COUNT = 148
 # tier loop (loop head + body) divided by its 8 rays; f32: FP32-pipe lane operations (a packed FFMA2 / FMUL2 / FADD2
 # counts as two); f64: FP64-pipe instructions.  Order: far-far series, far form, mid form, cold path (counted as far).
 # The mix of tiers is measured per run with jt_profile_tiers.
-TIER_COST = {"f32": (14.6, 29.6, 47.0, 29.6), "f64": (24.5, 50.6, 80.0, 50.6)}
+TIER_COST = {"f32": (14.5, 29.6, 47.0, 29.6), "f64": (25.2, 50.6, 80.0, 50.6)}
 ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
 
