@@ -75,6 +75,39 @@ def test_ray_shoot_through_subhalo_cores(jt, orc, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_ray_shoot_far_far_series(jt, orc, dtype):
+    """One subhalo at a time, rays at X = R/Rs from 4 to 1e4 times max(1, tau), tau from 0.3 to 30: both sides of the
+    far-far radius (9 / 8 max(1, tau)) where the kernel switches from the far form to the 1/X series of the brace.
+    The deflection itself is compared, relative to its own size (series error <= 1e-13 / 2e-8)."""
+    rng = np.random.default_rng(17)
+    worst = 0.0
+    for tau in (0.3, 0.7, 1.0, 2.0, 5.0, 12.0, 30.0):
+        Rs, aRs = 0.01, 5e-3
+        tn = np.array([[0.013], [-0.007], [Rs], [aRs], [tau * Rs]])
+        X = np.concatenate([np.logspace(np.log10(4.0), 4.0, 600), np.linspace(7.5, 10.5, 200)]) * max(1.0, tau)
+        ang = rng.uniform(0, 2 * np.pi, X.size)
+        tx = tn[0, 0] + X * Rs * np.cos(ang)
+        ty = tn[1, 0] + X * Rs * np.sin(ang)
+        if dtype == "f32":
+            tx, ty, tn = _f32r(tx), _f32r(ty), _f32r(tn)
+        bx, by = jt.ray_shoot(to_dev(tx, dtype), to_dev(ty, dtype), None, None, to_dev(tn, dtype))
+        wx, wy = orc.ray_shoot(tx, ty, None, None, tn)
+        ax, ay = tx - bx.double().cpu().numpy(), ty - by.double().cpu().numpy()
+        wax, way = tx - wx, ty - wy
+        mag = np.hypot(wax, way)
+        if dtype == "f64":
+            # beta = theta - alpha is stored in double: alpha is recovered to ~1e-16 |theta|
+            err = np.hypot(ax - wax, ay - way) / (mag + 1e-16 * np.hypot(tx, ty) / 1e-12)
+            worst = max(worst, float(err.max()))
+        else:
+            # float: beta is stored in float (half an ulp of |theta| = 6e-8 |theta|) and the float arithmetic of one
+            # evaluation is good to a few 1e-7 of alpha; the series adds 2e-8
+            err = np.hypot(ax - wax, ay - way) / (3e-6 * mag + 2e-7 * np.hypot(tx, ty))
+            worst = max(worst, float(err.max()))
+    assert worst < (1e-11 if dtype == "f64" else 1.0), worst
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("e1,e2", [(-0.3, 0.35), (0.0, 0.0), (1e-9, 0.0), (0.6, -0.5), (0.9, 0.9), (-0.19, -0.12)])
 def test_ray_shoot_sie_ellipticities(jt, orc, dtype, e1, e2):
     """SIE alone over the full range of definition E: q below 0.707 (f x'/psi above 1), circular, |e| clamped."""
