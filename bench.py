@@ -260,8 +260,14 @@ def cpu_baseline(w, target_evals):
     orc.set_threads(cores)
     sample = oracle_sample(w, target_evals)
     sec = oracle_step(orc, w, sample)
+    # the same oracle on ONE core, on a sample cores times smaller (both numbers are reported)
+    orc.set_threads(1)
+    s1 = oracle_sample(w, target_evals / max(cores, 1))
+    sec1 = oracle_step(orc, w, s1)
+    orc.set_threads(cores)
     return {"value": sample["evals"] / sec, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": sample["text"], "seconds": sec}
+            "sample": sample["text"], "seconds": sec,
+            "single_core": {"value": s1["evals"] / sec1, "sample": s1["text"], "seconds": sec1}}
 
 
 def run_reference(args, rank, world):
