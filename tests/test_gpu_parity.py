@@ -326,6 +326,31 @@ def test_image_edge_cases(jt, orc, dtype):
     _check_image(jt, orc, wn, method="auto")
 
 
+@pytest.mark.parametrize("seed", range(16))
+def test_image_random_shapes(jt, orc, seed):
+    """Seeded random configurations of the fused call: grid shape and offset, supersampling, subhalo count (around the
+    staging-tile and chunk-split boundaries), tau from 0.5 to 20 (all four tiers of definition T), 1-3 sources, PSF shape,
+    dtype and convolution method."""
+    rng = np.random.default_rng(9000 + seed)
+    dtype = "f64" if seed % 2 == 0 else "f32"
+    nx, ny = int(rng.integers(3, 70)), int(rng.integers(3, 70))
+    s = int(rng.choice([1, 2, 3, 4, 5, 7]))
+    M = int(rng.choice([0, 1, 31, 255, 257, 700, 1537, 3000]))
+    K = (int(rng.choice([1, 3, 9, 21, 33])), int(rng.choice([1, 5, 13, 27])))
+    w = workloads.config_c4(nx=nx, n_tnfw=M, K=9, half_width=0.04 * max(nx, ny) * 0.6, dtype="f64")
+    w.ny = ny
+    w.supersample = s
+    w.pixel_scale = 0.04
+    w.cx, w.cy = float(rng.uniform(-0.05, 0.05)), float(rng.uniform(-0.05, 0.05))
+    if M:
+        w.tnfw[4] = w.tnfw[2] * rng.uniform(0.5, 20.0, M)
+    w.sources = w.sources[: int(rng.integers(1, 4))]
+    psf = rng.uniform(0, 1, K)
+    w.psf = psf / psf.sum()
+    w = w.as_dtype(dtype)
+    _check_image(jt, orc, w, method=str(rng.choice(["direct", "fft", "auto"])))
+
+
 def test_c2_full_size_sampled_rows(jt, orc):
     """Full-size C2 (200x200, s=2, 10,000 subhalos) in the launch configuration bench.py times:
     three pixel rows of the pre-PSF image against the oracle, f64 and f32."""
