@@ -142,6 +142,16 @@ __device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, d
     for (int k = 2; k <= FarFar<T>::K; ++k) r.ak[k - 2] = (T)(f * farfar_coef(k, t));
 #pragma unroll
     for (int k = FarFar<T>::K - 1; k < (int)(sizeof(r.ak) / sizeof(T)); ++k) r.ak[k] = (T)0;
+    // extreme tau (float: beyond ~1e3): the top coefficients leave T's range -> no far-far tier for this record
+    bool ok = isfinite((double)r.a0);
+#pragma unroll
+    for (int k = 0; k < FarFar<T>::K - 1; ++k) ok = ok && isfinite((double)r.ak[k]) && fabs((double)r.ak[k]) < (sizeof(T) == 4 ? 1e30 : 1e250);
+    if (!ok) {
+        r.thr2 = (T)(sizeof(T) == 4 ? 3.0e38 : 1.0e300);
+        r.a0 = (T)0;
+#pragma unroll
+        for (int k = 0; k < FarFar<T>::K - 1; ++k) r.ak[k] = (T)0;
+    }
     return r;
 }
 // padding record: contributes exactly 0 and always takes the far path

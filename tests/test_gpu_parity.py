@@ -108,6 +108,27 @@ def test_ray_shoot_far_far_series(jt, orc, dtype):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_ray_shoot_extreme_truncation(jt, orc, dtype):
+    """tau = r_trunc/Rs far outside the priors (100 ... 1e5): the far-far coefficients grow like tau^12; records whose
+    coefficients leave the dtype's range must fall back to the far form -- finite results that still match."""
+    rng = np.random.default_rng(23)
+    for tau in (100.0, 3.0e3, 1.0e5):
+        Rs = 0.01
+        tn = np.array([[0.0], [0.0], [Rs], [1e-3], [tau * Rs]])
+        X = np.logspace(0.5, 7.0, 400)
+        ang = rng.uniform(0, 2 * np.pi, X.size)
+        tx, ty = X * Rs * np.cos(ang), X * Rs * np.sin(ang)
+        if dtype == "f32":
+            tx, ty, tn = _f32r(tx), _f32r(ty), _f32r(tn)
+        bx, by = jt.ray_shoot(to_dev(tx, dtype), to_dev(ty, dtype), None, None, to_dev(tn, dtype))
+        bx, by = bx.double().cpu().numpy(), by.double().cpu().numpy()
+        assert np.isfinite(bx).all() and np.isfinite(by).all(), tau
+        wx, wy = orc.ray_shoot(tx, ty, None, None, tn)
+        scale = np.hypot(tx - wx, ty - wy) * (1e-9 if dtype == "f64" else 1e-5) + np.hypot(tx, ty) * (1e-15 if dtype == "f64" else 2e-7)
+        assert (np.hypot(bx - wx, by - wy) <= scale).all(), tau
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("e1,e2", [(-0.3, 0.35), (0.0, 0.0), (1e-9, 0.0), (0.6, -0.5), (0.9, 0.9), (-0.19, -0.12)])
 def test_ray_shoot_sie_ellipticities(jt, orc, dtype, e1, e2):
     """SIE alone over the full range of definition E: q below 0.707 (f x'/psi above 1), circular, |e| clamped."""
