@@ -41,6 +41,9 @@ SM_COUNT = 148
 # counts as two); f64: FP64-pipe instructions.  Order: far-far series, far form, mid form, cold path (counted as far).
 # The mix of tiers is measured per run with jt_profile_tiers.
 TIER_COST = {"f32": (14.5, 29.6, 47.0, 29.6), "f64": (25.2, 50.6, 80.0, 50.6)}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu --set full captures in
+# profiles/r01d_ncu_{c2f64,c2f32,c3f32}.txt (the kernels are ALU-bound: compulsory traffic is parameters in, image out)
+NCU_TRAFFIC_BYTES = {"C2-f64": 483072 + 1126400, "C2-f32": 267008 + 510976, "C3-f32": 15798016 + 41087488}
 ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
 
@@ -404,7 +407,7 @@ def run_ours(args, rank, world, local_rank):
     achieved = w.evals * n_alg / (trace_ms * 1e-3) / 1e12
     line["roofline"] = {
         "bound": "alu", "kernel": "k_batch" if batch else "k_trace", "achieved": achieved, "peak": peak_tinstr,
-        "unit": "Tlaneop/s", "frac": achieved / peak_tinstr, "traffic": None,
+        "unit": "Tlaneop/s", "frac": achieved / peak_tinstr, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
         "peak_kind": "derived: 148 SMs x %d lanes/clk (%s) x %.0f MHz (max clock, %s)" % (
             lanes, "FP32 pipe" if w.dtype == "f32" else "FP64 pipe", peaks.get("sm_max_mhz", 1965.0),
             peak_kind),

@@ -5,7 +5,8 @@
 // two >= n + K - 1), Z = FFT2(z);  A = FFT2(img) = (Z(k) + conj Z(-k))/2,  B = FFT2(ker) = (Z(k) - conj Z(-k))/(2i);
 // C = A B is Hermitian, out = Re IFFT2(C) cropped at (ky/2, kx/2).
 //
-// Forward transforms are decimation-in-frequency (natural order in, bit-reversed positions out), inverse
+// Forward transforms are decimation-in-frequency (natural order in, bit-reversed positions out; two radix-2 stages
+// fused per shared-memory pass), inverse
 // transforms decimation-in-time with conjugate twiddles (bit-reversed positions in, natural order out), so no
 // permutation pass exists anywhere: position p of an axis holds frequency brev(p), and the pointwise step pairs
 // position (py, px) with (brev(-brev py), brev(-brev px)).
@@ -51,39 +52,82 @@ __device__ __forceinline__ void make_twiddles(Cd* tw, int n, int tid, int nthr) 
     }
 }
 
-// nb transforms of length n = 2^logn at s + b * pitch.  Forward, decimation in frequency.
+// nb transforms of length n = 2^logn at s + b * pitch.  Forward, decimation in frequency.  Two radix-2 stages are
+// fused per pass (a thread carries four points through both in registers: half the shared-memory traffic and half the
+// barriers of a stage-by-stage sweep, identical arithmetic); an odd logn ends with one plain radix-2 stage.
 __device__ __forceinline__ void fft_dif(Cd* s, const Cd* tw, int logn, int nb, int pitch, int tid, int nthr) {
-    const int half = 1 << (logn - 1);
-    const int total = nb * half;
-    for (int lh = logn - 1; lh >= 0; --lh) {
-        const int h = 1 << lh;
+    int lh = logn - 1;
+    for (; lh >= 1; lh -= 2) {                       // stages with half-sizes h = 2^lh and q = h/2
+        const int h = 1 << lh, q = h >> 1;
+        const int quarter = 1 << (logn - 2);
+        const int total = nb * quarter;
+        for (int u = tid; u < total; u += nthr) {
+            const int tr = u >> (logn - 2), uu = u & (quarter - 1);
+            const int k = uu & (q - 1), g = uu >> (lh - 1);
+            const int i0 = tr * pitch + (g << (lh + 1)) + k, i1 = i0 + q, i2 = i0 + h, i3 = i2 + q;
+            const Cd x0 = s[i0], x1 = s[i1], x2 = s[i2], x3 = s[i3];
+            const Cd wa = tw[k << (logn - 1 - lh)], wb = tw[(k + q) << (logn - 1 - lh)], wc = tw[k << (logn - lh)];
+            const Cd a0 = {x0.x + x2.x, x0.y + x2.y};
+            const Cd a2 = cmul({x0.x - x2.x, x0.y - x2.y}, wa);
+            const Cd a1 = {x1.x + x3.x, x1.y + x3.y};
+            const Cd a3 = cmul({x1.x - x3.x, x1.y - x3.y}, wb);
+            s[i0] = {a0.x + a1.x, a0.y + a1.y};
+            s[i1] = cmul({a0.x - a1.x, a0.y - a1.y}, wc);
+            s[i2] = {a2.x + a3.x, a2.y + a3.y};
+            s[i3] = cmul({a2.x - a3.x, a2.y - a3.y}, wc);
+        }
+        __syncthreads();
+    }
+    if (lh == 0) {                                   // last stage, h = 1, twiddle 1
+        const int half = 1 << (logn - 1);
+        const int total = nb * half;
         for (int b = tid; b < total; b += nthr) {
             const int tr = b >> (logn - 1), bb = b & (half - 1);
-            const int k = bb & (h - 1), g = bb >> lh;
-            const int i = tr * pitch + (g << (lh + 1)) + k, j = i + h;
+            const int i = tr * pitch + (bb << 1), j = i + 1;
             const Cd a = s[i], c = s[j];
-            const Cd w = tw[k << (logn - 1 - lh)];
             s[i] = {a.x + c.x, a.y + c.y};
-            s[j] = cmul({a.x - c.x, a.y - c.y}, w);
+            s[j] = cmul({a.x - c.x, a.y - c.y}, tw[0]);
         }
         __syncthreads();
     }
 }
 
-// Inverse of fft_dif stage by stage (unnormalised: fft_dit_inv(fft_dif(x)) = n x).
+// Inverse of fft_dif stage by stage (unnormalised: fft_dit_inv(fft_dif(x)) = n x), the stages fused in pairs likewise.
 __device__ __forceinline__ void fft_dit_inv(Cd* s, const Cd* tw, int logn, int nb, int pitch, int tid, int nthr) {
-    const int half = 1 << (logn - 1);
-    const int total = nb * half;
-    for (int lh = 0; lh < logn; ++lh) {
-        const int h = 1 << lh;
+    int lh = 0;
+    if (logn & 1) {                                  // undo fft_dif's last stage first (h = 1)
+        const int half = 1 << (logn - 1);
+        const int total = nb * half;
         for (int b = tid; b < total; b += nthr) {
             const int tr = b >> (logn - 1), bb = b & (half - 1);
-            const int k = bb & (h - 1), g = bb >> lh;
-            const int i = tr * pitch + (g << (lh + 1)) + k, j = i + h;
+            const int i = tr * pitch + (bb << 1), j = i + 1;
             const Cd a = s[i];
-            const Cd c = cmul_conj(s[j], tw[k << (logn - 1 - lh)]);
+            const Cd c = cmul_conj(s[j], tw[0]);
             s[i] = {a.x + c.x, a.y + c.y};
             s[j] = {a.x - c.x, a.y - c.y};
+        }
+        __syncthreads();
+        lh = 1;
+    }
+    for (; lh + 1 < logn; lh += 2) {                 // stages with half-sizes h = 2^lh and 2h
+        const int h = 1 << lh;
+        const int quarter = 1 << (logn - 2);
+        const int total = nb * quarter;
+        for (int u = tid; u < total; u += nthr) {
+            const int tr = u >> (logn - 2), uu = u & (quarter - 1);
+            const int k = uu & (h - 1), g = uu >> lh;
+            const int i0 = tr * pitch + (g << (lh + 2)) + k, i1 = i0 + h, i2 = i1 + h, i3 = i2 + h;
+            const Cd x0 = s[i0], x2 = s[i2];
+            const Cd w1 = tw[k << (logn - 1 - lh)];
+            const Cd c1 = cmul_conj(s[i1], w1), c3 = cmul_conj(s[i3], w1);
+            const Cd b0 = {x0.x + c1.x, x0.y + c1.y}, b1 = {x0.x - c1.x, x0.y - c1.y};
+            const Cd b2 = {x2.x + c3.x, x2.y + c3.y}, b3 = {x2.x - c3.x, x2.y - c3.y};
+            const Cd d2 = cmul_conj(b2, tw[k << (logn - 2 - lh)]);
+            const Cd d3 = cmul_conj(b3, tw[(k + h) << (logn - 2 - lh)]);
+            s[i0] = {b0.x + d2.x, b0.y + d2.y};
+            s[i2] = {b0.x - d2.x, b0.y - d2.y};
+            s[i1] = {b1.x + d3.x, b1.y + d3.y};
+            s[i3] = {b1.x - d3.x, b1.y - d3.y};
         }
         __syncthreads();
     }
@@ -264,11 +308,13 @@ static FftPlan plan_fft(jt_dtype d, int ny, int nx, int ky, int kx) {
 
 bool conv_fft_supported(jt_dtype d, int ny, int nx, int ky, int kx) { return plan_fft(d, ny, nx, ky, kx).ok; }
 
-// Time model behind JT_CONV_AUTO (bench.py --conv-sweep on B200: P = 128: 20 us, 256: 29, 512: 44, 1024: 104, 2048: 408)
+// Time model behind JT_CONV_AUTO (bench.py --conv-sweep on B200: P = 128: 17 us, 256: 21.5, 512: 34, 1024: 77, 2048: 305;
+// beyond 1024 x 1024 the 16 B/point plane no longer sits comfortably in L2)
 double conv_fft_estimate_us(jt_dtype d, int ny, int nx, int ky, int kx) {
     const FftPlan p = plan_fft(d, ny, nx, ky, kx);
     if (!p.ok) return 1e30;
-    return 8.0 + 0.9 * (p.logPx + p.logPy) + 90.0 * ((double)p.Px * p.Py / 1048576.0);
+    const double area = (double)p.Px * p.Py / 1048576.0;
+    return 1.17 * (p.logPx + p.logPy) + 54.0 * area + (area > 1.0 ? 20.0 * (area - 1.0) : 0.0);
 }
 
 size_t fft_conv_workspace_bytes(jt_dtype d, int ny, int nx, int ky, int kx) {
