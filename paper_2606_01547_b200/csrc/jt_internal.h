@@ -10,7 +10,6 @@ namespace jt {
 
 constexpr int kNumSMs = 148;            // B200
 constexpr int kTraceThreads = 256;      // 8 warps per CTA in the ray-tracing kernels
-template <typename T> struct SubTile { static constexpr int value = sizeof(T) == 8 ? 128 : 256; };   // records staged per shared-memory tile (224 B / 96 B each)
 
 // thread-local last CUDA error (jt_last_cuda_error)
 void set_last_cuda_error(int e);
@@ -42,7 +41,7 @@ struct TracePlan {
     int64_t n_wt;          // grid mode: warp tiles in all
     int64_t n_tiles;       // CTAs per subhalo chunk (8 warp tiles, or 8 * 32 * R rays in ray mode)
     int n_chunks;          // subhalo list split (1 = no workspace traffic)
-    int64_t chunk_len;     // subhalos per chunk (multiple of kSubTile unless n_chunks == 1)
+    int64_t chunk_len;     // subhalos per chunk
     size_t partial_bytes;  // n_chunks > 1: double2 per (chunk, ray slot)
     size_t counter_bytes;  // one uint32 per tile
     size_t tier_bytes;     // grid mode: four uint64 tier counters (jt_profile_tiers), always reserved

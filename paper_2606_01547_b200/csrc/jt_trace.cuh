@@ -5,14 +5,19 @@
 //              -> pre-PSF image.  Traced coordinates never leave the chip (PAPER.md:55 steps 1+2 fused).
 //   RAYS mode  (jt_ray_shoot): same subhalo sum + SIE + shear on caller-supplied ray positions -> beta.
 //
-// N-body-style structure (PAPER.md:47 is where the time goes): 256 threads, each owning R rays whose
-// deflection accumulators live in registers; the subhalo list streams through shared memory in tiles
-// of 256 derived records (SubRec, built in double by the staging threads).  Per record a warp takes the
-// logarithm-free far-field form when all of its rays have X^2 >= max(10, 3 tau^2) (>98 % of the
-// pairs in the paper-shaped workloads) and a per-ray generic form otherwise.
-// When there are too few ray tiles to fill 148 SMs the subhalo list is split into chunks; every
-// (tile, chunk) CTA writes double partial sums to the workspace and the last CTA to arrive for a tile
-// adds them in chunk order (deterministic) and runs the epilogue.
+// N-body-style structure (PAPER.md:47 is where the time goes): 256 threads, each owning R rays whose deflection
+// accumulators live in registers (float: per-tile float sums + double running sums in shared memory); a warp owns a
+// "warp tile" of cols_per_warp x R rays, warp tiles are dealt to CTAs eight at a time.  The subhalo list streams
+// through shared memory in tiles of derived records (SubRec, built in double by the staging threads; the CTA's whole
+// chunk when it fits).  Per record the warp votes on the form of definition T:
+//   far-far  X >= 9 max(1, tau):  the 1/X series of the brace (1 MUFU + K+1 multiply-adds), two records per iteration
+//   far      X^2 >= max(10, 3 tau^2): logarithm-free closed form (3 MUFU + two polynomials)
+//   mid      X^2 >= 2: the same with one logarithm
+//   else     queued per warp and handled per ray by the out-of-line subhalo_cold after the hot loop
+// float runs the far-far and far forms on two rays at once with packed f32x2 instructions (FFMA2 / FMUL2 / FADD2).
+// When there are too few ray tiles to fill 148 SMs the subhalo list is split into chunks (wave-aware choice in
+// jt_trace.cu); every (tile, chunk) CTA writes double partial sums to the workspace and the last CTA to arrive for
+// a tile adds them in chunk order (deterministic) and runs the epilogue.
 #pragma once
 #include "jt_internal.h"
 
