@@ -18,7 +18,8 @@
  * Pins (tests/test_oracle_*.py): SIS |alpha|=theta_E; point mass theta_E^2/r; div alpha =
  * 2 kappa and curl alpha = 0 by central differences for S, H, T; NFW limit of T; total-mass
  * limit of T; projected TNFW mass against numerical line-of-sight quadrature (mpmath);
- * Sersic isophote / total flux closed forms; grid + bin invariants; convolution against
+ * Sersic isophote / total flux closed forms and the half-light fraction inside R_sersic (pins the two
+ * constants of b_n, reading Q10); grid + bin invariants; convolution against
  * scipy.signal.convolve2d, delta / shift kernels, flux conservation, 8x8 brute force.
  * The composed pipeline has no external implementation to compare with: "parity unpinned"
  * end-to-end, pinned per step (SURVEY.md §8(c) last pin row).

@@ -59,6 +59,44 @@ def test_sersic_total_flux_closed_form(orc, n, e1, e2):
     assert abs(got - want) < 2e-8 * want
 
 
+def _golden(name):
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)
+    return np.loadtxt(path, comments="#", ndmin=2)
+
+
+@pytest.mark.parametrize("row", range(4))
+def test_sersic_half_light_fraction_pins_bn(orc, row):
+    """Pins the constants of b_n (reading Q10) without retyping them: the flux of orc.sersic inside the R_sersic isophote
+    over its total flux, both by quadrature of the oracle's own function, against (i) the four values SURVEY.md section
+    8(c) Q10 prints for this reading (tests/golden/sersic_half_light.txt), (ii) scipy's regularised incomplete gamma
+    function at the b recovered from the oracle's centre value I(0)/amp = e^b, and (iii) the definition of a half-light
+    radius (fraction near 1/2 for n in [0.5, 4]).  A wrong digit in either constant moves the fraction by > 1e-3."""
+    n, want = _golden("sersic_half_light.txt")[row]
+    amp, Rs = 2.0, 0.35
+    prof = lambda r: orc.sersic(r, 0.0, amp, Rs, n, 0.0, 0.0, 0.0, 0.0) * r
+    inner, _ = integrate.quad(prof, 0.0, Rs, epsabs=1e-13, epsrel=1e-12, limit=400)
+    outer = sum(integrate.quad(prof, a, b, epsabs=1e-13, epsrel=1e-12, limit=400)[0]
+                for a, b in ((Rs, 10 * Rs), (10 * Rs, 1e3 * Rs), (1e3 * Rs, 1e6 * Rs)))
+    frac = inner / (inner + outer)
+    assert abs(frac - want) < 2e-4                                         # the survey's printed value (4 digits)
+    b = math.log(orc.sersic(0.0, 0.0, amp, Rs, n, 0.0, 0.0, 0.0, 0.0) / amp)
+    assert abs(frac - special.gammainc(2 * n, b)) < 1e-9                   # textbook closed form P(2n, b)
+    assert abs(frac - 0.5) < 0.011                                         # R_sersic is (nearly) the half-light radius
+    # the same fraction for an elliptical source: the isophote region q x'^2 + y'^2/q <= Rs^2 (2-D quadrature)
+    if n == 1.5:
+        e1, e2 = 0.2, -0.15
+        phi, q = orc.ellipticity(e1, e2)
+
+        def f(u, t):        # u in [0,1]: elliptical radius u Rs; area element Rs^2 u du dt (unit Jacobian of the q-stretch)
+            xr, yr = u * Rs / math.sqrt(q) * math.cos(t), u * Rs * math.sqrt(q) * math.sin(t)
+            x = math.cos(phi) * xr - math.sin(phi) * yr
+            y = math.sin(phi) * xr + math.cos(phi) * yr
+            return orc.sersic(x, y, amp, Rs, n, e1, e2, 0.0, 0.0) * Rs * Rs * u
+        inner2, _ = integrate.dblquad(f, 0, 2 * math.pi, 0, 1.0, epsabs=1e-11, epsrel=1e-11)
+        assert abs(inner2 / (2 * math.pi * (inner + outer)) - want) < 2e-4
+
+
 def test_sersic_centre_and_profile(orc):
     n, Rs = 2.0, 0.4
     b = 1.9992 * n - 0.3271
