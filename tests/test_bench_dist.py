@@ -25,8 +25,6 @@ def _worker(rank, world, port, q):
     assert (r, w, lr) == (rank, world, rank)
     bench.barrier()
     units, ms = bench.aggregate(1000.0 * (rank + 1), 5.0 + 2.0 * rank, device="cpu")
-    # replicas get different seeds, same shapes
-    wl = bench.make_workload("C3-f32", rank) if False else None
     q.put((rank, units, ms, bench.shard_range(4096, rank, world)))
     import torch.distributed as dist
     dist.destroy_process_group()

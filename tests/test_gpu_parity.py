@@ -177,7 +177,8 @@ def test_source_brightness(jt, orc, dtype):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("ny,nx,ky,kx", [(8, 8, 3, 3), (8, 8, 5, 3), (60, 60, 11, 11), (100, 100, 31, 31),
                                          (64, 64, 21, 21), (37, 91, 7, 13), (130, 75, 45, 45), (5, 7, 11, 9),
-                                         (200, 200, 21, 21), (33, 31, 1, 1)])
+                                         (200, 200, 21, 21), (33, 31, 1, 1), (180, 180, 135, 135), (301, 203, 101, 7),
+                                         (300, 420, 101, 101), (64, 1000, 3, 201), (70, 66, 151, 9)])
 def test_convolve_direct(jt, orc, dtype, ny, nx, ky, kx):
     rng = np.random.default_rng(ny * 1000 + nx + ky)
     img = rng.uniform(0, 1, (ny, nx))
@@ -189,6 +190,34 @@ def test_convolve_direct(jt, orc, dtype, ny, nx, ky, kx):
     want = orc.convolve(img, ker)
     # f32: ky*kx sequential float additions of positive terms, random-walk rounding ~ sqrt(ky kx) 2^-24
     assert rel_err(got, want) < (1e-13 if dtype == "f64" else max(2e-6, 3.0 * (ky * kx) ** 0.5 * 2.0 ** -24))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("B,ny,nx,k", [(5, 60, 60, 21), (3, 100, 100, 13), (7, 33, 47, 45), (2, 180, 180, 135), (130, 16, 20, 5)])
+def test_convolve_batch(jt, orc, dtype, B, ny, nx, k):
+    """jt_psf_convolve_batch (B images, one kernel) = the oracle's convolution image by image, both methods;
+    covers the TMA tile path (aligned pitch) and the plain-load fallback (33 x 47: odd pitch)."""
+    rng = np.random.default_rng(B * 100 + k)
+    imgs = rng.uniform(0, 1, (B, ny, nx))
+    ker = rng.uniform(0, 1, (k, k))
+    ker /= ker.sum()
+    if dtype == "f32":
+        imgs, ker = _f32r(imgs), _f32r(ker)
+    want = np.stack([orc.convolve(imgs[b], ker) for b in range(B)])
+    for method in ("direct", "fft", "auto"):
+        got = jt.psf_convolve_batch(to_dev(imgs, dtype), to_dev(ker, dtype), method=method).double().cpu().numpy()
+        assert rel_err(got, want) < (1e-12 if dtype == "f64" else max(2e-6, 3.0 * k * 2.0 ** -24)), method
+
+
+def test_convolve_direct_unaligned_view(jt, orc):
+    """An image whose base address is not 16-byte aligned takes the plain-load tile fill, same result."""
+    rng = np.random.default_rng(12)
+    flat = to_dev(rng.uniform(0, 1, 64 * 64 + 1), "f32")
+    img = flat[1:].view(64, 64)
+    ker = to_dev(rng.uniform(0, 1, (9, 9)) / 40.0, "f32")
+    got = jt.psf_convolve(img, ker, method="direct").double().cpu().numpy()
+    want = orc.convolve(img.double().cpu().numpy(), ker.double().cpu().numpy())
+    assert rel_err(got, want) < 2e-6
 
 
 def test_convolve_delta_and_shift(jt):
