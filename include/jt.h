@@ -54,7 +54,7 @@
 extern "C" {
 #endif
 
-#define JT_VERSION 100           /* 0.1.0 */
+#define JT_VERSION 200           /* 0.2.0 */
 #define JT_MAX_SUPERSAMPLE 16    /* s x s sub-rays per pixel, binned with warp shuffles */
 #define JT_MAX_SOURCES 16        /* Sersic components per system (host arrays, passed by value to kernels) */
 
@@ -108,14 +108,28 @@ JT_API jt_status jt_source_brightness(jt_dtype dtype, int64_t n, const void *bet
  * out[j][i] = sum_{u<ky} sum_{v<kx} K[u][v] img[j-(u-ky/2)][i-(v-kx/2)], out-of-range terms dropped
  * (zero padding, 'same' size, true convolution -- kernel flipped relative to correlation).
  * image: device [ny][nx] (in).  kernel: device [ky][kx], ky and kx odd (in); used as given, never
- * renormalised.  out: device [ny][nx].  method: DIRECT = shared-memory tiled sum; FFT = zero-pad
- * to a power of two P >= n+K-1, hand-written shared-memory FFTs; AUTO picks the path a time model calibrated on B200 expects to be faster.
- * workspace: device scratch >= jt_psf_convolve_workspace_bytes(...) for the same arguments. */
+ * renormalised.  out: device [ny][nx].  method: DIRECT = register-blocked sum over a TMA-loaded shared-memory halo tile,
+ * taps fed from the constant bank through uniform registers, kernel rows split over a thread-block cluster; FFT =
+ * zero-pad to P >= n+K-1, hand-written shared-memory FFTs; AUTO picks the path a time model calibrated on B200 expects
+ * to be faster.  workspace: device scratch >= jt_psf_convolve_workspace_bytes(...) for the same arguments, 16-byte
+ * aligned.  Non-finite pixels may reach outputs up to one pixel beyond the kernel's support (0 x inf).
+ * DIRECT stages its taps in the library's one __constant__ buffer per device: calls on different streams are ordered
+ * by an event the library keeps for that purpose (not while a stream is being captured into a CUDA graph: graphs
+ * that contain DIRECT convolutions must not be replayed concurrently with other DIRECT calls). */
 JT_API size_t    jt_psf_convolve_workspace_bytes(jt_dtype dtype, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
                                           jt_conv_method method);
 JT_API jt_status jt_psf_convolve(jt_dtype dtype, int32_t ny, int32_t nx, const void *image,
                           int32_t ky, int32_t kx, const void *kernel, jt_conv_method method,
                           void *workspace, size_t workspace_bytes, void *out, void *stream);
+
+/* The same on B images with ONE kernel in one call (the batched form of the paper's convolution benchmark,
+ * PAPER.md:112-114; SURVEY.md section 8(d) D4 "batch B in {1, 1024} images").  images, out: device [B][ny][nx].
+ * DIRECT runs all images in one launch (B x tiles x row bands CTAs); FFT transforms them one after the other. */
+JT_API size_t    jt_psf_convolve_batch_workspace_bytes(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
+                                                jt_conv_method method);
+JT_API jt_status jt_psf_convolve_batch(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, const void *images,
+                                int32_t ky, int32_t kx, const void *kernel, jt_conv_method method,
+                                void *workspace, size_t workspace_bytes, void *out, void *stream);
 
 /* Steps 1-3 fused on one system: grid G generated in registers, ray-shoot, Sersic,
  * binning B (image[j][i] = pixel_scale^2/s^2 * sum of the pixel's s*s sub-ray brightnesses, reduced
@@ -158,16 +172,6 @@ JT_API jt_status jt_profile_read(float *trace_ms, float *conv_ms);
  * per-ray cold path.  The counters live in the call's workspace, which must still be allocated;
  * the call synchronises on the profiling events. */
 JT_API jt_status jt_profile_tiers(uint64_t *counts);
-
-/* Measurement aid: ALU peak microbenchmark (bench.py reports the measured rates beside the derived peaks of
- * DESIGN.md section 6; MEASURED_PEAKS.json covers only HBM and tensor cores).  Launches `blocks` CTAs of 256
- * threads, each thread running 8 independent chains of `kind` for iters * 4 rounds; *lane_ops (host, may be NULL)
- * receives the number of thread-level instructions of that kind the launch executes (an FFMA2 counts once but
- * performs two FMAs).  sink: device scratch of >= 4 bytes.  Time it with events on `stream`. */
-typedef enum { JT_PROBE_FFMA = 0, JT_PROBE_FFMA2 = 1, JT_PROBE_DFMA = 2, JT_PROBE_MUFU_RSQ = 3,
-               JT_PROBE_FFMA2_RF = 4, JT_PROBE_DFMA_RF = 5, /* FFMA2 / DFMA with the direct convolution's operand pattern */
-               JT_PROBE_FFMA2_LDS = 6 /* the same with one tap and one window shared-memory load per 8 FFMA2 */ } jt_probe_kind;
-JT_API jt_status jt_probe_alu(int32_t kind, int32_t blocks, int64_t iters, void *sink, int64_t *lane_ops, void *stream);
 
 /* Number of CUDA kernels this library has launched from the calling host thread since it was loaded
  * (bench.py's "gpu_launches" claim; memsets and event records are not counted). */

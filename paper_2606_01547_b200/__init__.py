@@ -11,10 +11,13 @@ from .binding import (  # noqa: F401
     kernel_launches,
     lib_path,
     probe_alu,
+    probe_lib_path,
     profile_enable,
     profile_read,
     profile_tiers,
     psf_convolve,
+    psf_convolve_batch,
+    psf_convolve_batch_workspace_bytes,
     psf_convolve_workspace_bytes,
     ray_shoot,
     ray_shoot_workspace_bytes,

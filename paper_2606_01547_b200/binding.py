@@ -93,6 +93,9 @@ def lib():
         L.jt_psf_convolve_workspace_bytes.restype = sz
         L.jt_psf_convolve_workspace_bytes.argtypes = [ctypes.c_int, i32, i32, i32, i32, ctypes.c_int]
         L.jt_psf_convolve.argtypes = [ctypes.c_int, i32, i32, vp, i32, i32, vp, ctypes.c_int, vp, sz, vp, vp]
+        L.jt_psf_convolve_batch_workspace_bytes.restype = sz
+        L.jt_psf_convolve_batch_workspace_bytes.argtypes = [ctypes.c_int, i64, i32, i32, i32, i32, ctypes.c_int]
+        L.jt_psf_convolve_batch.argtypes = [ctypes.c_int, i64, i32, i32, vp, i32, i32, vp, ctypes.c_int, vp, sz, vp, vp]
         L.jt_simulate_image_workspace_bytes.restype = sz
         L.jt_simulate_image_workspace_bytes.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), i64, i32, i32, ctypes.c_int]
         L.jt_simulate_image.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), ctypes.POINTER(_Lens),
@@ -102,7 +105,6 @@ def lib():
         L.jt_profile_enable.argtypes = [ctypes.c_int]
         L.jt_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
         L.jt_profile_tiers.argtypes = [ctypes.POINTER(ctypes.c_uint64)]
-        L.jt_probe_alu.argtypes = [i32, i32, i64, vp, ctypes.POINTER(i64), vp]
         _lib = L
     return _lib
 
@@ -135,12 +137,28 @@ def profile_tiers():
     return tuple(int(x) for x in c)
 
 
-PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3, "ffma2_rf": 4, "dfma_rf": 5, "ffma2_lds": 6}
+PROBE_KINDS = {"ffma": 0, "ffma2": 1, "dfma": 2, "mufu_rsq": 3}
+_probe_lib = None
+
+
+def probe_lib_path():
+    return os.path.join(_HERE, "libjtprobe.so")
+
+
+def _probe():
+    """libjtprobe.so (include/jt_probe.h): measurement aid, separate from the product library."""
+    global _probe_lib
+    if _probe_lib is None:
+        L = ctypes.CDLL(probe_lib_path())
+        L.jt_probe_alu.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int64, ctypes.c_void_p,
+                                   ctypes.POINTER(ctypes.c_int64), ctypes.c_void_p]
+        L.jt_probe_alu.restype = ctypes.c_int
+        _probe_lib = L
+    return _probe_lib
 
 
 def probe_alu(kind, blocks=148 * 8, iters=4096, repeats=3):
     """jt_probe_alu timed with CUDA events: returns thread-level instructions of `kind` per second (best of repeats)."""
-    import torch
     sink = torch.zeros(4, dtype=torch.float32, device="cuda")
     n = ctypes.c_int64()
     st = torch.cuda.current_stream()
@@ -148,8 +166,8 @@ def probe_alu(kind, blocks=148 * 8, iters=4096, repeats=3):
     for _ in range(repeats + 1):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(st)
-        _check(lib().jt_probe_alu(PROBE_KINDS[kind], blocks, iters, ctypes.c_void_p(sink.data_ptr()), ctypes.byref(n),
-                                  ctypes.c_void_p(st.cuda_stream)), "jt_probe_alu")
+        _check(_probe().jt_probe_alu(PROBE_KINDS[kind], blocks, iters, ctypes.c_void_p(sink.data_ptr()), ctypes.byref(n),
+                                     ctypes.c_void_p(st.cuda_stream)), "jt_probe_alu")
         b.record(st)
         b.synchronize()
         best = max(best, n.value / (a.elapsed_time(b) * 1e-3))
@@ -281,6 +299,27 @@ def psf_convolve(image, kernel, method="auto", workspace=None, out=None, stream=
         out = torch.empty_like(image)
     _check(lib().jt_psf_convolve(code, ny, nx, _ptr(image), ky, kx, _ptr(kernel), _METHODS[method], _ptr(ws), wsb,
                                  _ptr(out), _stream(stream)), "jt_psf_convolve")
+    return out
+
+
+def psf_convolve_batch_workspace_bytes(dtype, B, ny, nx, ky, kx, method="auto"):
+    return int(lib().jt_psf_convolve_batch_workspace_bytes(_code(dtype), B, ny, nx, ky, kx, _METHODS[method]))
+
+
+def psf_convolve_batch(images, kernel, method="auto", workspace=None, out=None, stream=None):
+    """jt_psf_convolve_batch: images [B][ny][nx], one kernel [ky][kx] for all of them."""
+    _dev(images, "images"), _dev(kernel, "kernel")
+    code = _dt(images)
+    if _dt(kernel) != code:
+        raise TypeError("images and kernel dtypes differ")
+    B, ny, nx = images.shape
+    ky, kx = kernel.shape
+    ws, wsb = _workspace(psf_convolve_batch_workspace_bytes(code, B, ny, nx, ky, kx, method) if B > 0 else 0,
+                         images.device, workspace)
+    if out is None:
+        out = torch.empty_like(images)
+    _check(lib().jt_psf_convolve_batch(code, B, ny, nx, _ptr(images), ky, kx, _ptr(kernel), _METHODS[method], _ptr(ws),
+                                       wsb, _ptr(out), _stream(stream)), "jt_psf_convolve_batch")
     return out
 
 

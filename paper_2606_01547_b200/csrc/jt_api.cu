@@ -42,23 +42,31 @@ static bool valid_lens(const jt_lens* l) {
 static bool valid_kernel_size(int ky, int kx) { return ky >= 1 && kx >= 1 && (ky & 1) && (kx & 1); }
 
 // AUTO: whichever of the two supported paths the calibrated time models expect to be faster.
-jt_conv_method resolve_conv_method(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method m) {
+jt_conv_method resolve_conv_method(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx, jt_conv_method m) {
     if (m == JT_CONV_DIRECT || m == JT_CONV_FFT) return m;
     if (!conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_CONV_FFT;
     if (!conv_fft_supported(dtype, ny, nx, ky, kx)) return JT_CONV_DIRECT;
-    return conv_fft_estimate_us(dtype, ny, nx, ky, kx) < conv_direct_estimate_us(dtype, ny, nx, ky, kx) ? JT_CONV_FFT : JT_CONV_DIRECT;
+    return (double)B * conv_fft_estimate_us(dtype, ny, nx, ky, kx) < conv_direct_estimate_us(dtype, B, ny, nx, ky, kx) ? JT_CONV_FFT
+                                                                                                                     : JT_CONV_DIRECT;
 }
 
-static size_t conv_ws(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method method) {
-    const jt_conv_method m = resolve_conv_method(dtype, ny, nx, ky, kx, method);
-    return m == JT_CONV_DIRECT ? conv_direct_workspace_bytes(dtype, ky, kx) : fft_conv_workspace_bytes(dtype, ny, nx, ky, kx);
+static size_t conv_ws(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx, jt_conv_method method) {
+    const jt_conv_method m = resolve_conv_method(dtype, B, ny, nx, ky, kx, method);
+    return m == JT_CONV_DIRECT ? conv_direct_workspace_bytes(dtype, B, ny, nx, ky, kx) : fft_conv_workspace_bytes(dtype, ny, nx, ky, kx);
 }
 
-static jt_status conv_dispatch(jt_dtype dtype, int ny, int nx, const void* image, int ky, int kx, const void* kernel,
+// B images [B][ny][nx] with one kernel.  The FFT path transforms the images one after the other (one plane of workspace).
+static jt_status conv_dispatch(jt_dtype dtype, int64_t B, int ny, int nx, const void* image, int ky, int kx, const void* kernel,
                                jt_conv_method method, void* workspace, void* out, cudaStream_t st) {
-    const jt_conv_method m = resolve_conv_method(dtype, ny, nx, ky, kx, method);
-    if (m == JT_CONV_DIRECT) return launch_conv_direct(dtype, ny, nx, image, ky, kx, kernel, workspace, out, st);
-    return launch_conv_fft(dtype, ny, nx, image, ky, kx, kernel, workspace, out, st);
+    const jt_conv_method m = resolve_conv_method(dtype, B, ny, nx, ky, kx, method);
+    if (m == JT_CONV_DIRECT) return launch_conv_direct(dtype, B, ny, nx, image, ky, kx, kernel, workspace, out, st);
+    const size_t img_bytes = (size_t)ny * nx * dtype_size(dtype);
+    for (int64_t b = 0; b < B; ++b) {
+        const jt_status s = launch_conv_fft(dtype, ny, nx, (const char*)image + b * img_bytes, ky, kx, kernel, workspace,
+                                            (char*)out + b * img_bytes, st);
+        if (s != JT_OK) return s;
+    }
+    return JT_OK;
 }
 
 }  // namespace jt
@@ -120,23 +128,42 @@ jt_status jt_source_brightness(jt_dtype dtype, int64_t n, const void* beta_x, co
 size_t jt_psf_convolve_workspace_bytes(jt_dtype dtype, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
                                        jt_conv_method method) {
     if (!valid_dtype(dtype) || !valid_method(method) || ny < 1 || nx < 1 || !valid_kernel_size(ky, kx)) return 0;
-    return conv_ws(dtype, ny, nx, ky, kx, method);
+    return conv_ws(dtype, 1, ny, nx, ky, kx, method);
+}
+
+static jt_status psf_convolve_impl(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, const void* image, int32_t ky, int32_t kx,
+                                   const void* kernel, jt_conv_method method, void* workspace, size_t workspace_bytes,
+                                   void* out, void* stream) {
+    if (!valid_dtype(dtype) || !valid_method(method)) return JT_ERR_UNSUPPORTED;
+    if (B < 0 || ny < 1 || nx < 1 || !valid_kernel_size(ky, kx)) return JT_ERR_INVALID_VALUE;
+    if (B == 0) return JT_OK;
+    if (!image || !kernel || !out || image == out) return JT_ERR_INVALID_VALUE;
+    if (method == JT_CONV_DIRECT && !conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_ERR_UNSUPPORTED;
+    if (resolve_conv_method(dtype, B, ny, nx, ky, kx, method) == JT_CONV_FFT && !conv_fft_supported(dtype, ny, nx, ky, kx))
+        return JT_ERR_UNSUPPORTED;
+    const size_t need = conv_ws(dtype, B, ny, nx, ky, kx, method);
+    if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return conv_dispatch(dtype, B, ny, nx, image, ky, kx, kernel, method, workspace, out, (cudaStream_t)stream);
 }
 
 jt_status jt_psf_convolve(jt_dtype dtype, int32_t ny, int32_t nx, const void* image, int32_t ky, int32_t kx,
                           const void* kernel, jt_conv_method method, void* workspace, size_t workspace_bytes, void* out,
                           void* stream) {
-    if (!valid_dtype(dtype) || !valid_method(method)) return JT_ERR_UNSUPPORTED;
-    if (ny < 1 || nx < 1 || !valid_kernel_size(ky, kx) || !image || !kernel || !out || image == out)
-        return JT_ERR_INVALID_VALUE;
-    if (method == JT_CONV_DIRECT && !conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_ERR_UNSUPPORTED;
-    if (resolve_conv_method(dtype, ny, nx, ky, kx, method) == JT_CONV_FFT && !conv_fft_supported(dtype, ny, nx, ky, kx))
-        return JT_ERR_UNSUPPORTED;
-    const size_t need = conv_ws(dtype, ny, nx, ky, kx, method);
-    if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
-    jt_status s = check_device();
-    if (s != JT_OK) return s;
-    return conv_dispatch(dtype, ny, nx, image, ky, kx, kernel, method, workspace, out, (cudaStream_t)stream);
+    return psf_convolve_impl(dtype, 1, ny, nx, image, ky, kx, kernel, method, workspace, workspace_bytes, out, stream);
+}
+
+size_t jt_psf_convolve_batch_workspace_bytes(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
+                                             jt_conv_method method) {
+    if (!valid_dtype(dtype) || !valid_method(method) || B < 1 || ny < 1 || nx < 1 || !valid_kernel_size(ky, kx)) return 0;
+    return conv_ws(dtype, B, ny, nx, ky, kx, method);
+}
+
+jt_status jt_psf_convolve_batch(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, const void* images, int32_t ky, int32_t kx,
+                                const void* kernel, jt_conv_method method, void* workspace, size_t workspace_bytes,
+                                void* out, void* stream) {
+    return psf_convolve_impl(dtype, B, ny, nx, images, ky, kx, kernel, method, workspace, workspace_bytes, out, stream);
 }
 
 // ------------------------------------------------------------------ fused image
@@ -149,7 +176,7 @@ size_t jt_simulate_image_workspace_bytes(jt_dtype dtype, const jt_grid* grid, in
     if (ky > 0 || kx > 0) {
         if (!valid_kernel_size(ky, kx)) return 0;
         total += align_up((size_t)grid->nx * grid->ny * dtype_size(dtype), 256);
-        total += conv_ws(dtype, grid->ny, grid->nx, ky, kx, method);
+        total += conv_ws(dtype, 1, grid->ny, grid->nx, ky, kx, method);
     }
     return total;
 }
@@ -165,7 +192,7 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
     const bool conv = !(ky == 0 && kx == 0 && kernel == nullptr);
     if (conv && (!valid_kernel_size(ky, kx) || !kernel)) return JT_ERR_INVALID_VALUE;
     if (conv && method == JT_CONV_DIRECT && !conv_direct_supported(dtype, grid->ny, grid->nx, ky, kx)) return JT_ERR_UNSUPPORTED;
-    if (conv && resolve_conv_method(dtype, grid->ny, grid->nx, ky, kx, method) == JT_CONV_FFT &&
+    if (conv && resolve_conv_method(dtype, 1, grid->ny, grid->nx, ky, kx, method) == JT_CONV_FFT &&
         !conv_fft_supported(dtype, grid->ny, grid->nx, ky, kx))
         return JT_ERR_UNSUPPORTED;
     const size_t need = jt_simulate_image_workspace_bytes(dtype, grid, lens->n_tnfw, conv ? ky : 0, conv ? kx : 0, method);
@@ -190,7 +217,7 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
     s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, pre, prof, st);
     if (s != JT_OK) return s;
     if (prof) JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st));
-    s = conv_dispatch(dtype, grid->ny, grid->nx, pre, ky, kx, kernel, method, conv_ws_ptr, out, st);
+    s = conv_dispatch(dtype, 1, grid->ny, grid->nx, pre, ky, kx, kernel, method, conv_ws_ptr, out, st);
     if (s == JT_OK && prof) { JT_CUDA_TRY(cudaEventRecord(g_prof.ev[2], st)); g_prof.had_conv = true; g_prof.recorded = true; }
     return s;
 }

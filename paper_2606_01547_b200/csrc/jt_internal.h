@@ -59,13 +59,13 @@ jt_status launch_source_brightness(jt_dtype dtype, int64_t n, const void* bx, co
                                    void* flux, cudaStream_t st);
 
 // ---- convolution (jt_conv.cu, jt_fft.cu) ----
-jt_conv_method resolve_conv_method(jt_dtype dtype, int ny, int nx, int ky, int kx, jt_conv_method m);
+jt_conv_method resolve_conv_method(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx, jt_conv_method m);
 bool      conv_direct_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
-size_t    conv_direct_workspace_bytes(jt_dtype dtype, int ky, int kx);
-double    conv_direct_estimate_us(jt_dtype dtype, int ny, int nx, int ky, int kx);
+size_t    conv_direct_workspace_bytes(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
+double    conv_direct_estimate_us(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
 double    conv_fft_estimate_us(jt_dtype dtype, int ny, int nx, int ky, int kx);
-jt_status launch_conv_direct(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
-                             void* workspace, void* out, cudaStream_t st);
+jt_status launch_conv_direct(jt_dtype dtype, int64_t B, int ny, int nx, const void* img, int ky, int kx, const void* ker,
+                             void* workspace, void* out, cudaStream_t st);   // B images [B][ny][nx], one kernel
 bool      conv_fft_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
 size_t    fft_conv_workspace_bytes(jt_dtype dtype, int ny, int nx, int ky, int kx);
 jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,

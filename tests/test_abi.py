@@ -7,20 +7,28 @@ import re
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+JT_VERSION_EXPECTED = 200
 
 
-def _declared():
-    src = open(os.path.join(ROOT, "include", "jt.h")).read()
-    return sorted(set(re.findall(r"JT_API[^;(]*?\b(jt_[a-z_]+)\s*\(", src)))
+def _declared(header, macro):
+    src = open(os.path.join(ROOT, "include", header)).read()
+    return sorted(set(re.findall(macro + r"[^;(]*?\b(jt_[a-z_0-9]+)\s*\(", src)))
 
 
 def test_header_symbols_exported(jt):
-    names = _declared()
-    assert len(names) == 16, names
+    """Every function include/*.h declares is exported by the library that header describes."""
+    assert sorted(f for f in os.listdir(os.path.join(ROOT, "include")) if f.endswith(".h")) == ["jt.h", "jt_probe.h"]
+    names = _declared("jt.h", "JT_API")
+    assert {"jt_ray_shoot", "jt_source_brightness", "jt_psf_convolve", "jt_simulate_image", "jt_simulate_batch",
+            "jt_psf_convolve_batch"} <= set(names), names
     L = ctypes.CDLL(jt.lib_path())
     for n in names:
         assert hasattr(L, n), n
-    assert jt.version() == 100
+    assert not hasattr(L, "jt_probe_alu")              # measurement probes live in their own library
+    P = ctypes.CDLL(jt.probe_lib_path())
+    assert _declared("jt_probe.h", "JT_PROBE_API") == ["jt_probe_alu"]
+    assert hasattr(P, "jt_probe_alu")
+    assert jt.version() == JT_VERSION_EXPECTED
 
 
 def test_status_strings(jt):
@@ -50,8 +58,15 @@ def test_argument_validation_without_device(jt):
     assert L.jt_ray_shoot(1, 10, dummy, dummy, ctypes.byref(lens), None, 0, ctypes.c_void_p(512), ctypes.c_void_p(768), None) == 1
     lens.n_tnfw = 0
     assert L.jt_ray_shoot(1, -1, dummy, dummy, ctypes.byref(lens), None, 0, ctypes.c_void_p(512), ctypes.c_void_p(768), None) == 1
-    # workspace too small: the FFT path needs its complex plane (the direct path needs none)
-    assert L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 1) == 0
+    # workspace too small: the direct path needs its tap table (+ partial sums when the kernel columns are split over
+    # CTAs), the FFT path its complex plane
+    L.jt_psf_convolve_batch_workspace_bytes.restype = ctypes.c_size_t
+    need = L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 1)
+    assert need >= 21 * 21 * 8
+    assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 1, dummy, need - 1, ctypes.c_void_p(512), None) == 3
+    assert L.jt_psf_convolve_batch_workspace_bytes(1, ctypes.c_int64(1), 64, 64, 21, 21, 1) == need
+    assert L.jt_psf_convolve_batch(1, ctypes.c_int64(0), 64, 64, None, 21, 21, None, 1, None, 0, None, None) == 0     # B = 0: no-op
+    assert L.jt_psf_convolve_batch(1, ctypes.c_int64(-1), 64, 64, dummy, 21, 21, dummy, 1, None, 0, ctypes.c_void_p(512), None) == 1
     need = L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 2)
     assert need >= 128 * 128 * 16
     assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 2, dummy, need - 1, ctypes.c_void_p(512), None) == 3
