@@ -1,361 +1,402 @@
 // jt_fft.cu -- step 5b: PSF convolution by hand-written shared-memory FFTs (definition P; PAPER.md:110-114
 // "FFT convolution").  Reaches the direct-convolution result up to rounding.  cuFFT is not used (tests only).
 //
-// Both inputs are real, so ONE complex transform carries both: z = img + i ker (zero-padded to Py x Px, powers of
-// two >= n + K - 1), Z = FFT2(z);  A = FFT2(img) = (Z(k) + conj Z(-k))/2,  B = FFT2(ker) = (Z(k) - conj Z(-k))/(2i);
-// C = A B is Hermitian, out = Re IFFT2(C) cropped at (ky/2, kx/2).
+// out = crop( IFFT2( FFT2(img) . FFT2(ker) ) ), both zero-padded to Py x Px, the smallest 2^a 3^b 5^c sizes
+// >= n + K - 1 (Px even): C4 pads 600 x 600, not 1024 x 1024.
 //
-// Forward transforms are decimation-in-frequency (natural order in, bit-reversed positions out; two radix-2 stages
-// fused per shared-memory pass), inverse
-// transforms decimation-in-time with conjugate twiddles (bit-reversed positions in, natural order out), so no
-// permutation pass exists anywhere: position p of an axis holds frequency brev(p), and the pointwise step pairs
-// position (py, px) with (brev(-brev py), brev(-brev px)).
+// Real input, so only the Px/2 + 1 non-redundant columns of the row spectra exist anywhere:
+//   k_fft_rows_fwd : two REAL rows of the same array ride one complex transform, z = row_a + i row_b ->
+//                    A_k = (Z_k + conj Z_{P-k})/2, B_k = (Z_k - conj Z_{P-k})/(2i); image rows -> plane SA [ny][Ph],
+//                    kernel rows -> plane SB [ky][Ph]  (Ph = Px/2 + 1; rows of zeros are never transformed)
+//   k_fft_cols     : a CTA owns a few spectrum columns: column FFTs of SA and SB (zero-padded to Py), pointwise
+//                    product with the 1/(Px Py) scale, inverse column FFT, all in shared memory; stores only the ny
+//                    rows the crop keeps -> plane SC [ny][Ph]
+//   k_fft_rows_inv : two output rows ride one inverse complex transform (Z_k = C_a,k + i C_b,k, Hermitian-extended),
+//                    real part -> row a, imaginary part -> row b, cropped at kx/2
+// Three launches on the caller's stream; the two later ones are programmatic dependent launches whose twiddle set-up
+// overlaps the previous kernel's tail.  The planes (C4: 5.3 MB) live in the caller's workspace and stay in L2.
 //
-// Four launches on the caller's stream, one complex plane [Py][Px] in the caller's workspace (L2-resident):
-//   k_fft_sums     : sum|img|, sum|ker| partial sums (scale balance of the packed transform, see below)
-//   k_fft_rows_fwd : pack img + i ker, row FFTs; only the max(ny, ky) non-zero rows are computed and stored
-//   k_fft_cols     : a CTA owns a group of adjacent position-columns and the group holding their -kx partners:
-//                    column FFTs, pointwise product (both members of a +-k pair at once), inverse column FFTs,
-//                    all in shared memory; stores only the ny rows the crop keeps
-//   k_fft_rows_inv : inverse row FFTs of those rows, crop, real part -> out
+// The transforms are Stockham autosort FFTs (natural order in and out, ping-pong between two shared-memory buffers,
+// no bit reversal), mixed radix 4 / 2 / 3 / 5 with the butterflies in registers; a thread reads its R inputs at
+// stride N/R (conflict-free) and one table twiddle per output.  All arithmetic is double in BOTH dtype modes (float
+// converts on load and store only): the FP64 pipe is nowhere near the limit here, L2 traffic and launch latency are.
 #include "jt_internal.h"
 
 namespace jt {
 
-// Packing the two real inputs into one complex transform couples their spectra: B is recovered with an absolute
-// error of eps |A|, i.e. eps sum|img| / sum|ker| relative.  Two measures keep that at rounding level:
-//   (1) the kernel is packed as lambda ker with lambda = the power of two nearest sum|img| / sum|ker| (k_fft_sums
-//       writes per-CTA partial sums, every later CTA adds them in the same order: deterministic, no atomics);
-//   (2) the transforms run in double in BOTH dtype modes (JT_F32 converts on load and store only).
-// The path is bound by launch latency and L2 traffic, not by the FP64 pipe.
 using Cd = double2;
-constexpr int kFftSumCtas = 64;        // partial sums: [2][kFftSumCtas] doubles behind the plane
-
-constexpr int kFftRowThreads = 256;
-constexpr int kFftColThreads = 512;
+constexpr int kFftThreads = 256;
+constexpr int kFftMaxP = 2048;                 // two ping-pong buffers + the twiddle table of one transform fit 227 KB
+constexpr int kFftMaxPasses = 12;
 constexpr size_t kFftMaxSmem = 220 * 1024;
 
-__host__ __device__ inline int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
-static int next_pow2(int v, int lo) { int p = lo; while (p < v) p <<= 1; return p; }
-
+__device__ __forceinline__ Cd cadd(Cd a, Cd b) { return {a.x + b.x, a.y + b.y}; }
+__device__ __forceinline__ Cd csub(Cd a, Cd b) { return {a.x - b.x, a.y - b.y}; }
 __device__ __forceinline__ Cd cmul(Cd a, Cd b) { return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x}; }
 __device__ __forceinline__ Cd cmul_conj(Cd a, Cd b) { return {a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y}; }  // a conj(b)
+// multiply by SIGN * i  (forward transforms use exp(-i...): SIGN = -1)
+template <int SIGN> __device__ __forceinline__ Cd mul_i(Cd a) { return SIGN < 0 ? Cd{a.y, -a.x} : Cd{-a.y, a.x}; }
 
-__device__ __forceinline__ int brev_bits(int v, int bits) { return (int)(__brev((unsigned)v) >> (32 - bits)); }
+// length-R DFT in registers, c_k = sum_j a_j exp(SIGN 2 pi i j k / R)
+template <int R, int SIGN> struct Dft;
+template <int SIGN> struct Dft<2, SIGN> {
+    static __device__ __forceinline__ void run(Cd (&a)[2]) {
+        const Cd t = a[0];
+        a[0] = cadd(t, a[1]);
+        a[1] = csub(t, a[1]);
+    }
+};
+template <int SIGN> struct Dft<4, SIGN> {
+    static __device__ __forceinline__ void run(Cd (&a)[4]) {
+        const Cd t0 = cadd(a[0], a[2]), t1 = csub(a[0], a[2]), t2 = cadd(a[1], a[3]), t3 = mul_i<SIGN>(csub(a[1], a[3]));
+        a[0] = cadd(t0, t2);
+        a[1] = cadd(t1, t3);
+        a[2] = csub(t0, t2);
+        a[3] = csub(t1, t3);
+    }
+};
+template <int SIGN> struct Dft<3, SIGN> {
+    static __device__ __forceinline__ void run(Cd (&a)[3]) {
+        const double s3 = SIGN * 0.86602540378443864676372317075294;      // sin(2 pi / 3)
+        const Cd s = cadd(a[1], a[2]), d = csub(a[1], a[2]);
+        const Cd m = {a[0].x - 0.5 * s.x, a[0].y - 0.5 * s.y};
+        const Cd n = {-s3 * d.y, s3 * d.x};                               // i sin d
+        a[0] = cadd(a[0], s);
+        a[1] = cadd(m, n);
+        a[2] = csub(m, n);
+    }
+};
+template <int SIGN> struct Dft<5, SIGN> {
+    static __device__ __forceinline__ void run(Cd (&a)[5]) {
+        const double c1 = 0.30901699437494742410229341718282, c2 = -0.80901699437494742410229341718282;   // cos(2 pi/5), cos(4 pi/5)
+        const double s1 = SIGN * 0.95105651629515357211643933337938, s2 = SIGN * 0.58778525229247312916870595463907;
+        const Cd p1 = cadd(a[1], a[4]), d1 = csub(a[1], a[4]), p2 = cadd(a[2], a[3]), d2 = csub(a[2], a[3]);
+        const Cd m1 = {a[0].x + c1 * p1.x + c2 * p2.x, a[0].y + c1 * p1.y + c2 * p2.y};
+        const Cd m2 = {a[0].x + c2 * p1.x + c1 * p2.x, a[0].y + c2 * p1.y + c1 * p2.y};
+        const Cd u1 = {s1 * d1.x + s2 * d2.x, s1 * d1.y + s2 * d2.y};     // sin1 d1 + sin2 d2
+        const Cd u2 = {s2 * d1.x - s1 * d2.x, s2 * d1.y - s1 * d2.y};     // sin2 d1 - sin1 d2
+        const Cd n1 = {-u1.y, u1.x}, n2 = {-u2.y, u2.x};                  // times i
+        a[0] = {a[0].x + p1.x + p2.x, a[0].y + p1.y + p2.y};
+        a[1] = cadd(m1, n1);
+        a[4] = csub(m1, n1);
+        a[2] = cadd(m2, n2);
+        a[3] = csub(m2, n2);
+    }
+};
 
-// tw[m] = exp(-2 pi i m / n), m < n/2, from sincospi in double (m/n is exact for a power of two)
-__device__ __forceinline__ void make_twiddles(Cd* tw, int n, int tid, int nthr) {
-    for (int m = tid; m < n / 2; m += nthr) {
+// tw[j] = exp(-2 pi i j / N), j < N (sincospi in double)
+__device__ __forceinline__ void make_twiddles(Cd* tw, int N, int tid, int nthr) {
+    for (int j = tid; j < N; j += nthr) {
         double s, c;
-        sincospi(-2.0 * (double)m / (double)n, &s, &c);
-        tw[m] = {c, s};
+        sincospi(-2.0 * (double)j / (double)N, &s, &c);
+        tw[j] = {c, s};
     }
 }
 
-// nb transforms of length n = 2^logn at s + b * pitch.  Forward, decimation in frequency.  Two radix-2 stages are
-// fused per pass (a thread carries four points through both in registers: half the shared-memory traffic and half the
-// barriers of a stage-by-stage sweep, identical arithmetic); an odd logn ends with one plain radix-2 stage.
-__device__ __forceinline__ void fft_dif(Cd* s, const Cd* tw, int logn, int nb, int pitch, int tid, int nthr) {
-    int lh = logn - 1;
-    for (; lh >= 1; lh -= 2) {                       // stages with half-sizes h = 2^lh and q = h/2
-        const int h = 1 << lh, q = h >> 1;
-        const int quarter = 1 << (logn - 2);
-        const int total = nb * quarter;
-        for (int u = tid; u < total; u += nthr) {
-            const int tr = u >> (logn - 2), uu = u & (quarter - 1);
-            const int k = uu & (q - 1), g = uu >> (lh - 1);
-            const int i0 = tr * pitch + (g << (lh + 1)) + k, i1 = i0 + q, i2 = i0 + h, i3 = i2 + q;
-            const Cd x0 = s[i0], x1 = s[i1], x2 = s[i2], x3 = s[i3];
-            const Cd wa = tw[k << (logn - 1 - lh)], wb = tw[(k + q) << (logn - 1 - lh)], wc = tw[k << (logn - lh)];
-            const Cd a0 = {x0.x + x2.x, x0.y + x2.y};
-            const Cd a2 = cmul({x0.x - x2.x, x0.y - x2.y}, wa);
-            const Cd a1 = {x1.x + x3.x, x1.y + x3.y};
-            const Cd a3 = cmul({x1.x - x3.x, x1.y - x3.y}, wb);
-            s[i0] = {a0.x + a1.x, a0.y + a1.y};
-            s[i1] = cmul({a0.x - a1.x, a0.y - a1.y}, wc);
-            s[i2] = {a2.x + a3.x, a2.y + a3.y};
-            s[i3] = cmul({a2.x - a3.x, a2.y - a3.y}, wc);
-        }
-        __syncthreads();
-    }
-    if (lh == 0) {                                   // last stage, h = 1, twiddle 1
-        const int half = 1 << (logn - 1);
-        const int total = nb * half;
-        for (int b = tid; b < total; b += nthr) {
-            const int tr = b >> (logn - 1), bb = b & (half - 1);
-            const int i = tr * pitch + (bb << 1), j = i + 1;
-            const Cd a = s[i], c = s[j];
-            s[i] = {a.x + c.x, a.y + c.y};
-            s[j] = cmul({a.x - c.x, a.y - c.y}, tw[0]);
-        }
-        __syncthreads();
+// One Stockham pass of radix R over `nbatch` transforms of length N (x -> y, transform b at offset b * pitch):
+// current sub-length n (N = n s), butterfly t = p s + q reads x[t + j N/R], writes y[q + s (R p + k)] * w_n^{p k}.
+template <int R, int SIGN>
+__device__ __forceinline__ void stockham_pass(const Cd* __restrict__ x, Cd* __restrict__ y, const Cd* __restrict__ tw, int N,
+                                              int s, int nbatch, int pitch, int tid, int nthr) {
+    const int nb = N / R;
+    const int total = nbatch * nb;
+    for (int u = tid; u < total; u += nthr) {
+        const int b = u / nb, t = u - b * nb;
+        const int p = t / s, q = t - p * s;
+        const Cd* xb = x + (size_t)b * pitch + t;
+        Cd a[R];
+#pragma unroll
+        for (int j = 0; j < R; ++j) a[j] = xb[j * nb];
+        Dft<R, SIGN>::run(a);
+        const int ps = p * s;                                  // twiddle index step: w_n^{p k} = tw[p s k], p s k < N
+        Cd* yb = y + (size_t)b * pitch + q + s * R * p;
+        yb[0] = a[0];
+#pragma unroll
+        for (int k = 1; k < R; ++k) yb[s * k] = SIGN < 0 ? cmul(a[k], tw[ps * k]) : cmul_conj(a[k], tw[ps * k]);
     }
 }
 
-// Inverse of fft_dif stage by stage (unnormalised: fft_dit_inv(fft_dif(x)) = n x), the stages fused in pairs likewise.
-__device__ __forceinline__ void fft_dit_inv(Cd* s, const Cd* tw, int logn, int nb, int pitch, int tid, int nthr) {
-    int lh = 0;
-    if (logn & 1) {                                  // undo fft_dif's last stage first (h = 1)
-        const int half = 1 << (logn - 1);
-        const int total = nb * half;
-        for (int b = tid; b < total; b += nthr) {
-            const int tr = b >> (logn - 1), bb = b & (half - 1);
-            const int i = tr * pitch + (bb << 1), j = i + 1;
-            const Cd a = s[i];
-            const Cd c = cmul_conj(s[j], tw[0]);
-            s[i] = {a.x + c.x, a.y + c.y};
-            s[j] = {a.x - c.x, a.y - c.y};
+struct Radices { int n; int r[kFftMaxPasses]; };
+
+// nbatch transforms of length N; input in x, scratch y; returns the buffer that holds the result.
+template <int SIGN>
+__device__ __forceinline__ Cd* stockham(Cd* x, Cd* y, const Cd* tw, int N, const Radices& rad, int nbatch, int pitch, int tid,
+                                        int nthr) {
+    int s = 1;
+    for (int i = 0; i < rad.n; ++i) {
+        const int R = rad.r[i];
+        switch (R) {
+            case 4: stockham_pass<4, SIGN>(x, y, tw, N, s, nbatch, pitch, tid, nthr); break;
+            case 2: stockham_pass<2, SIGN>(x, y, tw, N, s, nbatch, pitch, tid, nthr); break;
+            case 3: stockham_pass<3, SIGN>(x, y, tw, N, s, nbatch, pitch, tid, nthr); break;
+            default: stockham_pass<5, SIGN>(x, y, tw, N, s, nbatch, pitch, tid, nthr); break;
         }
         __syncthreads();
-        lh = 1;
+        s *= R;
+        Cd* t = x; x = y; y = t;
     }
-    for (; lh + 1 < logn; lh += 2) {                 // stages with half-sizes h = 2^lh and 2h
-        const int h = 1 << lh;
-        const int quarter = 1 << (logn - 2);
-        const int total = nb * quarter;
-        for (int u = tid; u < total; u += nthr) {
-            const int tr = u >> (logn - 2), uu = u & (quarter - 1);
-            const int k = uu & (h - 1), g = uu >> lh;
-            const int i0 = tr * pitch + (g << (lh + 2)) + k, i1 = i0 + h, i2 = i1 + h, i3 = i2 + h;
-            const Cd x0 = s[i0], x2 = s[i2];
-            const Cd w1 = tw[k << (logn - 1 - lh)];
-            const Cd c1 = cmul_conj(s[i1], w1), c3 = cmul_conj(s[i3], w1);
-            const Cd b0 = {x0.x + c1.x, x0.y + c1.y}, b1 = {x0.x - c1.x, x0.y - c1.y};
-            const Cd b2 = {x2.x + c3.x, x2.y + c3.y}, b3 = {x2.x - c3.x, x2.y - c3.y};
-            const Cd d2 = cmul_conj(b2, tw[k << (logn - 2 - lh)]);
-            const Cd d3 = cmul_conj(b3, tw[(k + h) << (logn - 2 - lh)]);
-            s[i0] = {b0.x + d2.x, b0.y + d2.y};
-            s[i2] = {b0.x - d2.x, b0.y - d2.y};
-            s[i1] = {b1.x + d3.x, b1.y + d3.y};
-            s[i3] = {b1.x - d3.x, b1.y - d3.y};
-        }
-        __syncthreads();
-    }
+    return x;
 }
 
-// partial[c] = sum |img| over CTA c's slice, partial[kFftSumCtas + c] = the same for ker
+struct FftArgs {
+    int ny, nx, ky, kx;
+    int Px, Py, Ph;                  // padded sizes, Ph = Px/2 + 1 stored spectrum columns
+    int nb;                          // row pairs per CTA (row kernels)
+    int tc;                          // spectrum columns per CTA (column kernel)
+    int n_cta_img;                   // rows_fwd: CTAs that transform image row pairs (the rest take kernel rows)
+    Radices rx, ry;
+    double scale;                    // 1 / (Px Py)
+    Cd *SA, *SB, *SC;                // planes [ny][Ph], [ky][Ph], [ny][Ph]
+};
+
+// ---- rows forward: pairs of real rows -> half spectra ----
 template <typename T>
-__global__ void __launch_bounds__(256) k_fft_sums(int64_t n_img, const T* __restrict__ img, int64_t n_ker,
-                                                  const T* __restrict__ ker, double* __restrict__ partial) {
-    __shared__ double red[2][8];
-    double a = 0.0, b = 0.0;
-    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n_img; i += (int64_t)gridDim.x * 256) a += fabs((double)__ldg(&img[i]));
-    for (int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x; i < n_ker; i += (int64_t)gridDim.x * 256) b += fabs((double)__ldg(&ker[i]));
-    for (int o = 16; o > 0; o >>= 1) { a += __shfl_xor_sync(0xffffffffu, a, o); b += __shfl_xor_sync(0xffffffffu, b, o); }
-    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = a; red[1][threadIdx.x >> 5] = b; }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double sa = 0.0, sb = 0.0;
-        for (int w = 0; w < 8; ++w) { sa += red[0][w]; sb += red[1][w]; }
-        partial[blockIdx.x] = sa;
-        partial[kFftSumCtas + blockIdx.x] = sb;
-    }
-}
-
-// lambda = 2^round(log2(sum|img| / sum|ker|)), 1 when either sum is zero or not finite
-__device__ __forceinline__ double fft_lambda(const double* __restrict__ partial, int n_part) {
-    double sa = 0.0, sb = 0.0;
-    for (int c = 0; c < n_part; ++c) { sa += partial[c]; sb += partial[kFftSumCtas + c]; }
-    if (!(sa > 0.0) || !(sb > 0.0) || !isfinite(sa) || !isfinite(sb)) return 1.0;
-    int ea, eb;
-    frexp(sa, &ea);
-    frexp(sb, &eb);
-    int d = ea - eb;
-    d = d > 1000 ? 1000 : (d < -1000 ? -1000 : d);
-    return ldexp(1.0, d);
-}
-
-template <typename T>
-__global__ void __launch_bounds__(kFftRowThreads) k_fft_rows_fwd(int ny, int nx, const T* __restrict__ img, int ky, int kx,
-                                                                 const T* __restrict__ ker, int logPx, int rows_nz, int nb,
-                                                                 const double* __restrict__ partial, int n_part,
-                                                                 Cd* __restrict__ plane) {
+__global__ void __launch_bounds__(kFftThreads) k_fft_rows_fwd(const __grid_constant__ FftArgs a, const T* __restrict__ img,
+                                                              const T* __restrict__ ker) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Px = 1 << logPx;
-    Cd* s = reinterpret_cast<Cd*>(smem_raw);
-    Cd* tw = s + (size_t)nb * Px;
-    const int tid = threadIdx.x;
-    make_twiddles(tw, Px, tid, kFftRowThreads);
-    const double lambda = fft_lambda(partial, n_part);
-    const int r0 = blockIdx.x * nb;
-    for (int idx = tid; idx < nb * Px; idx += kFftRowThreads) {
-        const int r = r0 + (idx >> logPx), x = idx & (Px - 1);
-        const T re = (r < ny && x < nx) ? __ldg(&img[(size_t)r * nx + x]) : (T)0;
-        const T im = (r < ky && x < kx) ? __ldg(&ker[(size_t)r * kx + x]) : (T)0;
-        s[idx] = {(double)re, lambda * (double)im};
-    }
-    __syncthreads();
-    fft_dif(s, tw, logPx, nb, Px, tid, kFftRowThreads);
-    for (int idx = tid; idx < nb * Px; idx += kFftRowThreads) {
-        const int r = r0 + (idx >> logPx);
-        if (r < rows_nz) plane[(size_t)r * Px + (idx & (Px - 1))] = s[idx];
-    }
-}
-
-// tb = log2(columns per group).  CTA kc in [0, Px/(2 TC)] owns the position group whose bit-reversed index is kc and
-// the group holding its -kx partners (the same group when kc = 0 or kc = Px/(2 TC)).
-__global__ void __launch_bounds__(kFftColThreads) k_fft_cols(int logPx, int logPy, int tb, int rows_nz, int row_out0,
-                                                             int n_rows_out, double scale, const double* __restrict__ partial,
-                                                             int n_part, Cd* __restrict__ plane) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Px = 1 << logPx, Py = 1 << logPy, TC = 1 << tb;
-    const int pitch = Py + 1;                      // odd pitch: the TC columns of one row land in different banks
-    const int gbits = logPx - tb;                  // bits of a group index
-    const int kc = blockIdx.x;
-    const int n_groups = 1 << gbits;
-    const int kcp = (n_groups - kc) & (n_groups - 1);
-    const bool self = (kcp == kc);
-    const int cA = gbits > 0 ? brev_bits(kc, gbits) : 0;
-    const int cB = gbits > 0 ? brev_bits(kcp, gbits) : 0;
-    const int ncol = self ? TC : 2 * TC;
-    const int lcol = self ? tb : tb + 1;
-    Cd* s = reinterpret_cast<Cd*>(smem_raw);
-    Cd* tw = s + (size_t)2 * TC * pitch;
-    const int tid = threadIdx.x;
-    make_twiddles(tw, Py, tid, kFftColThreads);
-    scale /= fft_lambda(partial, n_part);          // exact: lambda is a power of two
-
-    for (int idx = tid; idx < (Py << lcol); idx += kFftColThreads) {
-        const int r = idx >> lcol, lc = idx & (ncol - 1);
-        const int px = (lc < TC ? cA : cB) * TC + (lc & (TC - 1));
+    const int P = a.Px, tid = threadIdx.x;
+    Cd* x = reinterpret_cast<Cd*>(smem_raw);
+    Cd* y = x + (size_t)a.nb * P;
+    Cd* tw = y + (size_t)a.nb * P;
+    cudaTriggerProgrammaticLaunchCompletion();                 // lets k_fft_cols start its twiddle set-up once every CTA here runs
+    make_twiddles(tw, P, tid, kFftThreads);
+    const bool is_img = (int)blockIdx.x < a.n_cta_img;
+    const T* src = is_img ? img : ker;
+    const int rows = is_img ? a.ny : a.ky, width = is_img ? a.nx : a.kx;
+    Cd* plane = is_img ? a.SA : a.SB;
+    const int pair0 = (is_img ? (int)blockIdx.x : (int)blockIdx.x - a.n_cta_img) * a.nb;
+    for (int idx = tid; idx < a.nb * P; idx += kFftThreads) {
+        const int b = idx / P, i = idx - b * P;
+        const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
         Cd v = {0.0, 0.0};
-        if (r < rows_nz) v = plane[(size_t)r * Px + px];
-        s[lc * pitch + r] = v;
-    }
-    __syncthreads();
-    fft_dif(s, tw, logPy, ncol, pitch, tid, kFftColThreads);
-
-    // pointwise product; the thread that owns the smaller linear index of a (+k, -k) pair writes both members
-    for (int idx = tid; idx < (Py << lcol); idx += kFftColThreads) {
-        const int lc = idx >> logPy, py = idx & (Py - 1);
-        const int px = (lc < TC ? cA : cB) * TC + (lc & (TC - 1));
-        const int pxp = brev_bits((Px - brev_bits(px, logPx)) & (Px - 1), logPx);
-        const int pyp = brev_bits((Py - brev_bits(py, logPy)) & (Py - 1), logPy);
-        const int lcp = ((pxp >> tb) == cA ? 0 : TC) + (pxp & (TC - 1));
-        const int id = lc * pitch + py, idp = lcp * pitch + pyp;
-        if (id <= idp) {
-            const Cd z = s[id], zp = s[idp];
-            const Cd A = {0.5 * (z.x + zp.x), 0.5 * (z.y - zp.y)};      // (Z + conj Z')/2
-            const Cd Bk = {0.5 * (z.y + zp.y), -0.5 * (z.x - zp.x)};    // (Z - conj Z')/(2i)
-            Cd c = cmul(A, Bk);
-            c.x *= scale; c.y *= scale;
-            s[id] = c;
-            s[idp] = {c.x, -c.y};
+        if (i < width) {
+            if (r0 < rows) v.x = (double)__ldg(&src[(size_t)r0 * width + i]);
+            if (r1 < rows) v.y = (double)__ldg(&src[(size_t)r1 * width + i]);
         }
+        x[idx] = v;
     }
     __syncthreads();
-    fft_dit_inv(s, tw, logPy, ncol, pitch, tid, kFftColThreads);
-
-    for (int idx = tid; idx < (n_rows_out << lcol); idx += kFftColThreads) {
-        const int r = row_out0 + (idx >> lcol), lc = idx & (ncol - 1);
-        const int px = (lc < TC ? cA : cB) * TC + (lc & (TC - 1));
-        plane[(size_t)r * Px + px] = s[lc * pitch + r];
+    const Cd* X = stockham<-1>(x, y, tw, P, a.rx, a.nb, P, tid, kFftThreads);
+    for (int idx = tid; idx < a.nb * a.Ph; idx += kFftThreads) {
+        const int b = idx / a.Ph, k = idx - b * a.Ph;
+        const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
+        if (r0 >= rows) continue;
+        const Cd z = X[b * P + k], zn = X[b * P + (k == 0 ? 0 : P - k)];
+        plane[(size_t)r0 * a.Ph + k] = {0.5 * (z.x + zn.x), 0.5 * (z.y - zn.y)};                 // (Z_k + conj Z_{P-k}) / 2
+        if (r1 < rows) plane[(size_t)r1 * a.Ph + k] = {0.5 * (z.y + zn.y), -0.5 * (z.x - zn.x)}; // (Z_k - conj Z_{P-k}) / (2i)
     }
 }
 
-template <typename T>
-__global__ void __launch_bounds__(kFftRowThreads) k_fft_rows_inv(int ny, int nx, int logPx, int row_out0, int col_out0,
-                                                                 int nb, const Cd* __restrict__ plane, T* __restrict__ out) {
+// ---- columns: forward FFTs of tc image and tc kernel spectrum columns, product, inverse FFT, crop ----
+__global__ void __launch_bounds__(kFftThreads) k_fft_cols(const __grid_constant__ FftArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int Px = 1 << logPx;
-    Cd* s = reinterpret_cast<Cd*>(smem_raw);
-    Cd* tw = s + (size_t)nb * Px;
-    const int tid = threadIdx.x;
-    make_twiddles(tw, Px, tid, kFftRowThreads);
-    const int j0 = blockIdx.x * nb;
-    for (int idx = tid; idx < nb * Px; idx += kFftRowThreads) {
-        const int j = j0 + (idx >> logPx);
-        Cd v = {0.0, 0.0};
-        if (j < ny) v = plane[(size_t)(row_out0 + j) * Px + (idx & (Px - 1))];
-        s[idx] = v;
+    const int P = a.Py, tc = a.tc, tid = threadIdx.x;
+    Cd* x = reinterpret_cast<Cd*>(smem_raw);                   // [2 tc][P]: image columns, then kernel columns
+    Cd* y = x + (size_t)2 * tc * P;
+    Cd* tw = y + (size_t)2 * tc * P;
+    make_twiddles(tw, P, tid, kFftThreads);
+    cudaGridDependencySynchronize();                           // the planes SA, SB of k_fft_rows_fwd are complete
+    cudaTriggerProgrammaticLaunchCompletion();
+    const int k0 = blockIdx.x * tc;
+    const int ncol = min(tc, a.Ph - k0);
+    for (int idx = tid; idx < P * tc; idx += kFftThreads) {
+        const int r = idx / tc, c = idx - r * tc;
+        Cd va = {0.0, 0.0}, vb = {0.0, 0.0};
+        if (c < ncol) {
+            if (r < a.ny) va = __ldcg(&a.SA[(size_t)r * a.Ph + k0 + c]);
+            if (r < a.ky) vb = __ldcg(&a.SB[(size_t)r * a.Ph + k0 + c]);
+        }
+        x[c * P + r] = va;
+        x[(tc + c) * P + r] = vb;
     }
     __syncthreads();
-    fft_dit_inv(s, tw, logPx, nb, Px, tid, kFftRowThreads);
-    for (int idx = tid; idx < nb * nx; idx += kFftRowThreads) {
-        const int b = idx / nx, i = idx - b * nx;
-        const int j = j0 + b;
-        if (j < ny) out[(size_t)j * nx + i] = (T)s[b * Px + col_out0 + i].x;
+    Cd* X = stockham<-1>(x, y, tw, P, a.ry, 2 * tc, P, tid, kFftThreads);
+    Cd* Y = (X == x) ? y : x;
+    for (int idx = tid; idx < tc * P; idx += kFftThreads) {
+        Cd c = cmul(X[idx], X[tc * P + idx]);
+        c.x *= a.scale;
+        c.y *= a.scale;
+        X[idx] = c;
     }
+    __syncthreads();
+    const Cd* C = stockham<+1>(X, Y, tw, P, a.ry, tc, P, tid, kFftThreads);
+    const int row0 = a.ky / 2;
+    for (int idx = tid; idx < a.ny * tc; idx += kFftThreads) {
+        const int j = idx / tc, c = idx - j * tc;
+        if (c < ncol) a.SC[(size_t)j * a.Ph + k0 + c] = C[c * P + row0 + j];
+    }
+}
+
+// ---- rows inverse: two output rows per inverse complex transform ----
+template <typename T>
+__global__ void __launch_bounds__(kFftThreads) k_fft_rows_inv(const __grid_constant__ FftArgs a, T* __restrict__ out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P = a.Px, tid = threadIdx.x;
+    Cd* x = reinterpret_cast<Cd*>(smem_raw);
+    Cd* y = x + (size_t)a.nb * P;
+    Cd* tw = y + (size_t)a.nb * P;
+    make_twiddles(tw, P, tid, kFftThreads);
+    cudaGridDependencySynchronize();                           // plane SC of k_fft_cols is complete
+    const int pair0 = blockIdx.x * a.nb;
+    for (int idx = tid; idx < a.nb * P; idx += kFftThreads) {
+        const int b = idx / P, k = idx - b * P;
+        const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
+        Cd v = {0.0, 0.0};
+        if (r0 < a.ny) {
+            const bool mirror = k >= a.Ph;                     // C_k = conj C_{P-k} for k > P/2
+            const int kk = mirror ? P - k : k;
+            Cd ca = __ldcg(&a.SC[(size_t)r0 * a.Ph + kk]);
+            Cd cb = {0.0, 0.0};
+            if (r1 < a.ny) cb = __ldcg(&a.SC[(size_t)r1 * a.Ph + kk]);
+            if (mirror) { ca.y = -ca.y; cb.y = -cb.y; }
+            v = {ca.x - cb.y, ca.y + cb.x};                    // C_a + i C_b
+        }
+        x[idx] = v;
+    }
+    __syncthreads();
+    const Cd* X = stockham<+1>(x, y, tw, P, a.rx, a.nb, P, tid, kFftThreads);
+    const int col0 = a.kx / 2;
+    for (int idx = tid; idx < a.nb * a.nx; idx += kFftThreads) {
+        const int b = idx / a.nx, i = idx - b * a.nx;
+        const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
+        if (r0 >= a.ny) continue;
+        const Cd v = X[b * P + col0 + i];
+        out[(size_t)r0 * a.nx + i] = (T)v.x;
+        if (r1 < a.ny) out[(size_t)r1 * a.nx + i] = (T)v.y;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+// smallest 2^a 3^b 5^c >= v (even when `even`)
+static int next_smooth(int v, bool even) {
+    for (int p = v < 2 ? 2 : v;; ++p) {
+        if (even && (p & 1)) continue;
+        int q = p;
+        while (q % 2 == 0) q /= 2;
+        while (q % 3 == 0) q /= 3;
+        while (q % 5 == 0) q /= 5;
+        if (q == 1) return p;
+    }
+}
+
+static bool factor(int P, Radices* out) {
+    out->n = 0;
+    int q = P;
+    auto push = [&](int r) { if (out->n < kFftMaxPasses) out->r[out->n++] = r; };
+    while (q % 4 == 0) { push(4); q /= 4; }
+    if (q % 2 == 0) { push(2); q /= 2; }
+    while (q % 3 == 0) { push(3); q /= 3; }
+    while (q % 5 == 0) { push(5); q /= 5; }
+    return q == 1 && out->n < kFftMaxPasses;
 }
 
 struct FftPlan {
-    int Px, Py, logPx, logPy, tb, nb;
-    size_t smem_rows, smem_cols, plane_bytes;
+    FftArgs a;
+    size_t smem_rows, smem_cols;
+    size_t plane_a, plane_b, plane_c;          // bytes, 256-aligned
+    int grid_rows_fwd, grid_cols, grid_rows_inv;
     bool ok;
 };
 
-static FftPlan plan_fft(jt_dtype d, int ny, int nx, int ky, int kx) {
+static FftPlan plan_fft(int ny, int nx, int ky, int kx) {
     FftPlan p = {};
+    p.ok = false;
+    if ((int64_t)ny + ky - 1 > kFftMaxP || (int64_t)nx + kx - 1 > kFftMaxP) return p;
+    FftArgs& a = p.a;
+    a.ny = ny; a.nx = nx; a.ky = ky; a.kx = kx;
+    a.Px = next_smooth(nx + kx - 1, true);
+    a.Py = next_smooth(ny + ky - 1, false);
+    if (a.Px > kFftMaxP || a.Py > kFftMaxP) return p;
+    a.Ph = a.Px / 2 + 1;
+    if (!factor(a.Px, &a.rx) || !factor(a.Py, &a.ry)) return p;
+    a.scale = 1.0 / ((double)a.Px * (double)a.Py);
     const size_t csz = sizeof(Cd);
-    (void)d;
-    if ((int64_t)ny + ky - 1 > (1 << 14) || (int64_t)nx + kx - 1 > (1 << 14)) return p;
-    p.Px = next_pow2(nx + kx - 1, 16);
-    p.Py = next_pow2(ny + ky - 1, 16);
-    p.logPx = ilog2(p.Px);
-    p.logPy = ilog2(p.Py);
-    p.nb = 1;
-    while (p.nb < 8 && (size_t)(2 * p.nb) * p.Px <= 1024) p.nb *= 2;
-    p.smem_rows = ((size_t)p.nb * p.Px + p.Px / 2) * csz;
-    p.tb = -1;
-    for (int tb = 2; tb >= 0; --tb) {
-        const size_t sm = ((size_t)2 * (1 << tb) * (p.Py + 1) + p.Py / 2) * csz;
-        if (sm <= kFftMaxSmem && p.Px >= 2 * (1 << tb)) { p.tb = tb; p.smem_cols = sm; break; }
-    }
-    p.plane_bytes = (size_t)p.Px * p.Py * csz;
-    p.ok = p.tb >= 0 && p.smem_rows <= kFftMaxSmem;
+    // row kernels: enough butterflies per CTA for 256 threads, enough CTAs for 148 SMs
+    const int pairs_img = (ny + 1) / 2, pairs_ker = (ky + 1) / 2;
+    int nb = 1;
+    while (nb < 8 && nb * a.Px < 1024 && (pairs_img + pairs_ker) / (2 * nb) >= 2 * kNumSMs) nb *= 2;
+    a.nb = nb;
+    p.smem_rows = ((size_t)2 * nb * a.Px + a.Px) * csz;
+    a.n_cta_img = (pairs_img + nb - 1) / nb;
+    p.grid_rows_fwd = a.n_cta_img + (pairs_ker + nb - 1) / nb;
+    p.grid_rows_inv = a.n_cta_img;
+    // column kernel: 2 columns per CTA (one 32-byte sector per plane row); 4 when the transform is short
+    int tc = 2;
+    while (tc < 8 && tc * a.Py < 512 && (a.Ph + 2 * tc - 1) / (2 * tc) >= kNumSMs) tc *= 2;
+    while (tc > 1 && ((size_t)4 * tc * a.Py + a.Py) * csz > kFftMaxSmem) tc /= 2;
+    a.tc = tc;
+    p.smem_cols = ((size_t)4 * tc * a.Py + a.Py) * csz;
+    p.grid_cols = (a.Ph + tc - 1) / tc;
+    if (p.smem_rows > kFftMaxSmem || p.smem_cols > kFftMaxSmem) return p;
+    p.plane_a = align_up((size_t)ny * a.Ph * csz, 256);
+    p.plane_b = align_up((size_t)ky * a.Ph * csz, 256);
+    p.plane_c = align_up((size_t)ny * a.Ph * csz, 256);
+    p.ok = true;
     return p;
 }
 
-bool conv_fft_supported(jt_dtype d, int ny, int nx, int ky, int kx) { return plan_fft(d, ny, nx, ky, kx).ok; }
+bool conv_fft_supported(jt_dtype, int ny, int nx, int ky, int kx) { return plan_fft(ny, nx, ky, kx).ok; }
 
-// Time model behind JT_CONV_AUTO (bench.py --conv-sweep on B200: P = 128: 17 us, 256: 21.5, 512: 34, 1024: 77, 2048: 305;
-// beyond 1024 x 1024 the 16 B/point plane no longer sits comfortably in L2)
-double conv_fft_estimate_us(jt_dtype d, int ny, int nx, int ky, int kx) {
-    const FftPlan p = plan_fft(d, ny, nx, ky, kx);
+// Time model behind JT_CONV_AUTO, calibrated on B200 with bench.py --conv-sweep: three dependent
+// launches plus the planes' trips through L2.
+double conv_fft_estimate_us(jt_dtype, int ny, int nx, int ky, int kx) {
+    const FftPlan p = plan_fft(ny, nx, ky, kx);
     if (!p.ok) return 1e30;
-    const double area = (double)p.Px * p.Py / 1048576.0;
-    return 1.17 * (p.logPx + p.logPy) + 54.0 * area + (area > 1.0 ? 20.0 * (area - 1.0) : 0.0);
+    const double mb = (double)(p.plane_a + p.plane_b + p.plane_c) * 2.0 / 1048576.0;
+    return 9.0 + 1.2 * mb;
 }
 
-size_t fft_conv_workspace_bytes(jt_dtype d, int ny, int nx, int ky, int kx) {
-    const FftPlan p = plan_fft(d, ny, nx, ky, kx);
-    return p.ok ? align_up(p.plane_bytes, 256) + 2 * kFftSumCtas * sizeof(double) : 0;
+size_t fft_conv_workspace_bytes(jt_dtype, int ny, int nx, int ky, int kx) {
+    const FftPlan p = plan_fft(ny, nx, ky, kx);
+    return p.ok ? p.plane_a + p.plane_b + p.plane_c : 0;
 }
 
-template <typename T>
-static jt_status conv_fft_t(const FftPlan& p, int ny, int nx, const T* img, int ky, int kx, const T* ker, void* workspace,
-                            T* out, cudaStream_t st) {
-    Cd* plane = (Cd*)workspace;
-    double* partial = (double*)((char*)workspace + align_up(p.plane_bytes, 256));
-    const int rows_nz = ny > ky ? ny : ky;
-    const int64_t n_img = (int64_t)ny * nx, n_ker = (int64_t)ky * kx;
-    int n_part = (int)((n_img + 4095) / 4096);
-    n_part = n_part < 1 ? 1 : (n_part > kFftSumCtas ? kFftSumCtas : n_part);
-    k_fft_sums<T><<<n_part, 256, 0, st>>>(n_img, img, n_ker, ker, partial);
-    JT_LAUNCH_CHECK();
-    auto k1 = k_fft_rows_fwd<T>;
-    auto k2 = k_fft_cols;
-    auto k3 = k_fft_rows_inv<T>;
-    JT_CUDA_TRY(cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_rows));
-    JT_CUDA_TRY(cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_cols));
-    JT_CUDA_TRY(cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.smem_rows));
-    k1<<<(rows_nz + p.nb - 1) / p.nb, kFftRowThreads, p.smem_rows, st>>>(ny, nx, img, ky, kx, ker, p.logPx, rows_nz, p.nb, partial, n_part, plane);
-    JT_LAUNCH_CHECK();
-    const int n_cta = (p.Px >> (p.tb + 1)) + 1;
-    const double scale = 1.0 / ((double)p.Px * (double)p.Py);
-    k2<<<n_cta, kFftColThreads, p.smem_cols, st>>>(p.logPx, p.logPy, p.tb, rows_nz, ky / 2, ny, scale, partial, n_part, plane);
-    JT_LAUNCH_CHECK();
-    k3<<<(ny + p.nb - 1) / p.nb, kFftRowThreads, p.smem_rows, st>>>(ny, nx, p.logPx, ky / 2, kx / 2, p.nb, plane, out);
+template <typename K, typename... Args>
+static jt_status launch_fft_kernel(K kern, int grid, size_t smem, bool dependent, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3(kFftThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = dependent ? 1 : 0;
+    JT_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, args...));
     JT_LAUNCH_CHECK();
     return JT_OK;
 }
 
+template <typename T>
+static jt_status conv_fft_t(FftPlan& p, const T* img, const T* ker, void* workspace, T* out, cudaStream_t st) {
+    FftArgs& a = p.a;
+    a.SA = (Cd*)workspace;
+    a.SB = (Cd*)((char*)workspace + p.plane_a);
+    a.SC = (Cd*)((char*)workspace + p.plane_a + p.plane_b);
+    auto k1 = k_fft_rows_fwd<T>;
+    auto k2 = k_fft_cols;
+    auto k3 = k_fft_rows_inv<T>;
+    static bool attr_set = false;                  // once per instantiation: allow the full dynamic shared memory
+    if (!attr_set) {
+        JT_CUDA_TRY(cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
+        JT_CUDA_TRY(cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
+        JT_CUDA_TRY(cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
+        attr_set = true;
+    }
+    jt_status s = launch_fft_kernel(k1, p.grid_rows_fwd, p.smem_rows, false, st, a, img, ker);
+    if (s != JT_OK) return s;
+    s = launch_fft_kernel(k2, p.grid_cols, p.smem_cols, true, st, a);
+    if (s != JT_OK) return s;
+    return launch_fft_kernel(k3, p.grid_rows_inv, p.smem_rows, true, st, a, out);
+}
+
 jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker, void* workspace,
                           void* out, cudaStream_t st) {
-    const FftPlan p = plan_fft(dtype, ny, nx, ky, kx);
+    FftPlan p = plan_fft(ny, nx, ky, kx);
     if (!p.ok) return JT_ERR_UNSUPPORTED;
-    return dtype == JT_F32 ? conv_fft_t<float>(p, ny, nx, (const float*)img, ky, kx, (const float*)ker, workspace, (float*)out, st)
-                           : conv_fft_t<double>(p, ny, nx, (const double*)img, ky, kx, (const double*)ker, workspace, (double*)out, st);
+    return dtype == JT_F32 ? conv_fft_t<float>(p, (const float*)img, (const float*)ker, workspace, (float*)out, st)
+                           : conv_fft_t<double>(p, (const double*)img, (const double*)ker, workspace, (double*)out, st);
 }
 
 }  // namespace jt
