@@ -25,7 +25,7 @@
 namespace jt {
 
 using Cd = double2;
-constexpr int kFftThreads = 256;
+constexpr int kFftMaxThreads = 512;            // CTA size is chosen per plan
 constexpr int kFftMaxP = 2048;                 // two ping-pong buffers + the twiddle table of one transform fit 227 KB
 constexpr int kFftMaxPasses = 12;
 constexpr size_t kFftMaxSmem = 220 * 1024;
@@ -84,13 +84,17 @@ template <int SIGN> struct Dft<5, SIGN> {
     }
 };
 
-// tw[j] = exp(-2 pi i j / N), j < N (sincospi in double)
+// tw[j] = exp(-2 pi i j / N), j < N.  sincospi in double for j <= N/2 only; the upper half by conjugation.
+// Ends with a barrier.
 __device__ __forceinline__ void make_twiddles(Cd* tw, int N, int tid, int nthr) {
-    for (int j = tid; j < N; j += nthr) {
+    const int half = N / 2;
+    for (int j = tid; j <= half; j += nthr) {
         double s, c;
         sincospi(-2.0 * (double)j / (double)N, &s, &c);
         tw[j] = {c, s};
+        if (j > 0 && N - j > half) tw[N - j] = {c, -s};
     }
+    __syncthreads();
 }
 
 // One Stockham pass of radix R over `nbatch` transforms of length N (x -> y, transform b at offset b * pitch):
@@ -151,21 +155,21 @@ struct FftArgs {
 
 // ---- rows forward: pairs of real rows -> half spectra ----
 template <typename T>
-__global__ void __launch_bounds__(kFftThreads) k_fft_rows_fwd(const __grid_constant__ FftArgs a, const T* __restrict__ img,
+__global__ void __launch_bounds__(kFftMaxThreads) k_fft_rows_fwd(const __grid_constant__ FftArgs a, const T* __restrict__ img,
                                                               const T* __restrict__ ker) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int P = a.Px, tid = threadIdx.x;
+    const int P = a.Px, tid = threadIdx.x, nthr = blockDim.x;
     Cd* x = reinterpret_cast<Cd*>(smem_raw);
     Cd* y = x + (size_t)a.nb * P;
     Cd* tw = y + (size_t)a.nb * P;
     cudaTriggerProgrammaticLaunchCompletion();                 // lets k_fft_cols start its twiddle set-up once every CTA here runs
-    make_twiddles(tw, P, tid, kFftThreads);
+    make_twiddles(tw, P, tid, nthr);
     const bool is_img = (int)blockIdx.x < a.n_cta_img;
     const T* src = is_img ? img : ker;
     const int rows = is_img ? a.ny : a.ky, width = is_img ? a.nx : a.kx;
     Cd* plane = is_img ? a.SA : a.SB;
     const int pair0 = (is_img ? (int)blockIdx.x : (int)blockIdx.x - a.n_cta_img) * a.nb;
-    for (int idx = tid; idx < a.nb * P; idx += kFftThreads) {
+    for (int idx = tid; idx < a.nb * P; idx += nthr) {
         const int b = idx / P, i = idx - b * P;
         const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
         Cd v = {0.0, 0.0};
@@ -176,8 +180,8 @@ __global__ void __launch_bounds__(kFftThreads) k_fft_rows_fwd(const __grid_const
         x[idx] = v;
     }
     __syncthreads();
-    const Cd* X = stockham<-1>(x, y, tw, P, a.rx, a.nb, P, tid, kFftThreads);
-    for (int idx = tid; idx < a.nb * a.Ph; idx += kFftThreads) {
+    const Cd* X = stockham<-1>(x, y, tw, P, a.rx, a.nb, P, tid, nthr);
+    for (int idx = tid; idx < a.nb * a.Ph; idx += nthr) {
         const int b = idx / a.Ph, k = idx - b * a.Ph;
         const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
         if (r0 >= rows) continue;
@@ -188,18 +192,18 @@ __global__ void __launch_bounds__(kFftThreads) k_fft_rows_fwd(const __grid_const
 }
 
 // ---- columns: forward FFTs of tc image and tc kernel spectrum columns, product, inverse FFT, crop ----
-__global__ void __launch_bounds__(kFftThreads) k_fft_cols(const __grid_constant__ FftArgs a) {
+__global__ void __launch_bounds__(kFftMaxThreads) k_fft_cols(const __grid_constant__ FftArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int P = a.Py, tc = a.tc, tid = threadIdx.x;
+    const int P = a.Py, tc = a.tc, tid = threadIdx.x, nthr = blockDim.x;
     Cd* x = reinterpret_cast<Cd*>(smem_raw);                   // [2 tc][P]: image columns, then kernel columns
     Cd* y = x + (size_t)2 * tc * P;
     Cd* tw = y + (size_t)2 * tc * P;
-    make_twiddles(tw, P, tid, kFftThreads);
+    make_twiddles(tw, P, tid, nthr);
     cudaGridDependencySynchronize();                           // the planes SA, SB of k_fft_rows_fwd are complete
     cudaTriggerProgrammaticLaunchCompletion();
     const int k0 = blockIdx.x * tc;
     const int ncol = min(tc, a.Ph - k0);
-    for (int idx = tid; idx < P * tc; idx += kFftThreads) {
+    for (int idx = tid; idx < P * tc; idx += nthr) {
         const int r = idx / tc, c = idx - r * tc;
         Cd va = {0.0, 0.0}, vb = {0.0, 0.0};
         if (c < ncol) {
@@ -210,18 +214,18 @@ __global__ void __launch_bounds__(kFftThreads) k_fft_cols(const __grid_constant_
         x[(tc + c) * P + r] = vb;
     }
     __syncthreads();
-    Cd* X = stockham<-1>(x, y, tw, P, a.ry, 2 * tc, P, tid, kFftThreads);
+    Cd* X = stockham<-1>(x, y, tw, P, a.ry, 2 * tc, P, tid, nthr);
     Cd* Y = (X == x) ? y : x;
-    for (int idx = tid; idx < tc * P; idx += kFftThreads) {
+    for (int idx = tid; idx < tc * P; idx += nthr) {
         Cd c = cmul(X[idx], X[tc * P + idx]);
         c.x *= a.scale;
         c.y *= a.scale;
         X[idx] = c;
     }
     __syncthreads();
-    const Cd* C = stockham<+1>(X, Y, tw, P, a.ry, tc, P, tid, kFftThreads);
+    const Cd* C = stockham<+1>(X, Y, tw, P, a.ry, tc, P, tid, nthr);
     const int row0 = a.ky / 2;
-    for (int idx = tid; idx < a.ny * tc; idx += kFftThreads) {
+    for (int idx = tid; idx < a.ny * tc; idx += nthr) {
         const int j = idx / tc, c = idx - j * tc;
         if (c < ncol) a.SC[(size_t)j * a.Ph + k0 + c] = C[c * P + row0 + j];
     }
@@ -229,16 +233,16 @@ __global__ void __launch_bounds__(kFftThreads) k_fft_cols(const __grid_constant_
 
 // ---- rows inverse: two output rows per inverse complex transform ----
 template <typename T>
-__global__ void __launch_bounds__(kFftThreads) k_fft_rows_inv(const __grid_constant__ FftArgs a, T* __restrict__ out) {
+__global__ void __launch_bounds__(kFftMaxThreads) k_fft_rows_inv(const __grid_constant__ FftArgs a, T* __restrict__ out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int P = a.Px, tid = threadIdx.x;
+    const int P = a.Px, tid = threadIdx.x, nthr = blockDim.x;
     Cd* x = reinterpret_cast<Cd*>(smem_raw);
     Cd* y = x + (size_t)a.nb * P;
     Cd* tw = y + (size_t)a.nb * P;
-    make_twiddles(tw, P, tid, kFftThreads);
+    make_twiddles(tw, P, tid, nthr);
     cudaGridDependencySynchronize();                           // plane SC of k_fft_cols is complete
     const int pair0 = blockIdx.x * a.nb;
-    for (int idx = tid; idx < a.nb * P; idx += kFftThreads) {
+    for (int idx = tid; idx < a.nb * P; idx += nthr) {
         const int b = idx / P, k = idx - b * P;
         const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
         Cd v = {0.0, 0.0};
@@ -254,9 +258,9 @@ __global__ void __launch_bounds__(kFftThreads) k_fft_rows_inv(const __grid_const
         x[idx] = v;
     }
     __syncthreads();
-    const Cd* X = stockham<+1>(x, y, tw, P, a.rx, a.nb, P, tid, kFftThreads);
+    const Cd* X = stockham<+1>(x, y, tw, P, a.rx, a.nb, P, tid, nthr);
     const int col0 = a.kx / 2;
-    for (int idx = tid; idx < a.nb * a.nx; idx += kFftThreads) {
+    for (int idx = tid; idx < a.nb * a.nx; idx += nthr) {
         const int b = idx / a.nx, i = idx - b * a.nx;
         const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
         if (r0 >= a.ny) continue;
@@ -294,7 +298,7 @@ struct FftPlan {
     FftArgs a;
     size_t smem_rows, smem_cols;
     size_t plane_a, plane_b, plane_c;          // bytes, 256-aligned
-    int grid_rows_fwd, grid_cols, grid_rows_inv;
+    int grid_rows_fwd, grid_cols, grid_rows_inv, thr_rows, thr_cols;
     bool ok;
 };
 
@@ -328,6 +332,11 @@ static FftPlan plan_fft(int ny, int nx, int ky, int kx) {
     p.smem_cols = ((size_t)4 * tc * a.Py + a.Py) * csz;
     p.grid_cols = (a.Ph + tc - 1) / tc;
     if (p.smem_rows > kFftMaxSmem || p.smem_cols > kFftMaxSmem) return p;
+    // CTA sizes: about one radix-4 butterfly per thread and pass, capped where more warps only lengthen the barriers
+    // (measured on B200: rows 256, columns 384-512 are best from 60^2 to 1000^2)
+    auto pick_threads = [](int butterflies, int cap) { int t = (butterflies + 31) / 32 * 32; return t < 128 ? 128 : (t > cap ? cap : t); };
+    p.thr_rows = pick_threads(nb * a.Px / 4, 256);
+    p.thr_cols = pick_threads(2 * tc * a.Py / 4, 512);
     p.plane_a = align_up((size_t)ny * a.Ph * csz, 256);
     p.plane_b = align_up((size_t)ky * a.Ph * csz, 256);
     p.plane_c = align_up((size_t)ny * a.Ph * csz, 256);
@@ -352,10 +361,10 @@ size_t fft_conv_workspace_bytes(jt_dtype, int ny, int nx, int ky, int kx) {
 }
 
 template <typename K, typename... Args>
-static jt_status launch_fft_kernel(K kern, int grid, size_t smem, bool dependent, cudaStream_t st, Args... args) {
+static jt_status launch_fft_kernel(K kern, int grid, int threads, size_t smem, bool dependent, cudaStream_t st, Args... args) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)grid);
-    cfg.blockDim = dim3(kFftThreads);
+    cfg.blockDim = dim3((unsigned)threads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute at[1];
@@ -384,11 +393,11 @@ static jt_status conv_fft_t(FftPlan& p, const T* img, const T* ker, void* worksp
         JT_CUDA_TRY(cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         attr_set = true;
     }
-    jt_status s = launch_fft_kernel(k1, p.grid_rows_fwd, p.smem_rows, false, st, a, img, ker);
+    jt_status s = launch_fft_kernel(k1, p.grid_rows_fwd, p.thr_rows, p.smem_rows, false, st, a, img, ker);
     if (s != JT_OK) return s;
-    s = launch_fft_kernel(k2, p.grid_cols, p.smem_cols, true, st, a);
+    s = launch_fft_kernel(k2, p.grid_cols, p.thr_cols, p.smem_cols, true, st, a);
     if (s != JT_OK) return s;
-    return launch_fft_kernel(k3, p.grid_rows_inv, p.smem_rows, true, st, a, out);
+    return launch_fft_kernel(k3, p.grid_rows_inv, p.thr_rows, p.smem_rows, true, st, a, out);
 }
 
 jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker, void* workspace,
