@@ -46,6 +46,7 @@ TIER_COST = {"f32": (14.5, 29.6, 47.0, 29.6), "f64": (25.2, 50.6, 80.0, 50.6)}
 NCU_TRAFFIC_BYTES = {"C2-f64": 483072 + 1126400, "C2-f32": 267008 + 510976, "C3-f32": 15798016 + 41087488}
 ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
+PER_CONFIG = ("C2-f64", "C2-f32", "C3-f32")        # reported beside the headline workload in the same JSON line
 
 
 # ------------------------------------------------------------------ distributed plumbing
@@ -307,15 +308,92 @@ def load_peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-def run_ours(args, rank, world, local_rank):
-    import torch
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
-    torch.cuda.set_device(local_rank)
-    import paper_2606_01547_b200 as jt
-    jt.lib()
+def graph_time(torch, call, n_rep=20, repeats=3):
+    """Device time per call in microseconds: n_rep back-to-back calls captured into a CUDA graph on a side stream, the
+    replay timed with CUDA events (best of `repeats`) -- no Python / ctypes cost inside the number."""
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        for _ in range(3):
+            call()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            for _ in range(n_rep):
+                call()
+    torch.cuda.synchronize()
+    g.replay()
+    torch.cuda.synchronize()
+    best = None
+    for _ in range(repeats):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        g.replay()
+        b.record()
+        b.synchronize()
+        t = 1e3 * a.elapsed_time(b) / n_rep
+        best = t if best is None else min(best, t)
+    return best
 
-    w = make_workload(args.workload, rank)
+
+def fft_conv_bytes(ny, nx, ky, kx, esz):
+    """Algorithmic bytes of the FFT convolution: image in and out, kernel in, and the three
+    half-spectrum planes of complex doubles, each written once and read once (SA [ny][Ph], SB [ky][Ph], SC [ny][Ph])."""
+    def smooth(v, even):
+        p = max(v, 2)
+        while True:
+            q = p
+            for f in (2, 3, 5):
+                while q % f == 0:
+                    q //= f
+            if q == 1 and not (even and p % 2):
+                return p
+            p += 1
+    Px, Py = smooth(nx + kx - 1, True), smooth(ny + ky - 1, False)
+    Ph = Px // 2 + 1
+    return (2 * nx * ny + ky * kx) * esz + 2 * 16 * Ph * (2 * ny + ky), (Py, Px)
+
+
+def conv_block(torch, jt, w, peaks, probes):
+    """jt_psf_convolve alone on this workload's image and PSF shape, BOTH methods (CUDA-graph replay, device time per
+    call), each against its own roofline: direct -> FMA peak of the dtype, FFT -> measured HBM bandwidth."""
+    tdt = torch.float32 if w.dtype == "f32" else torch.float64
+    esz = 4 if w.dtype == "f32" else 8
+    lanes = ALU_LANES_PER_SM[w.dtype]
+    ky, kx = w.psf.shape[-2:]
+    psf = w.psf if w.psf.ndim == 2 else w.psf[0]
+    rng = np.random.default_rng(154710)
+    img = torch.as_tensor(rng.uniform(0.0, 1.0, (w.ny, w.nx)), dtype=tdt, device="cuda")
+    ker = torch.as_tensor(np.ascontiguousarray(psf), dtype=tdt, device="cuda")
+    out = torch.empty_like(img)
+    fma = w.nx * w.ny * ky * kx
+    fma_peak = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6
+    nbytes, pad = fft_conv_bytes(w.ny, w.nx, ky, kx, esz)
+    blk = {"shape": "%dx%d image, %dx%d kernel" % (w.ny, w.nx, ky, kx), "dtype": w.dtype,
+           "auto_picks": "fft" if jt.psf_convolve_workspace_bytes(w.dtype, w.ny, w.nx, ky, kx, "auto") ==
+                         jt.psf_convolve_workspace_bytes(w.dtype, w.ny, w.nx, ky, kx, "fft") else "direct"}
+    for method in ("direct", "fft"):
+        try:
+            ws = torch.empty(max(jt.psf_convolve_workspace_bytes(w.dtype, w.ny, w.nx, ky, kx, method), 1),
+                             dtype=torch.uint8, device="cuda")
+            us = graph_time(torch, lambda: jt.psf_convolve(img, ker, method=method, workspace=ws, out=out))
+        except jt.JtError as e:
+            blk[method] = {"error": str(e)}
+            continue
+        d = {"us": us, "gbs_algorithmic_io": (2 * w.nx * w.ny + ky * kx) * esz / (us * 1e-6) / 1e9}
+        if method == "direct":
+            meas = 2 * probes["ffma2"] if w.dtype == "f32" else probes["dfma"]
+            d.update({"bound": "alu", "fma_per_s": fma / (us * 1e-6), "frac_of_derived_fma_peak": fma / (us * 1e-6) / fma_peak,
+                      "frac_of_measured_fma_rate": fma / (us * 1e-6) / meas})
+        else:
+            d.update({"bound": "hbm", "bytes": nbytes, "pad": "%dx%d" % pad, "gbs": nbytes / (us * 1e-6) / 1e9,
+                      "frac_of_measured_hbm": nbytes / (us * 1e-6) / 1e9 / peaks.get("hbm_gbs", 6650.0)})
+        blk[method] = d
+    return blk
+
+
+def measure(torch, jt, name, args, rank, world, sample_clocks=False):
+    """Both timed legs and the roofline record of one workload.  Returns a dict (rank 0) or None."""
+    w = make_workload(name, rank)
     batch = hasattr(w, "B")
     runner = BatchRunner(jt, w) if batch else ImageRunner(jt, w, args.method)
     flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")     # 256 MiB > 126 MB L2
@@ -325,7 +403,7 @@ def run_ours(args, rank, world, local_rank):
     for _ in range(args.warmup):
         runner.step()
     torch.cuda.synchronize()
-    sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
+    sampler = ClockSampler(torch.cuda.current_device()) if (rank == 0 and sample_clocks) else None
     if sampler:
         sampler.start()
         time.sleep(0.25)
@@ -365,20 +443,18 @@ def run_ours(args, rank, world, local_rank):
     e2e_ms_local = 1e3 * (time.perf_counter() - t0)
     barrier()
     e2e_units, e2e_ms = aggregate(w.evals * args.steps, e2e_ms_local)
-
+    del flush
     if rank != 0:
-        return
+        return None
+
     peaks, peak_kind = load_peaks()
-    value = units / (ms_total * 1e-3)
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
-            "config": describe(args.workload, w, world),
-            "images_per_s": world * runner.images * args.steps / (ms_total * 1e-3),
-            "clocks": clocks,
-            "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": runner.h2d,
-                    "d2h_bytes_per_step": runner.d2h, "ms_per_step": e2e_ms / args.steps},
-            "gpu_launches": int(launches)}
+    rec = {"value": units / (ms_total * 1e-3), "ms_per_step": ms_total / args.steps,
+           "ms_per_step_median": float(np.median(ms)), "ms_per_step_best": float(np.min(ms)), "dtype": w.dtype,
+           "config": describe(name, w, world),
+           "images_per_s": world * runner.images * args.steps / (ms_total * 1e-3), "clocks": clocks,
+           "e2e": {"value": e2e_units / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": runner.h2d,
+                   "d2h_bytes_per_step": runner.d2h, "ms_per_step": e2e_ms / args.steps},
+           "gpu_launches": int(launches)}
 
     # ---- roofline of the dominant kernel: the ray-tracing kernel, issue-limited ALU peak ----
     f_mhz = (clocks or {}).get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
@@ -405,9 +481,9 @@ def run_ours(args, rank, world, local_rank):
     mix = tiers / tiers.sum() if tiers.sum() > 0 else np.array([0.0, 1.0, 0.0, 0.0])
     n_alg = float(np.dot(mix, TIER_COST[w.dtype]))
     achieved = w.evals * n_alg / (trace_ms * 1e-3) / 1e12
-    line["roofline"] = {
+    rec["roofline"] = {
         "bound": "alu", "kernel": "k_batch" if batch else "k_trace", "achieved": achieved, "peak": peak_tinstr,
-        "unit": "Tlaneop/s", "frac": achieved / peak_tinstr, "traffic": NCU_TRAFFIC_BYTES.get(args.workload),
+        "unit": "Tlaneop/s", "frac": achieved / peak_tinstr, "traffic": NCU_TRAFFIC_BYTES.get(name),
         "peak_kind": "derived: 148 SMs x %d lanes/clk (%s) x %.0f MHz (max clock, %s)" % (
             lanes, "FP32 pipe" if w.dtype == "f32" else "FP64 pipe", peaks.get("sm_max_mhz", 1965.0),
             peak_kind),
@@ -416,39 +492,45 @@ def run_ours(args, rank, world, local_rank):
         "kernel_share_of_step": trace_ms / (ms_total_local / args.steps),
         "frac_at_observed_clock": achieved / (SM_COUNT * lanes * f_mhz * 1e6 / 1e12),
         "evals_per_s_kernel": w.evals / (trace_ms * 1e-3)}
-    # ---- ALU rates measured in this run by the library's microbenchmark (thread-level instructions / s) ----
+    rec["_w"] = w
+    return rec
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    import paper_2606_01547_b200 as jt
+    jt.lib()
+
+    head = measure(torch, jt, args.workload, args, rank, world, sample_clocks=True)
+    # the other paper-shaped workloads, same legs, in the same JSON line (single-GPU runs only: replicas add nothing here)
+    per_config = {}
+    if world == 1 and not args.no_per_config:
+        for name in PER_CONFIG:
+            if name != args.workload:
+                r = measure(torch, jt, name, args, rank, world)
+                r.pop("_w")
+                per_config[name] = r
+    if rank != 0:
+        return
+    peaks, _ = load_peaks()
+    w = head.pop("_w")
+    line = {"metric": METRIC, "value": head.pop("value"), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": head.pop("ms_per_step"), "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": head.pop("dtype"), "data": "synthetic"}
+    line.update(head)
+    # ---- ALU rates measured in this run by the probe library's microbenchmark (thread-level instructions / s) ----
     probes = {k: jt.probe_alu(k) for k in ("ffma", "ffma2", "dfma", "mufu_rsq")}
     line["alu_peaks_measured"] = {k: {"Tlaneinstr_per_s": v / 1e12, "lanes_per_clk_per_sm_at_max_clock":
                                       v / SM_COUNT / (peaks.get("sm_max_mhz", 1965.0) * 1e6)} for k, v in probes.items()}
-    meas = probes["ffma"] if w.dtype == "f32" else probes["dfma"]
-    line["roofline"]["frac_of_measured_alu_rate"] = achieved * 1e12 / meas
-    if not batch:
-        ky, kx = w.psf.shape
-        K = ky * kx
-        esz = 4 if w.dtype == "f32" else 8
-        lanes = 128 if w.dtype == "f32" else 64
-        fma_peak = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6
-        method = args.method
-        if method == "auto":                                       # what jt_api.cu's resolve_conv_method picked
-            method = "fft" if jt.psf_convolve_workspace_bytes(w.dtype, w.ny, w.nx, ky, kx, "auto") > 0 else "direct"
-        conv = {"method": method, "ms": conv_ms,
-                "gbs_algorithmic": (2 * w.nx * w.ny + K) * esz / (conv_ms * 1e-3) / 1e9 if conv_ms > 0 else None}
-        if conv_ms > 0 and method == "direct":
-            conv.update({"bound": "alu", "fma_per_s": w.nx * w.ny * K / (conv_ms * 1e-3),
-                         "frac_of_derived_fma_peak": w.nx * w.ny * K / (conv_ms * 1e-3) / fma_peak,
-                         "frac_of_measured_fma_rate": w.nx * w.ny * K / (conv_ms * 1e-3) /
-                                                      (2 * probes["ffma2"] if w.dtype == "f32" else probes["dfma"])})
-        elif conv_ms > 0:
-            # FFT path: image in + image out + kernel in, plus the complex-double plane written by the row pass, read and
-            # written (cropped rows only) by the column pass and read by the inverse row pass
-            p2 = lambda v: 1 << max(4, int(np.ceil(np.log2(v))))
-            Px, Py = p2(w.nx + kx - 1), p2(w.ny + ky - 1)
-            plane = 16 * Px * (2 * max(w.ny, ky) + 2 * w.ny)
-            nbytes = (2 * w.nx * w.ny + K) * esz + plane
-            conv.update({"bound": "hbm", "bytes": nbytes, "gbs": nbytes / (conv_ms * 1e-3) / 1e9,
-                         "frac_of_measured_hbm": nbytes / (conv_ms * 1e-3) / 1e9 / peaks.get("hbm_gbs", 6650.0),
-                         "pad": "%dx%d" % (Py, Px)})
-        line["conv"] = conv
+    for r in [line] + list(per_config.values()):
+        meas = probes["ffma"] if r["dtype"] == "f32" else probes["dfma"]
+        r["roofline"]["frac_of_measured_alu_rate"] = r["roofline"]["achieved"] * 1e12 / meas
+    line["conv"] = conv_block(torch, jt, w, peaks, probes)
+    if per_config:
+        line["per_config"] = per_config
     if not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w, args.cpu_evals)
     print(json.dumps(line), flush=True)
@@ -472,32 +554,6 @@ def run_conv_sweep(args, rank):
              [(100, 13), (100, 31), (200, 21), (500, 101), (1000, 31)]
     reps = 20
     rows = []
-    side = torch.cuda.Stream()
-
-    def graph_time(call, n_rep):
-        """device time per call: n_rep back-to-back calls captured into a CUDA graph, the replay timed with events"""
-        with torch.cuda.stream(side):
-            for _ in range(3):
-                call()
-            torch.cuda.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g, stream=side):
-                for _ in range(n_rep):
-                    call()
-        torch.cuda.synchronize()
-        g.replay()
-        torch.cuda.synchronize()
-        best = None
-        for _ in range(3):
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            g.replay()
-            b.record()
-            b.synchronize()
-            t = 1e3 * a.elapsed_time(b) / n_rep
-            best = t if best is None else min(best, t)
-        return best
-
     paper_shapes = set([(60, k) for k in (3, 11, 21, 31, 45)] + [(180, k) for k in (9, 45, 87, 135)] + [(100, 13)])
     for dtype, tdt, lanes, esz in (("f32", torch.float32, 128, 4), ("f64", torch.float64, 64, 8)):
         fma_peak = SM_COUNT * lanes * peaks.get("sm_max_mhz", 1965.0) * 1e6
@@ -515,7 +571,7 @@ def run_conv_sweep(args, rank):
                         nb = jt.psf_convolve_batch_workspace_bytes(dtype, B, n, n, k, k, method)
                         ws = torch.empty(max(nb, 1), dtype=torch.uint8, device="cuda")
                         call = lambda: jt.psf_convolve_batch(img, ker, method=method, workspace=ws, out=out)
-                        us = graph_time(call, reps if B == 1 else 3)
+                        us = graph_time(torch, call, reps if B == 1 else 3)
                         row[method + "_us"] = us
                         row[method + "_gbs"] = B * (2 * n * n + k * k) * esz / (us * 1e-6) / 1e9
                         if method == "direct":
@@ -534,11 +590,12 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C2-f64", choices=WORKLOADS)
+    ap.add_argument("--workload", default="C4-f64", choices=WORKLOADS)
     ap.add_argument("--method", default="auto", choices=["auto", "direct", "fft"])
     ap.add_argument("--cpu-evals", type=float, default=1.5e9, help="oracle sample size for cpu_baseline")
     ap.add_argument("--ref-evals", type=float, default=2.0e8, help="oracle sample size per --impl reference step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (C2-f64, C2-f32, C3-f32)")
     ap.add_argument("--conv-sweep", action="store_true", help="time jt_psf_convolve alone at the paper's shapes")
     ap.add_argument("--sweep-batch", type=int, default=1024, help="batch size of the batched rows of --conv-sweep")
     args = ap.parse_args()
