@@ -15,8 +15,11 @@
  *   - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default
  *     stream).  No function synchronises the device; host structs are read before the call
  *     returns, so the caller may free them immediately.
- *   - The caller owns every buffer, workspace included.  The library allocates no device memory
- *     and keeps no device state between calls.
+ *   - The caller owns every buffer, workspace included.  The library allocates no device memory.
+ *     State it keeps between calls, all of it listed here: per host thread the last CUDA error code, the
+ *     launch counter and -- only while jt_profile_enable(1) is in force -- four CUDA events and a 32-byte
+ *     pinned host buffer; per process one 60 KB __constant__ buffer per device (the taps of the direct
+ *     convolution) with the event that orders its users (see jt_psf_convolve).
  *   - "device [n]" = pointer to device memory holding n elements of the call's dtype
  *     (float for JT_F32, double for JT_F64), aligned to the element size.  "host" = ordinary
  *     host memory.  Arrays are row-major, x (column) fastest.
@@ -159,18 +162,17 @@ JT_API jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid *gri
                             void *out, void *stream);
 
 /* Measurement aid (bench.py's roofline leg).  jt_profile_enable(1) makes every following
- * jt_simulate_image call on this host thread record CUDA events on its stream before the ray-tracing
- * kernel, between it and the convolution, and after the convolution (three cudaEventRecord calls, no
- * synchronisation).  jt_profile_read waits for the events of the LAST such call and returns the two
- * intervals in milliseconds (conv_ms = 0 when the call had no PSF).  JT_ERR_INVALID_VALUE when profiling is
- * off or no call has been recorded.  The events are the only state the library keeps; jt_profile_enable(0)
- * destroys them. */
+ * jt_simulate_image call on this host thread record CUDA events on its stream before the ray-tracing kernel, between it
+ * and the convolution, and after the convolution, and copy the kernel's four tier counters (32 bytes) to a pinned host
+ * buffer the library owns (event records and one cudaMemcpyAsync: no synchronisation, nothing keeps pointing into the
+ * caller's workspace).  jt_profile_read waits for the events of the LAST such call and returns the two intervals in
+ * milliseconds (conv_ms = 0 when the call had no PSF).  JT_ERR_INVALID_VALUE when profiling is off or no call has been
+ * recorded.  jt_profile_enable(0) destroys the events and frees the buffer. */
 JT_API jt_status jt_profile_enable(int on);
 JT_API jt_status jt_profile_read(float *trace_ms, float *conv_ms);
-/* After jt_profile_read semantics: copies the four counters of the LAST profiled jt_simulate_image call to host
- * memory counts[4]: (warp, subhalo-record) pairs evaluated by the far-far series, the far form, the mid form and the
- * per-ray cold path.  The counters live in the call's workspace, which must still be allocated;
- * the call synchronises on the profiling events. */
+/* counts[4] (host) receives, for the LAST profiled jt_simulate_image call, the number of (warp, subhalo-record) pairs
+ * evaluated by the far-far series, the far form, the mid form and the per-ray cold path.
+ * Waits for that call's counter copy (an event), not for the device. */
 JT_API jt_status jt_profile_tiers(uint64_t *counts);
 
 /* Number of CUDA kernels this library has launched from the calling host thread since it was loaded

@@ -244,11 +244,15 @@ def _sources(sources):
     return S, a          # keep `a` alive during the call
 
 
-def _workspace(nbytes, device, workspace):
+def _workspace(nbytes, device, workspace, stream=None):
+    """Caller's workspace, or a scratch tensor; a scratch tensor used on a non-current stream is tied to that stream
+    (record_stream) so that the caching allocator cannot hand it out again while the kernels still run."""
     if nbytes == 0:
         return None, 0
     if workspace is None:
         workspace = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        if stream is not None:
+            workspace.record_stream(stream)
     return workspace, workspace.numel() * workspace.element_size()
 
 
@@ -263,7 +267,7 @@ def ray_shoot(theta_x, theta_y, sie=None, shear=None, tnfw=None, workspace=None,
     code = _dt(theta_x)
     n = theta_x.numel()
     L = _lens(code, sie, shear, tnfw)
-    ws, wsb = _workspace(ray_shoot_workspace_bytes(code, n, L.n_tnfw), theta_x.device, workspace)
+    ws, wsb = _workspace(ray_shoot_workspace_bytes(code, n, L.n_tnfw), theta_x.device, workspace, stream)
     bx, by = torch.empty_like(theta_x), torch.empty_like(theta_y)
     _check(lib().jt_ray_shoot(code, n, _ptr(theta_x), _ptr(theta_y), ctypes.byref(L), _ptr(ws), wsb,
                               _ptr(bx), _ptr(by), _stream(stream)), "jt_ray_shoot")
@@ -294,7 +298,7 @@ def psf_convolve(image, kernel, method="auto", workspace=None, out=None, stream=
         raise TypeError("image and kernel dtypes differ")
     ny, nx = image.shape
     ky, kx = kernel.shape
-    ws, wsb = _workspace(psf_convolve_workspace_bytes(code, ny, nx, ky, kx, method), image.device, workspace)
+    ws, wsb = _workspace(psf_convolve_workspace_bytes(code, ny, nx, ky, kx, method), image.device, workspace, stream)
     if out is None:
         out = torch.empty_like(image)
     _check(lib().jt_psf_convolve(code, ny, nx, _ptr(image), ky, kx, _ptr(kernel), _METHODS[method], _ptr(ws), wsb,
@@ -315,7 +319,7 @@ def psf_convolve_batch(images, kernel, method="auto", workspace=None, out=None, 
     B, ny, nx = images.shape
     ky, kx = kernel.shape
     ws, wsb = _workspace(psf_convolve_batch_workspace_bytes(code, B, ny, nx, ky, kx, method) if B > 0 else 0,
-                         images.device, workspace)
+                         images.device, workspace, stream)
     if out is None:
         out = torch.empty_like(images)
     _check(lib().jt_psf_convolve_batch(code, B, ny, nx, _ptr(images), ky, kx, _ptr(kernel), _METHODS[method], _ptr(ws),
@@ -343,7 +347,7 @@ def simulate_image(grid, sie, shear, tnfw, sources, psf, dtype=None, method="aut
         device = psf.device
     elif tnfw is not None:
         device = tnfw.device
-    ws, wsb = _workspace(simulate_image_workspace_bytes(code, grid, L.n_tnfw, ky, kx, method), device, workspace)
+    ws, wsb = _workspace(simulate_image_workspace_bytes(code, grid, L.n_tnfw, ky, kx, method), device, workspace, stream)
     if out is None:
         out = torch.empty((grid.ny, grid.nx), dtype=_torch_dtype(code), device=device)
     _check(lib().jt_simulate_image(code, ctypes.byref(g), ctypes.byref(L), ctypes.byref(S), ky, kx, _ptr(psf),

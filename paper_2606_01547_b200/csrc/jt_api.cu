@@ -12,8 +12,9 @@ void count_launch() { ++g_launches; }
 // ---- profiling events (jt_profile_enable / jt_profile_read) ----
 struct ProfileState {
     bool on = false, recorded = false, had_conv = false;
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
-    void* tiers = nullptr;             // device: four uint64 counters in the last profiled call's workspace
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};      // start, after trace, after conv, after the counter copy
+    uint64_t* host_tiers = nullptr;    // pinned host copy of the last profiled call's four tier counters
+    bool have_tiers = false;
 };
 static thread_local ProfileState g_prof;
 
@@ -205,34 +206,57 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
     cudaStream_t st = (cudaStream_t)stream;
     const bool prof = g_prof.on;
     if (prof) { g_prof.recorded = false; JT_CUDA_TRY(cudaEventRecord(g_prof.ev[0], st)); }
+    // profiling: the kernel's tier counters (in the workspace) are copied to the library's pinned buffer right behind
+    // the kernel, so nothing points into the caller's workspace once the call returns
+    auto fetch_tiers = [&]() -> jt_status {
+        JT_CUDA_TRY(cudaMemcpyAsync(g_prof.host_tiers, trace_tier_counters(plan, trace_ws), 4 * sizeof(uint64_t),
+                                    cudaMemcpyDeviceToHost, st));
+        g_prof.have_tiers = true;
+        return JT_OK;
+    };
     if (!conv) {
-        if (prof) g_prof.tiers = trace_tier_counters(plan, trace_ws);
         s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, out, prof, st);
-        if (s == JT_OK && prof) { JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st)); g_prof.had_conv = false; g_prof.recorded = true; }
+        if (s == JT_OK && prof) {
+            JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st));
+            s = fetch_tiers();
+            if (s == JT_OK) JT_CUDA_TRY(cudaEventRecord(g_prof.ev[3], st));
+            g_prof.had_conv = false;
+            g_prof.recorded = s == JT_OK;
+        }
         return s;
     }
     void* pre = ws + align_up(plan.total_bytes, 256);
     void* conv_ws_ptr = (char*)pre + align_up((size_t)grid->nx * grid->ny * dtype_size(dtype), 256);
-    if (prof) g_prof.tiers = trace_tier_counters(plan, trace_ws);
     s = launch_trace_grid(dtype, grid, lens, S, plan, trace_ws, pre, prof, st);
     if (s != JT_OK) return s;
     if (prof) JT_CUDA_TRY(cudaEventRecord(g_prof.ev[1], st));
     s = conv_dispatch(dtype, 1, grid->ny, grid->nx, pre, ky, kx, kernel, method, conv_ws_ptr, out, st);
-    if (s == JT_OK && prof) { JT_CUDA_TRY(cudaEventRecord(g_prof.ev[2], st)); g_prof.had_conv = true; g_prof.recorded = true; }
+    if (s == JT_OK && prof) {
+        JT_CUDA_TRY(cudaEventRecord(g_prof.ev[2], st));
+        s = fetch_tiers();
+        // a fourth record so that jt_profile_tiers can wait for the copy without a device-wide synchronisation
+        if (s == JT_OK) JT_CUDA_TRY(cudaEventRecord(g_prof.ev[3], st));
+        g_prof.had_conv = true;
+        g_prof.recorded = s == JT_OK;
+    }
     return s;
 }
 
 // ------------------------------------------------------------------ profiling
 jt_status jt_profile_enable(int on) {
     if (on && !g_prof.on) {
-        for (int i = 0; i < 3; ++i) JT_CUDA_TRY(cudaEventCreate(&g_prof.ev[i]));
+        for (int i = 0; i < 4; ++i) JT_CUDA_TRY(cudaEventCreate(&g_prof.ev[i]));
+        JT_CUDA_TRY(cudaHostAlloc((void**)&g_prof.host_tiers, 4 * sizeof(uint64_t), cudaHostAllocDefault));
         g_prof.on = true;
         g_prof.recorded = false;
+        g_prof.have_tiers = false;
     } else if (!on && g_prof.on) {
-        for (int i = 0; i < 3; ++i) { cudaEventDestroy(g_prof.ev[i]); g_prof.ev[i] = nullptr; }
+        for (int i = 0; i < 4; ++i) { cudaEventDestroy(g_prof.ev[i]); g_prof.ev[i] = nullptr; }
+        cudaFreeHost(g_prof.host_tiers);
+        g_prof.host_tiers = nullptr;
         g_prof.on = false;
         g_prof.recorded = false;
-        g_prof.tiers = nullptr;
+        g_prof.have_tiers = false;
     }
     return JT_OK;
 }
@@ -247,9 +271,9 @@ jt_status jt_profile_read(float* trace_ms, float* conv_ms) {
 }
 
 jt_status jt_profile_tiers(uint64_t* counts) {
-    if (!g_prof.on || !g_prof.recorded || !g_prof.tiers || !counts) return JT_ERR_INVALID_VALUE;
-    JT_CUDA_TRY(cudaEventSynchronize(g_prof.ev[g_prof.had_conv ? 2 : 1]));
-    JT_CUDA_TRY(cudaMemcpy(counts, g_prof.tiers, 4 * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+    if (!g_prof.on || !g_prof.recorded || !g_prof.have_tiers || !counts) return JT_ERR_INVALID_VALUE;
+    JT_CUDA_TRY(cudaEventSynchronize(g_prof.ev[3]));
+    for (int k = 0; k < 4; ++k) counts[k] = g_prof.host_tiers[k];
     return JT_OK;
 }
 

@@ -33,7 +33,7 @@ struct BatchArgs {
 
 template <typename T, int R>
 __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch(const __grid_constant__ BatchArgs<T> a) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(32) unsigned char smem_raw[];      // SubRec<double> is 32-byte aligned
     __shared__ MacroLens s_m;
     __shared__ SrcSet s_src;
     __shared__ unsigned short s_queue[kTraceThreads / 32][kBatchRecCap];
@@ -155,7 +155,11 @@ static size_t batch_smem_front(const BatchArgs<T>& a) {
 #define JT_BATCH_CASE(RR)                                                                              \
     case RR: {                                                                                         \
         auto kern = k_batch<T, RR>;                                                                    \
-        JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        static bool attr_set = false;   /* once per instantiation: allow the full dynamic shared memory */ \
+        if (!attr_set) {                                                                               \
+            JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBatchMaxSmem)); \
+            attr_set = true;                                                                           \
+        }                                                                                              \
         kern<<<(unsigned)B, kTraceThreads, smem, st>>>(a);                                             \
         break;                                                                                         \
     }
@@ -180,8 +184,11 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     constexpr int kBatchOY = BatchOY<T>::value;
     a.kyp = (a.ky + kBatchOY - 1) / kBatchOY * kBatchOY;
     constexpr int TH = (kTraceThreads / 32) * kBatchOY;
-    a.pw = conv ? (g->nx + kBatchTW - 1) / kBatchTW * kBatchTW + a.kx - 1 : 0;        // even: pair loads stay aligned
-    a.ph = conv ? (g->ny + TH - 1) / TH * TH + a.kyp - 1 : 0;
+    const int64_t pw64 = conv ? ((int64_t)g->nx + kBatchTW - 1) / kBatchTW * kBatchTW + a.kx - 1 : 0;   // even: pair loads stay aligned
+    const int64_t ph64 = conv ? ((int64_t)g->ny + TH - 1) / TH * TH + a.kyp - 1 : 0;
+    if (pw64 * ph64 * (int64_t)sizeof(T) > (int64_t)kBatchMaxSmem) return JT_ERR_UNSUPPORTED;   // before any int arithmetic on it
+    a.pw = (int)pw64;
+    a.ph = (int)ph64;
     a.img_elems = (a.pw * a.ph + 3) / 4 * 4;
     a.rec_cap = a.M < BatchRecCap<T>::value ? (a.M > 0 ? a.M : 1) : BatchRecCap<T>::value;
     a.sie = (const T*)p->sie; a.shear = (const T*)p->shear; a.tnfw = (const T*)p->tnfw;

@@ -507,7 +507,11 @@ jt_status launch_trace_t(const TraceArgs<T>& a, int R, cudaStream_t st);
     case RR: {                                                                                    \
         auto kern = k_trace<T, RR, GRID>;                                                         \
         const size_t dsm = dacc_smem_bytes<T, RR>() + (size_t)a.tile_recs * (sizeof(SubRec<T>) + (kTraceThreads / 32) * 2); \
-        JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));   \
+        static bool attr_set = false;   /* once per instantiation: allow the full dynamic shared memory */ \
+        if (!attr_set) {                                                                          \
+            JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024)); \
+            attr_set = true;                                                                      \
+        }                                                                                         \
         kern<<<(unsigned)grid, kTraceThreads, dsm, st>>>(a);                                      \
         break;                                                                                    \
     }

@@ -68,7 +68,7 @@ def test_argument_validation_without_device(jt):
     assert L.jt_psf_convolve_batch(1, ctypes.c_int64(0), 64, 64, None, 21, 21, None, 1, None, 0, None, None) == 0     # B = 0: no-op
     assert L.jt_psf_convolve_batch(1, ctypes.c_int64(-1), 64, 64, dummy, 21, 21, dummy, 1, None, 0, ctypes.c_void_p(512), None) == 1
     need = L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, 2)
-    assert need >= 128 * 128 * 16
+    assert need >= (64 + 64 + 21) * (84 // 2 + 1) * 16        # three half-spectrum planes of the 84 x 84 padded transform
     assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 2, dummy, need - 1, ctypes.c_void_p(512), None) == 3
     assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 2, None, 0, ctypes.c_void_p(512), None) == 3
     # zero-sized problems are no-ops
