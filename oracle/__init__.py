@@ -26,11 +26,12 @@ _dp = ctypes.POINTER(ctypes.c_double)
 
 def build(force=False):
     """Compile oracle.c -> liboracle.so with gcc (-O2, no fast-math; OpenMP on the outer loops only)."""
+    srcs = [_SRC, os.path.join(os.path.dirname(_SRC), "oracle_next.c")]
     if (not force and os.path.exists(_LIB_PATH)
-            and os.path.getmtime(_LIB_PATH) >= os.path.getmtime(_SRC)):
+            and all(os.path.getmtime(_LIB_PATH) >= os.path.getmtime(f) for f in srcs)):
         return _LIB_PATH
     cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-           "-o", _LIB_PATH, _SRC, "-lm"]
+           "-o", _LIB_PATH] + srcs + ["-lm"]
     subprocess.run(cmd, check=True)
     return _LIB_PATH
 
@@ -82,6 +83,16 @@ def lib():
                                          _i, _i, _dp, _dp, _dp]
         L.orc_simulate_batch.argtypes = [_i64, _i, _i, _d, _d, _d, _i, _dp, _dp, _i64, _dp, _i, _dp,
                                          _i, _i, _dp, _dp]
+        _i32p = ctypes.POINTER(ctypes.c_int32)
+        L.orc_chi2_batch.argtypes = [_i64, _i64, _dp, _dp, _dp, _dp]
+        L.orc_lensing_maps.argtypes = [_i64, _dp, _dp, _dp, _dp, _i64, _dp, _dp, _dp, _dp, _dp]
+        L.orc_profile_alpha.argtypes = [_i, _dp, _d, _d, _dp, _dp]
+        L.orc_profile_kappa.argtypes = [_i, _dp, _d, _d]
+        L.orc_profile_kappa.restype = _d
+        L.orc_ray_shoot_profiles.argtypes = [_i64, _dp, _dp, _i64, _i32p, _dp, _dp, _dp]
+        L.orc_light.argtypes = [_i, _dp, _d, _d]
+        L.orc_light.restype = _d
+        L.orc_light_profiles.argtypes = [_i64, _dp, _dp, _i64, _i32p, _dp, _dp]
         _lib = L
     return _lib
 
@@ -270,3 +281,82 @@ def simulate_batch(bw, systems=None):
                              _ptr(sie), _ptr(shear), tnfw.shape[2], _ptr(tnfw), src.shape[1], _ptr(src),
                              psf.shape[1], psf.shape[2], _ptr(psf), _ptr(out))
     return out
+
+
+def chi2_batch(models, data, sigma):
+    """chi2[b] = sum_pixels ((models[b] - data) / sigma)^2 (reading Q24; PAPER.md:120-126 swarm inner loop)."""
+    m = _arr(models)
+    d = _arr(data)
+    sg = _arr(sigma)
+    m = m.reshape(-1, d.size)
+    out = np.empty(m.shape[0])
+    lib().orc_chi2_batch(m.shape[0], d.size, _ptr(m), _ptr(d), _ptr(sg), _ptr(out))
+    return out
+
+
+# ------------------------------------------------------------------ SURVEY section 8(f) rows (oracle_next.c)
+DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7}
+LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
+
+
+def _typed(records, table):
+    """[(name, [params...]), ...] -> (int32 types [n], float64 params [n][8])"""
+    types = np.array([table[name] for name, _ in records], dtype=np.int32)
+    params = np.zeros((len(records), 8))
+    for k, (_, p) in enumerate(records):
+        params[k, :len(p)] = p
+    return types, params
+
+
+def lensing_maps(theta_x, theta_y, sie=None, shear=None, tnfw=None):
+    """(kappa, gamma1, gamma2, mu) of SIE + shear + TNFW at the given points (NEXT-2)."""
+    tx = _arr(theta_x).ravel()
+    ty = _arr(theta_y).ravel()
+    sie_a, shear_a, tn = _lens_args(sie, shear, tnfw)
+    out = [np.empty_like(tx) for _ in range(4)]
+    lib().orc_lensing_maps(tx.size, _ptr(tx), _ptr(ty), _ptr(sie_a), _ptr(shear_a), tn.shape[1], _ptr(tn),
+                           *[_ptr(o) for o in out])
+    return tuple(out)
+
+
+def profile_alpha(name, params, x, y):
+    p = np.zeros(8)
+    p[:len(params)] = params
+    ax, ay = ctypes.c_double(), ctypes.c_double()
+    lib().orc_profile_alpha(DEFLECTOR_TYPES[name], _ptr(p), float(x), float(y), ctypes.byref(ax), ctypes.byref(ay))
+    return ax.value, ay.value
+
+
+def profile_kappa(name, params, x, y):
+    p = np.zeros(8)
+    p[:len(params)] = params
+    return lib().orc_profile_kappa(DEFLECTOR_TYPES[name], _ptr(p), float(x), float(y))
+
+
+def ray_shoot_profiles(theta_x, theta_y, deflectors):
+    """beta = theta - sum of the typed deflectors [(name, params), ...] (NEXT-1)."""
+    tx = _arr(theta_x).ravel()
+    ty = _arr(theta_y).ravel()
+    types, params = _typed(deflectors, DEFLECTOR_TYPES)
+    bx, by = np.empty_like(tx), np.empty_like(ty)
+    lib().orc_ray_shoot_profiles(tx.size, _ptr(tx), _ptr(ty), len(types), types.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                                 _ptr(params), _ptr(bx), _ptr(by))
+    return bx, by
+
+
+def light(name, params, x, y):
+    p = np.zeros(8)
+    p[:len(params)] = params
+    return lib().orc_light(LIGHT_TYPES[name], _ptr(p), float(x), float(y))
+
+
+def light_profiles(beta_x, beta_y, components):
+    """sum of typed light components [(name, params), ...] at (beta_x, beta_y) (NEXT-1)."""
+    bx = _arr(beta_x).ravel()
+    by = _arr(beta_y).ravel()
+    types, params = _typed(components, LIGHT_TYPES)
+    out = np.empty_like(bx)
+    lib().orc_light_profiles(bx.size, _ptr(bx), _ptr(by), len(types), types.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                             _ptr(params), _ptr(out))
+    return out
+

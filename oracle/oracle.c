@@ -340,3 +340,20 @@ void orc_simulate_batch(int64_t B, int nx, int ny, double pixel_scale, double gc
     }
     free(pre);
 }
+
+/* ------------------------------------------------------------------ chi^2 of B model images against one data image
+ * NEXT-3 (the particle-swarm benchmark: every particle is one simulated image
+ * compared with the same data).  The paper prints no likelihood formula; reading Q24: Gaussian pixel noise,
+ *   chi2[b] = sum_{j,i} ( (model[b][j][i] - data[j][i]) / sigma[j][i] )^2 ,   log L = -chi2 / 2,
+ * sigma = the per-pixel noise rms map (> 0).  Plain double loop in row-major order. */
+void orc_chi2_batch(int64_t B, int64_t n_pix, const double *models, const double *data, const double *sigma, double *chi2) {
+    for (int64_t b = 0; b < B; ++b) {
+        double acc = 0.0;
+        for (int64_t p = 0; p < n_pix; ++p) {
+            const double r = (models[b * n_pix + p] - data[p]) / sigma[p];
+            acc += r * r;
+        }
+        chi2[b] = acc;
+    }
+}
+
