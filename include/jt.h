@@ -161,6 +161,58 @@ typedef struct {
 JT_API jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid *grid, const jt_batch_params *params,
                             void *out, void *stream);
 
+/* ---------------------------------------------------------------------------------------------------------------
+ * SURVEY.md section 8(f) rows beside the hot path.  Correct-first kernels: parity with the oracle and a measured rate,
+ * not tier-tuned like the subhalo sum.
+ * --------------------------------------------------------------------------------------------------------------- */
+
+/* NEXT-3 (the particle-swarm benchmark evaluates every particle's simulated image against the same
+ * data).  Reading Q24: chi2[b] = sum over pixels of ((model[b] - data) / sigma)^2, log-likelihood = -chi2 / 2.
+ * models: device [B][ny][nx]; data, sigma (noise rms, > 0): device [ny][nx], all of the call's dtype.
+ * chi2: device [B], ALWAYS double.  One thread block per image, fixed summation order (deterministic). */
+JT_API jt_status jt_chi2_batch(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, const void *models, const void *data,
+                        const void *sigma, double *chi2, void *stream);
+/* jt_simulate_batch with the chi^2 against (data, sigma) accumulated by the same thread block that forms the image,
+ * so a swarm step returns B doubles instead of B images.  images: device [B][ny][nx] or NULL (images not wanted).
+ * chi2: device [B] double.  Same limits as jt_simulate_batch. */
+JT_API jt_status jt_simulate_batch_chi2(jt_dtype dtype, int64_t B, const jt_grid *grid, const jt_batch_params *params,
+                                 const void *data, const void *sigma, void *images, double *chi2, void *stream);
+
+/* NEXT-2 (the paper differentiates by autodiff; reading Q25 writes the derivatives out).  Jacobian of
+ * the lens equation A = d beta / d theta = I - H at caller-supplied points, for the hot path's deflectors:
+ * kappa = (H_xx + H_yy)/2, gamma1 = (H_xx - H_yy)/2, gamma2 = H_xy, mu = 1/((1 - kappa)^2 - gamma1^2 - gamma2^2).
+ * theta_x, theta_y: device [n] (in); kappa, gamma1, gamma2, mu: device [n] (out), any of them may be NULL.
+ * A point exactly on a deflector's centre gets no contribution from that deflector. */
+JT_API jt_status jt_lensing_maps(jt_dtype dtype, int64_t n, const void *theta_x, const void *theta_y, const jt_lens *lens,
+                          void *kappa, void *gamma1, void *gamma2, void *mu, void *stream);
+
+/* NEXT-1 (PAPER.md:63-87 deflector table, :95-108 light table): typed profile lists.  A record is a type and up to
+ * eight double parameters; the lists are DEVICE arrays of jt_profile (72 bytes each), whatever the call's dtype.
+ *   deflectors                          p[]
+ *   JT_DEFL_CONVERGENCE   kappa, cx, cy                 alpha = kappa (theta - c)
+ *   JT_DEFL_SIS         (:86)           theta_E, cx, cy
+ *   JT_DEFL_NFW         (:81)           Rs, alpha_Rs, cx, cy          alpha_Rs = deflection at Rs
+ *   JT_DEFL_HERNQUIST   (:71)           Rs, sigma0, cx, cy            sigma0 = rho0 Rs
+ *   JT_DEFL_PJAFFE      (:83)           sigma0, Ra, Rs, cx, cy
+ *   JT_DEFL_SIE         (:80)           theta_E, e1, e2, cx, cy       definition S
+ *   JT_DEFL_SHEAR       (:85)           gamma1, gamma2                definition H
+ *   JT_DEFL_TNFW        (:87)           Rs, alpha_Rs, r_trunc, cx, cy definition T
+ *   light
+ *   JT_LIGHT_SERSIC_ELLIPSE   (:103)    amp, R_sersic, n_sersic, e1, e2, cx, cy      definition R
+ *   JT_LIGHT_GAUSSIAN_ELLIPSE (:98-101) amp (total flux), sigma, e1, e2, cx, cy; GAUSSIAN is e1 = e2 = 0,
+ *                                       MULTI_GAUSSIAN(_ELLIPSE) is several records
+ * Formulas: DESIGN.md readings Q26-Q30.  Unknown types contribute nothing. */
+typedef enum { JT_DEFL_CONVERGENCE = 0, JT_DEFL_SIS = 1, JT_DEFL_NFW = 2, JT_DEFL_HERNQUIST = 3, JT_DEFL_PJAFFE = 4,
+               JT_DEFL_SIE = 5, JT_DEFL_SHEAR = 6, JT_DEFL_TNFW = 7 } jt_deflector_type;
+typedef enum { JT_LIGHT_SERSIC_ELLIPSE = 0, JT_LIGHT_GAUSSIAN_ELLIPSE = 1 } jt_light_type;
+typedef struct { int32_t type; int32_t reserved; double p[8]; } jt_profile;
+/* beta = theta - sum of the n_def deflectors.  theta, beta: device [n]; deflectors: device [n_def]. */
+JT_API jt_status jt_ray_shoot_profiles(jt_dtype dtype, int64_t n, const void *theta_x, const void *theta_y, int64_t n_def,
+                                const jt_profile *deflectors, void *beta_x, void *beta_y, void *stream);
+/* flux[i] = sum of the n_comp light components at (beta_x[i], beta_y[i]) (surface brightness). */
+JT_API jt_status jt_light_profiles(jt_dtype dtype, int64_t n, const void *beta_x, const void *beta_y, int64_t n_comp,
+                            const jt_profile *components, void *flux, void *stream);
+
 /* Measurement aid (bench.py's roofline leg).  jt_profile_enable(1) makes every following
  * jt_simulate_image call on this host thread record CUDA events on its stream before the ray-tracing kernel, between it
  * and the convolution, and after the convolution, and copy the kernel's four tier counters (32 bytes) to a pinned host

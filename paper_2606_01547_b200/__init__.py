@@ -6,6 +6,14 @@ There is no CPU fallback: calls raise if libjt.so is missing or no sm_100 device
 """
 from .binding import (  # noqa: F401
     Grid,
+    chi2_batch,
+    simulate_batch_chi2,
+    lensing_maps,
+    ray_shoot_profiles,
+    light_profiles,
+    profile_records,
+    DEFLECTOR_TYPES,
+    LIGHT_TYPES,
     JtError,
     lib,
     kernel_launches,

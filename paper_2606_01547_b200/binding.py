@@ -101,6 +101,13 @@ def lib():
         L.jt_simulate_image.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), ctypes.POINTER(_Lens),
                                         ctypes.POINTER(_Sources), i32, i32, vp, ctypes.c_int, vp, sz, vp, vp]
         L.jt_simulate_batch.argtypes = [ctypes.c_int, i64, ctypes.POINTER(_Grid), ctypes.POINTER(_Batch), vp, vp]
+        dbl = ctypes.POINTER(ctypes.c_double)
+        L.jt_chi2_batch.argtypes = [ctypes.c_int, i64, i32, i32, vp, vp, vp, vp, vp]
+        L.jt_simulate_batch_chi2.argtypes = [ctypes.c_int, i64, ctypes.POINTER(_Grid), ctypes.POINTER(_Batch), vp, vp, vp, vp, vp]
+        L.jt_lensing_maps.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Lens), vp, vp, vp, vp, vp]
+        L.jt_ray_shoot_profiles.argtypes = [ctypes.c_int, i64, vp, vp, i64, vp, vp, vp, vp]
+        L.jt_light_profiles.argtypes = [ctypes.c_int, i64, vp, vp, i64, vp, vp, vp]
+        del dbl
         L.jt_kernel_launches.restype = ctypes.c_uint64
         L.jt_profile_enable.argtypes = [ctypes.c_int]
         L.jt_profile_read.argtypes = [ctypes.POINTER(ctypes.c_float), ctypes.POINTER(ctypes.c_float)]
@@ -356,11 +363,9 @@ def simulate_image(grid, sie, shear, tnfw, sources, psf, dtype=None, method="aut
     return out
 
 
-def simulate_batch(grid, sie, shear, tnfw, sersic, psf, out=None, stream=None):
-    """jt_simulate_batch: B independent systems.  sie [B][5], shear [B][2], tnfw [B][5][M], sersic [B][n][7], psf [B][ky][kx]."""
+def _batch_struct(sie, shear, tnfw, sersic, psf):
     _dev(sie, "sie"), _dev(shear, "shear")
     code = _dt(sie)
-    B = sie.shape[0]
     P = _Batch()
     P.sie, P.shear = sie.data_ptr(), shear.data_ptr()
     if tnfw is not None and tnfw.numel() > 0:
@@ -375,9 +380,99 @@ def simulate_batch(grid, sie, shear, tnfw, sersic, psf, out=None, stream=None):
     for t in (shear, tnfw, sersic, psf):
         if t is not None and t.numel() > 0 and _dt(t) != code:
             raise TypeError("all batch tensors must share one dtype")
+    return code, P
+
+
+def simulate_batch(grid, sie, shear, tnfw, sersic, psf, out=None, stream=None):
+    """jt_simulate_batch: B independent systems.  sie [B][5], shear [B][2], tnfw [B][5][M], sersic [B][n][7], psf [B][ky][kx]."""
+    code, P = _batch_struct(sie, shear, tnfw, sersic, psf)
+    B = sie.shape[0]
     g = grid._c()
     if out is None:
         out = torch.empty((B, grid.ny, grid.nx), dtype=_torch_dtype(code), device=sie.device)
     _check(lib().jt_simulate_batch(code, B, ctypes.byref(g), ctypes.byref(P), _ptr(out), _stream(stream)),
            "jt_simulate_batch")
     return out
+
+
+# ------------------------------------------------------------------ SURVEY section 8(f) rows
+def chi2_batch(models, data, sigma, out=None, stream=None):
+    """jt_chi2_batch: chi2[b] = sum ((models[b] - data) / sigma)^2 as a float64 tensor [B]."""
+    _dev(models, "models"), _dev(data, "data"), _dev(sigma, "sigma")
+    code = _dt(models)
+    if _dt(data) != code or _dt(sigma) != code:
+        raise TypeError("models, data and sigma must share one dtype")
+    B, ny, nx = models.shape
+    if out is None:
+        out = torch.empty(B, dtype=torch.float64, device=models.device)
+    _check(lib().jt_chi2_batch(code, B, ny, nx, _ptr(models), _ptr(data), _ptr(sigma), _ptr(out), _stream(stream)), "jt_chi2_batch")
+    return out
+
+
+def simulate_batch_chi2(grid, sie, shear, tnfw, sersic, psf, data, sigma, images=False, chi2=None, stream=None):
+    """jt_simulate_batch_chi2: the batch kernel with the chi^2 against (data, sigma) accumulated in the same thread block.
+    Returns chi2 [B] (float64), or (chi2, images) with images=True / an images tensor."""
+    code, P = _batch_struct(sie, shear, tnfw, sersic, psf)
+    _dev(data, "data"), _dev(sigma, "sigma")
+    if _dt(data) != code or _dt(sigma) != code:
+        raise TypeError("data and sigma must have the batch's dtype")
+    B = sie.shape[0]
+    g = grid._c()
+    img = None
+    if images is True:
+        img = torch.empty((B, grid.ny, grid.nx), dtype=_torch_dtype(code), device=sie.device)
+    elif isinstance(images, torch.Tensor):
+        img = images
+    if chi2 is None:
+        chi2 = torch.empty(B, dtype=torch.float64, device=sie.device)
+    _check(lib().jt_simulate_batch_chi2(code, B, ctypes.byref(g), ctypes.byref(P), _ptr(data), _ptr(sigma), _ptr(img), _ptr(chi2),
+                                        _stream(stream)), "jt_simulate_batch_chi2")
+    return chi2 if img is None else (chi2, img)
+
+
+def lensing_maps(theta_x, theta_y, sie=None, shear=None, tnfw=None, stream=None):
+    """jt_lensing_maps: (kappa, gamma1, gamma2, mu) of SIE + shear + TNFW at the given points."""
+    _dev(theta_x, "theta_x"), _dev(theta_y, "theta_y")
+    code = _dt(theta_x)
+    L = _lens(code, sie, shear, tnfw)
+    out = [torch.empty_like(theta_x) for _ in range(4)]
+    _check(lib().jt_lensing_maps(code, theta_x.numel(), _ptr(theta_x), _ptr(theta_y), ctypes.byref(L), _ptr(out[0]), _ptr(out[1]),
+                                 _ptr(out[2]), _ptr(out[3]), _stream(stream)), "jt_lensing_maps")
+    return tuple(out)
+
+
+DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7}
+LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
+_PROFILE_DT = np.dtype([("type", np.int32), ("reserved", np.int32), ("p", np.float64, 8)])     # jt_profile, 72 bytes
+
+
+def profile_records(records, table, device="cuda"):
+    """[(name, [params...]), ...] -> device array of jt_profile (a uint8 tensor of 72-byte records)."""
+    a = np.zeros(len(records), dtype=_PROFILE_DT)
+    for k, (name, p) in enumerate(records):
+        a[k]["type"] = table[name]
+        a[k]["p"][:len(p)] = p
+    return torch.as_tensor(a.view(np.uint8).reshape(-1).copy(), device=device)
+
+
+def ray_shoot_profiles(theta_x, theta_y, deflectors, stream=None):
+    """jt_ray_shoot_profiles: beta = theta - sum of typed deflectors [(name, params), ...] (or a profile_records tensor)."""
+    _dev(theta_x, "theta_x"), _dev(theta_y, "theta_y")
+    code = _dt(theta_x)
+    recs = deflectors if isinstance(deflectors, torch.Tensor) else profile_records(deflectors, DEFLECTOR_TYPES, theta_x.device)
+    bx, by = torch.empty_like(theta_x), torch.empty_like(theta_y)
+    _check(lib().jt_ray_shoot_profiles(code, theta_x.numel(), _ptr(theta_x), _ptr(theta_y), recs.numel() // 72,
+                                       _ptr(recs) if recs.numel() else None, _ptr(bx), _ptr(by), _stream(stream)),
+           "jt_ray_shoot_profiles")
+    return bx, by
+
+
+def light_profiles(beta_x, beta_y, components, stream=None):
+    """jt_light_profiles: sum of typed light components [(name, params), ...] at (beta_x, beta_y)."""
+    _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y")
+    code = _dt(beta_x)
+    recs = components if isinstance(components, torch.Tensor) else profile_records(components, LIGHT_TYPES, beta_x.device)
+    flux = torch.empty_like(beta_x)
+    _check(lib().jt_light_profiles(code, beta_x.numel(), _ptr(beta_x), _ptr(beta_y), recs.numel() // 72,
+                                   _ptr(recs) if recs.numel() else None, _ptr(flux), _stream(stream)), "jt_light_profiles")
+    return flux

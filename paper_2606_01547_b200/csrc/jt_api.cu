@@ -278,19 +278,75 @@ jt_status jt_profile_tiers(uint64_t* counts) {
 }
 
 // ------------------------------------------------------------------ batch
-jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid* grid, const jt_batch_params* p, void* out,
-                            void* stream) {
+static jt_status simulate_batch_impl(jt_dtype dtype, int64_t B, const jt_grid* grid, const jt_batch_params* p, void* out,
+                                     const void* data, const void* sigma, double* chi2, bool want_chi2, void* stream) {
     if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
     if (B < 0 || !valid_grid(grid) || !p) return JT_ERR_INVALID_VALUE;
     if (B == 0) return JT_OK;
-    if (!out || !p->sie || !p->shear || p->n_tnfw < 0 || (p->n_tnfw > 0 && !p->tnfw) || p->n_src < 0 ||
+    if ((!want_chi2 && !out) || !p->sie || !p->shear || p->n_tnfw < 0 || (p->n_tnfw > 0 && !p->tnfw) || p->n_src < 0 ||
         p->n_src > JT_MAX_SOURCES || (p->n_src > 0 && !p->sersic))
         return JT_ERR_INVALID_VALUE;
+    if (want_chi2 && (!data || !sigma || !chi2)) return JT_ERR_INVALID_VALUE;
     const bool conv = !(p->ky == 0 && p->kx == 0 && p->psf == nullptr);
     if (conv && (!valid_kernel_size(p->ky, p->kx) || !p->psf)) return JT_ERR_INVALID_VALUE;
     jt_status s = check_device();
     if (s != JT_OK) return s;
-    return launch_batch(dtype, B, grid, p, out, (cudaStream_t)stream);
+    return launch_batch(dtype, B, grid, p, out, data, sigma, chi2, (cudaStream_t)stream);
+}
+
+jt_status jt_simulate_batch(jt_dtype dtype, int64_t B, const jt_grid* grid, const jt_batch_params* p, void* out,
+                            void* stream) {
+    return simulate_batch_impl(dtype, B, grid, p, out, nullptr, nullptr, nullptr, false, stream);
+}
+
+// ------------------------------------------------------------------ SURVEY 8(f) rows
+jt_status jt_simulate_batch_chi2(jt_dtype dtype, int64_t B, const jt_grid* grid, const jt_batch_params* p, const void* data,
+                                 const void* sigma, void* images, double* chi2, void* stream) {
+    return simulate_batch_impl(dtype, B, grid, p, images, data, sigma, chi2, true, stream);
+}
+
+jt_status jt_chi2_batch(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, const void* models, const void* data,
+                        const void* sigma, double* chi2, void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (B < 0 || ny < 1 || nx < 1) return JT_ERR_INVALID_VALUE;
+    if (B == 0) return JT_OK;
+    if (!models || !data || !sigma || !chi2) return JT_ERR_INVALID_VALUE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_chi2(dtype, B, (int64_t)ny * nx, models, data, sigma, chi2, (cudaStream_t)stream);
+}
+
+jt_status jt_lensing_maps(jt_dtype dtype, int64_t n, const void* theta_x, const void* theta_y, const jt_lens* lens,
+                          void* kappa, void* gamma1, void* gamma2, void* mu, void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (n < 0 || !valid_lens(lens)) return JT_ERR_INVALID_VALUE;
+    if (n == 0) return JT_OK;
+    if (!theta_x || !theta_y) return JT_ERR_INVALID_VALUE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_lensing_maps(dtype, n, theta_x, theta_y, lens, kappa, gamma1, gamma2, mu, (cudaStream_t)stream);
+}
+
+jt_status jt_ray_shoot_profiles(jt_dtype dtype, int64_t n, const void* theta_x, const void* theta_y, int64_t n_def,
+                                const jt_profile* deflectors, void* beta_x, void* beta_y, void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (n < 0 || n_def < 0 || (n_def > 0 && !deflectors)) return JT_ERR_INVALID_VALUE;
+    if (n == 0) return JT_OK;
+    if (!theta_x || !theta_y || !beta_x || !beta_y || theta_x == beta_x || theta_y == beta_y) return JT_ERR_INVALID_VALUE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_ray_shoot_profiles(dtype, n, theta_x, theta_y, n_def, deflectors, beta_x, beta_y, (cudaStream_t)stream);
+}
+
+jt_status jt_light_profiles(jt_dtype dtype, int64_t n, const void* beta_x, const void* beta_y, int64_t n_comp,
+                            const jt_profile* components, void* flux, void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (n < 0 || n_comp < 0 || (n_comp > 0 && !components)) return JT_ERR_INVALID_VALUE;
+    if (n == 0) return JT_OK;
+    if (!beta_x || !beta_y || !flux || flux == beta_x || flux == beta_y) return JT_ERR_INVALID_VALUE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_light_profiles(dtype, n, beta_x, beta_y, n_comp, components, flux, (cudaStream_t)stream);
 }
 
 }  // extern "C"

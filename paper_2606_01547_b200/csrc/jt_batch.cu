@@ -28,7 +28,9 @@ struct BatchArgs {
     int rec_cap;
     int dacc_off;                            // byte offset of the DAcc columns (float mode), 16-byte aligned
     const T *sie, *shear, *tnfw, *sersic, *psf;
-    T* out;
+    T* out;                                  // [B][ny][nx] or nullptr (chi^2 only)
+    const T *data, *sigma;                   // chi^2 mode (jt_simulate_batch_chi2): [ny][nx] each, else nullptr
+    double* chi2;                            // [B]
 };
 
 template <typename T, int R>
@@ -77,7 +79,19 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     __syncthreads();
 
     // ---- ray tiles: steps 1-4 ----
-    T* gout = a.out + b * (int64_t)a.ny * a.nx;
+    T* gout = a.out ? a.out + b * (int64_t)a.ny * a.nx : nullptr;
+    double chi = 0.0;                              // this thread's share of chi^2 (NEXT-3), summed per block at the end
+    const T* cdata = a.data;
+    const T* csigma = a.sigma;
+    const int onx = a.nx;
+    auto emit = [&chi, gout, cdata, csigma, onx](int j, int i, T v) {       // a finished pixel of the final image
+        const int64_t p = (int64_t)j * onx + i;
+        if (gout) gout[p] = v;
+        if (cdata) {
+            const double r = ((double)v - (double)__ldg(&cdata[p])) / (double)__ldg(&csigma[p]);
+            chi = fma(r, r, chi);
+        }
+    };
     for (int tile = 0; tile < a.n_tiles; ++tile) {
         RayGeom g = {a.hh, a.cx, a.cy, a.NX, a.NY, a.NX, a.NY};     // idle warp: clamped coordinates, no stores
         const int wt = tile * (kTraceThreads / 32) + warp;
@@ -115,12 +129,11 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
             grid_epilogue<T, R>(s_m, s_src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
                                 [img, pw, hy, hx](int j, int i, double v) { img[(j + hy) * pw + (i + hx)] = (T)v; });
         } else {
-            const int nx = a.nx;
             grid_epilogue<T, R>(s_m, s_src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
-                                [gout, nx](int j, int i, double v) { gout[(int64_t)j * nx + i] = (T)v; });
+                                [&emit](int j, int i, double v) { emit(j, i, (T)v); });
         }
     }
-    if (!conv) return;
+    if (conv) {
     __syncthreads();
 
     // ---- step 5a out of shared memory: passes of 64 columns x 64 rows, OY x 2 outputs per thread ----
@@ -137,10 +150,22 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
             for (int r = 0; r < kBatchOY; ++r) {
                 const int j = j0 + warp * kBatchOY + r;
                 if (j < a.ny) {
-                    if (i < a.nx) gout[(int64_t)j * a.nx + i] = acc.col0(r);
-                    if (i + 1 < a.nx) gout[(int64_t)j * a.nx + i + 1] = acc.col1(r);
+                    if (i < a.nx) emit(j, i, acc.col0(r));
+                    if (i + 1 < a.nx) emit(j, i + 1, acc.col1(r));
                 }
             }
+        }
+    }
+    }
+    if (a.chi2 != nullptr) {                       // fixed summation tree: lanes, then the 8 warps in order
+        __shared__ double s_red[kTraceThreads / 32];
+        for (int o = 16; o > 0; o >>= 1) chi += __shfl_xor_sync(0xffffffffu, chi, o);
+        if (lane == 0) s_red[warp] = chi;
+        __syncthreads();
+        if (tid == 0) {
+            double tot = 0.0;
+            for (int w = 0; w < kTraceThreads / 32; ++w) tot += s_red[w];
+            a.chi2[b] = tot;
         }
     }
 }
@@ -166,7 +191,7 @@ static size_t batch_smem_front(const BatchArgs<T>& a) {
 
 template <typename T>
 static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
-                         cudaStream_t st) {
+                         const void* data, const void* sigma, double* chi2, cudaStream_t st) {
     if (B > 0x7fffffffLL) return JT_ERR_UNSUPPORTED;
     const TracePlan plan = plan_trace_grid(dtype, g, 0);
     BatchArgs<T> a = {};
@@ -194,6 +219,7 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.sie = (const T*)p->sie; a.shear = (const T*)p->shear; a.tnfw = (const T*)p->tnfw;
     a.sersic = (const T*)p->sersic; a.psf = (const T*)p->psf;
     a.out = (T*)out;
+    a.data = (const T*)data; a.sigma = (const T*)sigma; a.chi2 = chi2;
     a.dacc_off = (int)batch_smem_front(a);
     const size_t smem = (size_t)a.dacc_off + (sizeof(T) == 4 ? (size_t)plan.R * kTraceThreads * sizeof(double2) : 0);
     if (smem > kBatchMaxSmem) return JT_ERR_UNSUPPORTED;
@@ -207,8 +233,9 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
 }
 
 jt_status launch_batch(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
-                       cudaStream_t st) {
-    return dtype == JT_F32 ? batch_t<float>(dtype, B, g, p, out, st) : batch_t<double>(dtype, B, g, p, out, st);
+                       const void* data, const void* sigma, double* chi2, cudaStream_t st) {
+    return dtype == JT_F32 ? batch_t<float>(dtype, B, g, p, out, data, sigma, chi2, st)
+                           : batch_t<double>(dtype, B, g, p, out, data, sigma, chi2, st);
 }
 
 }  // namespace jt

@@ -71,8 +71,18 @@ size_t    fft_conv_workspace_bytes(jt_dtype dtype, int ny, int nx, int ky, int k
 jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
                           void* workspace, void* out, cudaStream_t st);
 
-// ---- batch (jt_batch.cu) ----
+// ---- batch (jt_batch.cu); data / sigma / chi2 non-null: chi^2 accumulated in the kernel, out may then be null ----
 jt_status launch_batch(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
-                       cudaStream_t st);
+                       const void* data, const void* sigma, double* chi2, cudaStream_t st);
+
+// ---- SURVEY 8(f) rows (jt_next.cu) ----
+jt_status launch_chi2(jt_dtype dtype, int64_t B, int64_t n_pix, const void* models, const void* data, const void* sigma,
+                      double* chi2, cudaStream_t st);
+jt_status launch_lensing_maps(jt_dtype dtype, int64_t n, const void* tx, const void* ty, const jt_lens* lens, void* kappa,
+                              void* gamma1, void* gamma2, void* mu, cudaStream_t st);
+jt_status launch_ray_shoot_profiles(jt_dtype dtype, int64_t n, const void* tx, const void* ty, int64_t n_def,
+                                    const jt_profile* defs, void* bx, void* by, cudaStream_t st);
+jt_status launch_light_profiles(jt_dtype dtype, int64_t n, const void* bx, const void* by, int64_t n_comp,
+                                const jt_profile* comps, void* flux, cudaStream_t st);
 
 }  // namespace jt

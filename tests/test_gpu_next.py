@@ -1,0 +1,160 @@
+"""GPU parity for the SURVEY.md section 8(f) rows (through the C ABI) against oracle/oracle_next.c:
+NEXT-3 chi^2 (standalone and fused into the batch kernel), NEXT-2 lensing maps, NEXT-1 typed profile lists."""
+import numpy as np
+import pytest
+
+import workloads
+from conftest import rel_err, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+def _f32r(a):
+    return np.asarray(a, dtype=np.float64).astype(np.float32).astype(np.float64)
+
+
+# ------------------------------------------------------------------ NEXT-3
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("B,ny,nx", [(1, 8, 8), (5, 100, 100), (64, 33, 47), (3, 257, 300)])
+def test_chi2_batch(jt, orc, dtype, B, ny, nx):
+    """jt_chi2_batch = the oracle's plain loop; includes image vs itself (0) and image + sigma (N pixels)."""
+    rng = np.random.default_rng(B * 7 + nx)
+    data = rng.uniform(1, 5, (ny, nx))
+    sigma = rng.uniform(0.05, 0.3, (ny, nx))
+    models = rng.uniform(1, 5, (B, ny, nx))
+    models[0] = data
+    if B > 1:
+        models[1] = data + sigma
+    if dtype == "f32":
+        data, sigma, models = _f32r(data), _f32r(sigma), _f32r(models)
+    got = jt.chi2_batch(to_dev(models, dtype), to_dev(data, dtype), to_dev(sigma, dtype)).cpu().numpy()
+    want = orc.chi2_batch(models, data, sigma)
+    assert got[0] == 0.0
+    assert np.max(np.abs(got - want)) <= 1e-12 * np.max(want)         # double accumulation on both sides, different order
+    if B > 1 and dtype == "f64":
+        assert abs(got[1] - ny * nx) < 1e-9 * ny * nx
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("conv", [True, False])
+def test_swarm_fused_chi2(jt, orc, dtype, conv):
+    """jt_simulate_batch_chi2 on the swarm shape (100x100 grid, 13-pixel PSF): chi^2 of every particle =
+    oracle chi^2 of the oracle's images; the images it optionally returns = jt_simulate_batch's; particle 0 (the truth)
+    against data = truth + noise gives the noise's own chi^2."""
+    w = workloads.config_swarm(B=12, dtype=dtype)
+    truth = orc.simulate_batch(w, systems=[0])[0] if conv else None
+    g = jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample)
+    d = lambda a: to_dev(a, dtype)
+    psf = d(w.psf) if conv else None
+    imgs = jt.simulate_batch(g, d(w.sie), d(w.shear), None, d(w.sources), psf)
+    want_imgs = imgs.double().cpu().numpy()
+    if not conv:
+        truth = want_imgs[0]
+    data = truth + w.data
+    if dtype == "f32":
+        data = _f32r(data)
+    chi, got_imgs = jt.simulate_batch_chi2(g, d(w.sie), d(w.shear), None, d(w.sources), psf, d(data), d(w.sigma), images=True)
+    assert np.array_equal(got_imgs.double().cpu().numpy(), want_imgs)
+    only = jt.simulate_batch_chi2(g, d(w.sie), d(w.shear), None, d(w.sources), psf, d(data), d(w.sigma))
+    assert np.array_equal(only.cpu().numpy(), chi.cpu().numpy())          # images not requested: same numbers
+    # against the oracle end to end: its images, its chi^2
+    orc_imgs = orc.simulate_batch(w) if conv else np.stack([orc.prepsf_rows(w.system(b)) for b in range(w.B)])
+    want = orc.chi2_batch(orc_imgs, data, w.sigma)
+    tol = 1e-8 if dtype == "f64" else 2e-2          # chi^2 amplifies image error by |residual| / sigma^2; float images carry ~1e-6
+    assert np.max(np.abs(chi.cpu().numpy() - want) / np.maximum(want, 1.0)) < tol
+    assert np.max(np.abs(chi.cpu().numpy() - orc.chi2_batch(want_imgs, data, w.sigma))) <= 1e-11 * np.max(want)
+    noise_chi2 = float(np.sum((w.data / w.sigma) ** 2))
+    assert abs(chi.cpu().numpy()[0] / noise_chi2 - 1.0) < (1e-6 if dtype == "f64" else 5e-3)
+
+
+# ------------------------------------------------------------------ NEXT-2
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_lensing_maps(jt, orc, dtype):
+    """kappa, gamma1, gamma2, mu of SIE + shear + 700 TNFW at 5000 points (incl. points at X = 1e-4 ... 30 around
+    subhalo centres) against the oracle's analytic Jacobian."""
+    rng = np.random.default_rng(31)
+    M = 700
+    tn = np.zeros((5, M))
+    tn[0], tn[1] = rng.uniform(-1.5, 1.5, M), rng.uniform(-1.5, 1.5, M)
+    tn[2] = np.exp(rng.uniform(np.log(0.005), np.log(0.05), M))
+    tn[3] = np.exp(rng.uniform(np.log(1e-4), np.log(1e-2), M))
+    tn[4] = tn[2] * np.exp(rng.uniform(np.log(0.5), np.log(20.0), M))
+    x, y = rng.uniform(-1.5, 1.5, 5000), rng.uniform(-1.5, 1.5, 5000)
+    Xs = np.logspace(-4, np.log10(30.0), 400)
+    ang = rng.uniform(0, 2 * np.pi, 400)
+    j = rng.integers(0, M, 400)
+    x[:400] = tn[0, j] + Xs * tn[2, j] * np.cos(ang)
+    y[:400] = tn[1, j] + Xs * tn[2, j] * np.sin(ang)
+    sie, shear = (1.1, 0.15, -0.1, 0.02, 0.01), (0.03, -0.02)
+    if dtype == "f32":
+        x, y, tn = _f32r(x), _f32r(y), _f32r(tn)
+        sie, shear = tuple(_f32r(sie)), tuple(_f32r(shear))
+    got = [t.double().cpu().numpy() for t in jt.lensing_maps(to_dev(x, dtype), to_dev(y, dtype), sie, shear, to_dev(tn, dtype))]
+    want = orc.lensing_maps(x, y, sie, shear, tn)
+    # double: definition T's closed form loses digits just above the series switch (brace ~ X^2 ln X from terms of size
+    # tau^2: relative error 3e-15 / (X^2 ln(2/X)) = 4e-10 at X = 1e-3) on BOTH sides independently; harmless for the
+    # deflection alpha = f R, but the mean convergence alpha / R that enters gamma keeps it (reading Q25)
+    tol = 5e-9 if dtype == "f64" else 3e-6
+    for name, g_, w_ in zip(("kappa", "gamma1", "gamma2"), got[:3], want[:3]):
+        assert np.max(np.abs(g_ - w_) / np.maximum(np.abs(w_), 1.0)) < tol, name
+        assert np.max(np.abs(g_[400:] - w_[400:]) / np.maximum(np.abs(w_[400:]), 1.0)) < (1e-11 if dtype == "f64" else 3e-6), name
+    ok = np.abs(want[3]) < 30
+    assert np.max(np.abs(got[3][ok] / want[3][ok] - 1.0)) < (1e-8 if dtype == "f64" else 2e-3)
+    # no subhalos, SIE only: |gamma| = kappa (closed form), through the kernel
+    k, g1, g2, _ = [t.double().cpu().numpy() for t in jt.lensing_maps(to_dev(x, dtype), to_dev(y, dtype), sie, None, None)]
+    assert np.max(np.abs(np.hypot(g1, g2) - k)) < (1e-13 if dtype == "f64" else 2e-6) * np.max(k)
+
+
+# ------------------------------------------------------------------ NEXT-1
+DEFLECTORS = [("CONVERGENCE", [0.07, 0.1, -0.2]), ("SIS", [1.2, 0.05, -0.1]), ("NFW", [0.3, 0.15, -0.1, 0.2]),
+              ("HERNQUIST", [0.4, 0.8, 0.1, 0.0]), ("PJAFFE", [0.9, 0.05, 0.6, -0.1, 0.1]),
+              ("SIE", [1.0, 0.1, -0.05, 0.0, 0.0]), ("SHEAR", [0.03, 0.01]), ("TNFW", [0.2, 0.1, 1.0, 0.8, 0.3])]
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_ray_shoot_profiles(jt, orc, dtype):
+    """Every deflector type alone and all together (plus 150 NFW subhalos: three staging rounds of the list), rays incl.
+    X = 1 +- 1e-7 of the NFW / Hernquist scale radii and a ray exactly on a centre."""
+    rng = np.random.default_rng(41)
+    x, y = rng.uniform(-2, 2, 3000), rng.uniform(-2, 2, 3000)
+    x[:6] = [-0.1 + 0.3 * (1 + e) for e in (-1e-7, 0.0, 1e-7)] + [0.1 + 0.4 * (1 + e) for e in (-1e-7, 0.0, 1e-7)]
+    y[:6] = [0.2, 0.2, 0.2, 0.0, 0.0, 0.0]
+    x[6], y[6] = 0.05, -0.1                                          # on the SIS centre
+    many = [("NFW", [float(r), float(a), float(cx), float(cy)]) for r, a, cx, cy in
+            zip(np.exp(rng.uniform(np.log(0.005), np.log(0.05), 150)), np.exp(rng.uniform(np.log(1e-4), np.log(1e-2), 150)),
+                rng.uniform(-2, 2, 150), rng.uniform(-2, 2, 150))]
+    lists = [[d] for d in DEFLECTORS] + [DEFLECTORS + many]
+    for defl in lists:
+        xx, yy, dd = x, y, defl
+        if dtype == "f32":
+            xx, yy = _f32r(x), _f32r(y)
+        bx, by = jt.ray_shoot_profiles(to_dev(xx, dtype), to_dev(yy, dtype), dd)
+        wx, wy = orc.ray_shoot_profiles(xx, yy, dd)
+        tol = 2e-13 if dtype == "f64" else 6e-7                      # float: storage of beta (|beta| up to ~3)
+        assert np.max(np.abs(bx.double().cpu().numpy() - wx)) < tol * (1 + len(dd) / 50), dd[0][0]
+        assert np.max(np.abs(by.double().cpu().numpy() - wy)) < tol * (1 + len(dd) / 50), dd[0][0]
+    # the hot path's three profiles through the typed list = jt_ray_shoot
+    tn = np.array([[0.8], [0.3], [0.2], [0.1], [1.0]])
+    a = jt.ray_shoot(to_dev(x, "f64"), to_dev(y, "f64"), (1.0, 0.1, -0.05, 0.0, 0.0), (0.03, 0.01), to_dev(tn, "f64"))
+    b = jt.ray_shoot_profiles(to_dev(x, "f64"), to_dev(y, "f64"), DEFLECTORS[5:])
+    assert float((a[0] - b[0]).abs().max()) < 2e-13 and float((a[1] - b[1]).abs().max()) < 2e-13
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_light_profiles(jt, orc, dtype):
+    """MULTI_GAUSSIAN_ELLIPSE (5 components) + a Sersic component, and 70 Gaussians (two staging rounds)."""
+    rng = np.random.default_rng(43)
+    bx, by = rng.uniform(-1, 1, 4000), rng.uniform(-1, 1, 4000)
+    mg = [("GAUSSIAN_ELLIPSE", [a, s, 0.2, -0.1, 0.05, 0.0]) for a, s in zip((1.0, 2.0, 0.5, 0.3, 1.2), (0.05, 0.1, 0.2, 0.4, 0.8))]
+    ser = [("SERSIC_ELLIPSE", [10.0, 0.2, 1.5, 0.05, 0.02, 0.05, 0.0])]
+    lots = [("GAUSSIAN_ELLIPSE", [1.0, 0.1 + 0.01 * k, 0.0, 0.0, 0.02 * k - 0.7, 0.1]) for k in range(70)]
+    if dtype == "f32":
+        bx, by = _f32r(bx), _f32r(by)
+    for comps in (mg, mg + ser, lots, ser):
+        got = jt.light_profiles(to_dev(bx, dtype), to_dev(by, dtype), comps).double().cpu().numpy()
+        want = orc.light_profiles(bx, by, comps)
+        assert rel_err(got, want) < (1e-13 if dtype == "f64" else 2e-7)
+    # Sersic through the typed list = jt_source_brightness
+    a = jt.source_brightness(to_dev(bx, "f64"), to_dev(by, "f64"), [ser[0][1]])
+    b = jt.light_profiles(to_dev(bx, "f64"), to_dev(by, "f64"), ser)
+    assert float((a - b).abs().max()) < 1e-12 * float(a.abs().max())

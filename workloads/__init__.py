@@ -10,6 +10,8 @@ The recipe follows BASELINE.json:configs[0..4] (0-based, named C0..C4).
 from .configs import (  # noqa: F401
     Workload,
     BatchWorkload,
+    SwarmWorkload,
+    config_swarm,
     config_c0,
     config_c1,
     config_c2,

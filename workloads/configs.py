@@ -216,6 +216,49 @@ def config_c3(B=4096, nx=64, supersample=2, n_tnfw=100, K=21, dtype="f32", seed_
     return w.as_dtype(dtype)
 
 
+@dataclass
+class SwarmWorkload(BatchWorkload):
+    """A particle swarm's inner loop: B parameter vectors, one data image and noise map."""
+    data: np.ndarray = None          # [ny][nx]
+    sigma: np.ndarray = None         # [ny][nx]
+
+    def as_dtype(self, dtype):
+        w = super().as_dtype(dtype)
+        if dtype == "f32":
+            w = replace(w, data=_f32_round(self.data), sigma=_f32_round(self.sigma))
+        return w
+
+
+def config_swarm(B=256, nx=100, K=13, supersample=1, dtype="f64", seed_offset=0):
+    """NEXT-3: the shape of the paper's particle-swarm benchmark, PAPER.md:122 -- a 100x100 grid
+    (0.05 arcsec pixels as in C1), a 13-pixel PSF (Gaussian FWHM 0.1 arcsec, the same for every particle), SIE + shear
+    mass model and one elliptical Sersic source per particle, no subhalos.  The particles are a seeded truth (C1 priors)
+    perturbed by 5 % Gaussian scatter; the data image is the pre-computed noise-free truth plus noise of rms sigma.
+    The paper's lens light and point source are outside the hot path.
+    `data` is filled by the caller (tests and bench.py form it with the oracle or with jt_simulate_batch on the truth,
+    which this module -- free of lensing arithmetic -- cannot do); `sigma` is a constant background rms."""
+    rng = np.random.default_rng(SEEDS["sweep"] + 77 + seed_offset)
+    truth_sie = np.array([rng.uniform(0.8, 1.5), rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), 0.0, 0.0])
+    truth_shear = rng.uniform(-0.05, 0.05, size=2)
+    truth_src = np.array([rng.uniform(5.0, 20.0), rng.uniform(0.1, 0.5), rng.uniform(0.5, 4.0), rng.uniform(-0.2, 0.2),
+                          rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2)])
+    jitter = lambda v, n: v[None, :] * (1.0 + 0.05 * rng.standard_normal((n, v.size))) + 0.01 * rng.standard_normal((n, v.size))
+    sie = jitter(truth_sie, B)
+    sie[0] = truth_sie                                   # particle 0 is the truth itself
+    shear = jitter(truth_shear, B)
+    shear[0] = truth_shear
+    src = jitter(truth_src, B)
+    src[0] = truth_src
+    src[:, 2] = np.clip(src[:, 2], 0.5, 4.0)
+    psf = np.broadcast_to(gaussian_psf(0.1, 0.05, K=K), (B, K, K)).copy()
+    sigma = np.full((nx, nx), 0.02)
+    noise = sigma * rng.standard_normal((nx, nx))
+    w = SwarmWorkload(name="swarm", dtype="f64", B=B, nx=nx, ny=nx, pixel_scale=0.05, supersample=supersample,
+                      sie=sie, shear=shear, tnfw=np.zeros((B, 5, 0)), sources=src[:, None, :], psf=psf,
+                      data=noise, sigma=sigma)           # data = truth image + this noise: the caller adds the truth
+    return w.as_dtype(dtype)
+
+
 def config_c4(nx=500, supersample=5, n_tnfw=50000, K=101, half_width=5.0, dtype="f64", seed_offset=0):
     """C4: 500x500 @0.02, supersampling 5, C0 macro-lens + 50,000 TNFW over 10x10, 3 Sersics, AiryMix(101)."""
     rng = np.random.default_rng(SEEDS["C4"] + seed_offset)
