@@ -40,7 +40,8 @@ SM_COUNT = 148
 # tier loop (loop head + body) divided by its 8 rays; f32: FP32-pipe lane operations (a packed FFMA2 / FMUL2 / FADD2
 # counts as two); f64: FP64-pipe instructions.  Order: far-far series, far form, mid form, cold path (counted as far).
 # The mix of tiers is measured per run with jt_profile_tiers.
-TIER_COST = {"f32": (14.5, 29.6, 47.0, 29.6), "f64": (25.2, 50.6, 80.0, 50.6)}
+TIER_COST = {"f32": (14.5, 14.5, 14.5, 29.6, 47.0, 29.6), "f64": (25.2, 25.2, 25.2, 50.6, 80.0, 50.6)}
+TIER_NAMES = ("far_far_long", "far_far_mid", "far_far_short", "far", "mid", "cold")
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu --set full captures in
 # profiles/r01d_ncu_{c2f64,c2f32,c3f32}.txt (the kernels are ALU-bound: compulsory traffic is parameters in, image out)
 NCU_TRAFFIC_BYTES = {"C2-f64": 483072 + 1126400, "C2-f32": 267008 + 510976, "C3-f32": 15798016 + 41087488}
@@ -412,7 +413,7 @@ def measure(torch, jt, name, args, rank, world, sample_clocks=False):
     launches0 = jt.kernel_launches()
 
     phase = []
-    tier_counts = (0, 0, 0, 0)
+    tier_counts = (0,) * len(TIER_NAMES)
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     for a, b in ev:
         flush.add_(1)
@@ -468,7 +469,7 @@ def measure(torch, jt, name, args, rank, world, sample_clocks=False):
     # tier mix of the (warp, subhalo record) pairs: counters of the last timed jt_simulate_image call; for the batch
     # kernel (no workspace, no counters) the same warp tiling is sampled through jt_simulate_image on 4 of its systems
     if batch:
-        tiers = np.zeros(4)
+        tiers = np.zeros(len(TIER_NAMES))
         jt.profile_enable(True)
         for b in range(min(4, w.B)):
             one = ImageRunner(jt, w.system(b), "direct")
@@ -478,7 +479,7 @@ def measure(torch, jt, name, args, rank, world, sample_clocks=False):
         jt.profile_enable(False)
     else:
         tiers = np.array(tier_counts, dtype=np.float64)
-    mix = tiers / tiers.sum() if tiers.sum() > 0 else np.array([0.0, 1.0, 0.0, 0.0])
+    mix = tiers / tiers.sum() if tiers.sum() > 0 else np.array([0.0, 0.0, 0.0, 1.0, 0.0, 0.0])
     n_alg = float(np.dot(mix, TIER_COST[w.dtype]))
     achieved = w.evals * n_alg / (trace_ms * 1e-3) / 1e12
     rec["roofline"] = {
@@ -487,8 +488,8 @@ def measure(torch, jt, name, args, rank, world, sample_clocks=False):
         "peak_kind": "derived: 148 SMs x %d lanes/clk (%s) x %.0f MHz (max clock, %s)" % (
             lanes, "FP32 pipe" if w.dtype == "f32" else "FP64 pipe", peaks.get("sm_max_mhz", 1965.0),
             peak_kind),
-        "alg_instr_per_eval": n_alg, "tier_mix": {"far_far": mix[0], "far": mix[1], "mid": mix[2], "cold": mix[3]},
-        "tier_cost_per_eval": dict(zip(("far_far", "far", "mid", "cold"), TIER_COST[w.dtype])), "kernel_ms": trace_ms, "conv_ms": conv_ms,
+        "alg_instr_per_eval": n_alg, "tier_mix": dict(zip(TIER_NAMES, (float(x) for x in mix))),
+        "tier_cost_per_eval": dict(zip(TIER_NAMES, TIER_COST[w.dtype])), "kernel_ms": trace_ms, "conv_ms": conv_ms,
         "kernel_share_of_step": trace_ms / (ms_total_local / args.steps),
         "frac_at_observed_clock": achieved / (SM_COUNT * lanes * f_mhz * 1e6 / 1e12),
         "evals_per_s_kernel": w.evals / (trace_ms * 1e-3)}

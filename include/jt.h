@@ -17,7 +17,7 @@
  *     returns, so the caller may free them immediately.
  *   - The caller owns every buffer, workspace included.  The library allocates no device memory.
  *     State it keeps between calls, all of it listed here: per host thread the last CUDA error code, the
- *     launch counter and -- only while jt_profile_enable(1) is in force -- four CUDA events and a 32-byte
+ *     launch counter and -- only while jt_profile_enable(1) is in force -- four CUDA events and a 48-byte
  *     pinned host buffer; per process one 60 KB __constant__ buffer per device (the taps of the direct
  *     convolution) with the event that orders its users (see jt_psf_convolve).
  *   - "device [n]" = pointer to device memory holding n elements of the call's dtype
@@ -94,8 +94,9 @@ typedef struct {
 /* Step 1 ("ray-traced through the deflectors back to the source plane"):
  * beta = theta - alpha_SIE - alpha_shear - sum_j alpha_TNFW,j on caller-supplied ray positions.
  * theta_x, theta_y: device [n_rays] (in).  beta_x, beta_y: device [n_rays] (out).
- * workspace: device scratch of at least jt_ray_shoot_workspace_bytes(dtype, n_rays, n_tnfw) bytes
- * (partial sums when the subhalo list is split over thread blocks; may be NULL when that is 0). */
+ * workspace: device scratch of at least jt_ray_shoot_workspace_bytes(dtype, n_rays, n_tnfw) bytes, 16-byte aligned
+ * (the derived subhalo records, written at the start of every call, and partial sums when the subhalo list is split
+ * over thread blocks; may be NULL when that is 0, i.e. when n_tnfw = 0). */
 JT_API size_t    jt_ray_shoot_workspace_bytes(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw);
 JT_API jt_status jt_ray_shoot(jt_dtype dtype, int64_t n_rays, const void *theta_x, const void *theta_y,
                        const jt_lens *lens, void *workspace, size_t workspace_bytes,
@@ -215,16 +216,18 @@ JT_API jt_status jt_light_profiles(jt_dtype dtype, int64_t n, const void *beta_x
 
 /* Measurement aid (bench.py's roofline leg).  jt_profile_enable(1) makes every following
  * jt_simulate_image call on this host thread record CUDA events on its stream before the ray-tracing kernel, between it
- * and the convolution, and after the convolution, and copy the kernel's four tier counters (32 bytes) to a pinned host
+ * and the convolution, and after the convolution, and copy the kernel's JT_N_TIERS tier counters (48 bytes) to a pinned host
  * buffer the library owns (event records and one cudaMemcpyAsync: no synchronisation, nothing keeps pointing into the
  * caller's workspace).  jt_profile_read waits for the events of the LAST such call and returns the two intervals in
  * milliseconds (conv_ms = 0 when the call had no PSF).  JT_ERR_INVALID_VALUE when profiling is off or no call has been
  * recorded.  jt_profile_enable(0) destroys the events and frees the buffer. */
 JT_API jt_status jt_profile_enable(int on);
 JT_API jt_status jt_profile_read(float *trace_ms, float *conv_ms);
-/* counts[4] (host) receives, for the LAST profiled jt_simulate_image call, the number of (warp, subhalo-record) pairs
- * evaluated by the far-far series, the far form, the mid form and the per-ray cold path.
- * Waits for that call's counter copy (an event), not for the device. */
+/* counts[JT_N_TIERS] (host) receives, for the LAST profiled jt_simulate_image call, the number of (warp, subhalo-record)
+ * pairs evaluated by each form of definition T: the far-far series at its three lengths (longest first), the far form,
+ * the mid form and the per-ray cold path.  Waits for that call's counter copy (an event), not
+ * for the device. */
+#define JT_N_TIERS 6
 JT_API jt_status jt_profile_tiers(uint64_t *counts);
 
 /* Number of CUDA kernels this library has launched from the calling host thread since it was loaded

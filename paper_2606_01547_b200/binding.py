@@ -138,8 +138,9 @@ def profile_read():
 
 
 def profile_tiers():
-    """jt_profile_tiers: (far-far, far, mid, cold) counts of (warp, subhalo record) pairs of the last profiled call."""
-    c = (ctypes.c_uint64 * 4)()
+    """jt_profile_tiers: (far-far long / middle / short series, far, mid, cold) counts of (warp, subhalo record) pairs of
+    the last profiled call (JT_N_TIERS = 6 values)."""
+    c = (ctypes.c_uint64 * 6)()
     _check(lib().jt_profile_tiers(c), "jt_profile_tiers")
     return tuple(int(x) for x in c)
 

@@ -13,7 +13,7 @@ void count_launch() { ++g_launches; }
 struct ProfileState {
     bool on = false, recorded = false, had_conv = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};      // start, after trace, after conv, after the counter copy
-    uint64_t* host_tiers = nullptr;    // pinned host copy of the last profiled call's four tier counters
+    uint64_t* host_tiers = nullptr;    // pinned host copy of the last profiled call's JT_N_TIERS tier counters
     bool have_tiers = false;
 };
 static thread_local ProfileState g_prof;
@@ -209,7 +209,7 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
     // profiling: the kernel's tier counters (in the workspace) are copied to the library's pinned buffer right behind
     // the kernel, so nothing points into the caller's workspace once the call returns
     auto fetch_tiers = [&]() -> jt_status {
-        JT_CUDA_TRY(cudaMemcpyAsync(g_prof.host_tiers, trace_tier_counters(plan, trace_ws), 4 * sizeof(uint64_t),
+        JT_CUDA_TRY(cudaMemcpyAsync(g_prof.host_tiers, trace_tier_counters(plan, trace_ws), JT_N_TIERS * sizeof(uint64_t),
                                     cudaMemcpyDeviceToHost, st));
         g_prof.have_tiers = true;
         return JT_OK;
@@ -246,7 +246,7 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
 jt_status jt_profile_enable(int on) {
     if (on && !g_prof.on) {
         for (int i = 0; i < 4; ++i) JT_CUDA_TRY(cudaEventCreate(&g_prof.ev[i]));
-        JT_CUDA_TRY(cudaHostAlloc((void**)&g_prof.host_tiers, 4 * sizeof(uint64_t), cudaHostAllocDefault));
+        JT_CUDA_TRY(cudaHostAlloc((void**)&g_prof.host_tiers, JT_N_TIERS * sizeof(uint64_t), cudaHostAllocDefault));
         g_prof.on = true;
         g_prof.recorded = false;
         g_prof.have_tiers = false;
@@ -273,7 +273,7 @@ jt_status jt_profile_read(float* trace_ms, float* conv_ms) {
 jt_status jt_profile_tiers(uint64_t* counts) {
     if (!g_prof.on || !g_prof.recorded || !g_prof.have_tiers || !counts) return JT_ERR_INVALID_VALUE;
     JT_CUDA_TRY(cudaEventSynchronize(g_prof.ev[3]));
-    for (int k = 0; k < 4; ++k) counts[k] = g_prof.host_tiers[k];
+    for (int k = 0; k < JT_N_TIERS; ++k) counts[k] = g_prof.host_tiers[k];
     return JT_OK;
 }
 

@@ -8,6 +8,7 @@
 //   direct convolution (definition P) out of that shared image with the register-window sweep of jt_conv.cuh
 //   one coalesced HBM write of the final image.
 // HBM traffic per system is its parameters in and its image out; nothing intermediate leaves the SM.
+#include <stdlib.h>
 #include "jt_conv.cuh"
 #include "jt_trace.cuh"
 
@@ -15,6 +16,7 @@ namespace jt {
 
 constexpr int kBatchRecCap = 512;            // subhalo records resident per staging round (float; 256 in double)
 template <typename T> struct BatchRecCap { static constexpr int value = sizeof(T) == 8 ? 256 : 512; };
+constexpr int kBatchVar = 2;                 // subhalo_tile_sorted variant (jt_trace.cuh): the batch kernel's code must stay small
 constexpr int kBatchTW = 64;                 // convolution pass: 64 columns (32 lanes x 2) x 8 warps * OY rows
 template <typename T> struct BatchOY { static constexpr int value = sizeof(T) == 4 ? 8 : 4; };   // as in jt_conv.cu
 
@@ -33,12 +35,13 @@ struct BatchArgs {
     double* chi2;                            // [B]
 };
 
-template <typename T, int R>
-__global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch(const __grid_constant__ BatchArgs<T> a) {
+template <typename T, int R, int VAR>
+__global__ void __launch_bounds__(kBatchThreads, sizeof(T) == 4 ? 2 : 1) k_batch(const __grid_constant__ BatchArgs<T> a) {
     extern __shared__ __align__(32) unsigned char smem_raw[];      // SubRec<double> is 32-byte aligned
     __shared__ MacroLens s_m;
     __shared__ SrcSet s_src;
-    __shared__ unsigned short s_queue[kTraceThreads / 32][kBatchRecCap];
+    __shared__ int s_next;                         // next warp tile to hand out
+    __shared__ unsigned short s_queue[kBatchThreads / 32][2 * kBatchRecCap];
 
     SubRec<T>* recs = reinterpret_cast<SubRec<T>*>(smem_raw);
     T* img = reinterpret_cast<T*>(smem_raw + (size_t)a.rec_cap * sizeof(SubRec<T>));
@@ -57,7 +60,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
         s_m = derive_macro(1, (double)p[0], (double)p[1], (double)p[2], (double)p[3], (double)p[4], 1, (double)g[0],
                            (double)g[1]);
     }
-    if (tid == 32) s_src.n = a.n_src;
+    if (tid == 32) { s_src.n = a.n_src; s_next = 0; }
     if (tid >= 32 && tid < 32 + a.n_src) {
         const int k = tid - 32;
         const T* q = a.sersic + (b * a.n_src + k) * 7;
@@ -65,14 +68,14 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
                       (double)q[6]);
     }
     if (conv) {
-        for (int i = tid; i < a.pw * a.ph; i += kTraceThreads) img[i] = (T)0;
-        stage_taps<T>(Kc, a.psf + b * (int64_t)a.ky * a.kx, a.ky, a.kx, a.kyp, 0, (a.kx + 1) / 2, tid, kTraceThreads);
+        for (int i = tid; i < a.pw * a.ph; i += kBatchThreads) img[i] = (T)0;
+        stage_taps<T>(Kc, a.psf + b * (int64_t)a.ky * a.kx, a.ky, a.kx, a.kyp, 0, (a.kx + 1) / 2, tid, kBatchThreads);
     }
     const RawTn<T> raw = {{a.tnfw + (b * 5 + 0) * a.M, a.tnfw + (b * 5 + 1) * a.M, a.tnfw + (b * 5 + 2) * a.M,
                            a.tnfw + (b * 5 + 3) * a.M, a.tnfw + (b * 5 + 4) * a.M}};
     const bool resident = a.M <= a.rec_cap;        // the whole subhalo list is staged once
     if (resident) {
-        for (int k = tid; k < a.M; k += kTraceThreads)
+        for (int k = tid; k < a.M; k += kBatchThreads)
             recs[k] = make_rec<T>((double)raw.p[0][k], (double)raw.p[1][k], (double)raw.p[2][k], (double)raw.p[3][k],
                                   (double)raw.p[4][k]);
     }
@@ -92,9 +95,20 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
             chi = fma(r, r, chi);
         }
     };
-    for (int tile = 0; tile < a.n_tiles; ++tile) {
+    // Warp tiles are handed out dynamically (a shared counter): a warp whose tiles hold subhalo cores takes fewer of
+    // them, so the warps reach the barrier in front of the convolution together.  A pixel's value does not depend on
+    // which warp forms it; only the chi^2 of the no-PSF path sums per thread in tile order, so that path deals statically.
+    const bool dynamic = !resident ? false : (conv || a.chi2 == nullptr);
+    for (int tile = 0;; ++tile) {
+        int wt = tile * (kBatchThreads / 32) + warp;
+        if (dynamic) {
+            if (lane == 0) wt = atomicAdd(&s_next, 1);
+            wt = __shfl_sync(0xffffffffu, wt, 0);
+            if (wt >= a.n_wt) break;
+        } else if (tile >= a.n_tiles) {
+            break;
+        }
         RayGeom g = {a.hh, a.cx, a.cy, a.NX, a.NY, a.NX, a.NY};     // idle warp: clamped coordinates, no stores
-        const int wt = tile * (kTraceThreads / 32) + warp;
         if (wt < a.n_wt) {
             g.I = (wt % a.wtiles_x) * a.cols_per_warp + lane;
             g.J0 = (wt / a.wtiles_x) * R;
@@ -104,22 +118,27 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
         pin(x);
 #pragma unroll
         for (int r = 0; r < R; ++r) { xs[r] = x; ys[r] = (T)g.yd(r); pin(ys[r]); }
-        DAcc<T, R> acc;
+        DAcc<T, R, kBatchThreads> acc;
         acc.init(dacc + tid);
-        TierCount tiers = {{0u, 0u, 0u, 0u}};
+        TierCount tiers = {};
+        WarpBox<T> box;
+        box.xlo = __shfl_sync(0xffffffffu, xs[0], 0);
+        box.xhi = __shfl_sync(0xffffffffu, xs[0], 31);      // columns ascend with the lane (clamped at the grid edge)
+        box.ylo = ys[0];
+        box.yhi = ys[R - 1];
 
         if (resident) {
-            subhalo_tile<T, R, true, false>(recs, a.M, 0, raw, g, xs, ys, acc, s_queue[warp], tiers);
+            subhalo_tile_sorted<T, R, kBatchThreads, VAR>(recs, a.M, kBatchRecCap, 0, raw, g, box, xs, ys, acc, s_queue[warp], tiers);
         } else {
             for (int base = 0; base < a.M; base += a.rec_cap) {
                 const int count = min(a.rec_cap, a.M - base);
                 __syncthreads();
-                for (int k = tid; k < count; k += kTraceThreads)
+                for (int k = tid; k < count; k += kBatchThreads)
                     recs[k] = make_rec<T>((double)raw.p[0][base + k], (double)raw.p[1][base + k],
                                           (double)raw.p[2][base + k], (double)raw.p[3][base + k],
                                           (double)raw.p[4][base + k]);
                 __syncthreads();
-                subhalo_tile<T, R, true, false>(recs, count, base, raw, g, xs, ys, acc, s_queue[warp], tiers);
+                subhalo_tile_sorted<T, R, kBatchThreads, VAR>(recs, count, kBatchRecCap, base, raw, g, box, xs, ys, acc, s_queue[warp], tiers);
             }
         }
         double axd[R], ayd[R];
@@ -138,7 +157,7 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
 
     // ---- step 5a out of shared memory: passes of 64 columns x 64 rows, OY x 2 outputs per thread ----
     constexpr int kBatchOY = BatchOY<T>::value;
-    constexpr int TH = (kTraceThreads / 32) * kBatchOY;
+    constexpr int TH = (kBatchThreads / 32) * kBatchOY;
     const int npairs = (a.kx + 1) / 2;
     for (int j0 = 0; j0 < a.ny; j0 += TH) {
         for (int i0 = 0; i0 < a.nx; i0 += kBatchTW) {
@@ -158,34 +177,35 @@ __global__ void __launch_bounds__(kTraceThreads, sizeof(T) == 4 ? 2 : 1) k_batch
     }
     }
     if (a.chi2 != nullptr) {                       // fixed summation tree: lanes, then the 8 warps in order
-        __shared__ double s_red[kTraceThreads / 32];
+        __shared__ double s_red[kBatchThreads / 32];
         for (int o = 16; o > 0; o >>= 1) chi += __shfl_xor_sync(0xffffffffu, chi, o);
         if (lane == 0) s_red[warp] = chi;
         __syncthreads();
         if (tid == 0) {
             double tot = 0.0;
-            for (int w = 0; w < kTraceThreads / 32; ++w) tot += s_red[w];
+            for (int w = 0; w < kBatchThreads / 32; ++w) tot += s_red[w];
             a.chi2[b] = tot;
         }
     }
 }
 
-constexpr size_t kBatchMaxSmem = 227 * 1024 - 4096 - 8192;      // static MacroLens + SrcSet live beside the dynamic part
+constexpr size_t kBatchMaxSmem = 227 * 1024 - 4096 - 16384;      // static MacroLens + SrcSet live beside the dynamic part
 
 template <typename T>
 static size_t batch_smem_front(const BatchArgs<T>& a) {
     return align_up((size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)4 * ((a.kx + 1) / 2) * a.kyp) * sizeof(T), 16);
 }
 
-#define JT_BATCH_CASE(RR)                                                                              \
-    case RR: {                                                                                         \
-        auto kern = k_batch<T, RR>;                                                                    \
+#define JT_BATCH_CASE(RR) JT_BATCH_CASE_V(RR, RR, kBatchVar)
+#define JT_BATCH_CASE_V(TAG, RR, VV)                                                                   \
+    case TAG: {                                                                                        \
+        auto kern = k_batch<T, RR, VV>;                                                                \
         static bool attr_set = false;   /* once per instantiation: allow the full dynamic shared memory */ \
         if (!attr_set) {                                                                               \
             JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBatchMaxSmem)); \
             attr_set = true;                                                                           \
         }                                                                                              \
-        kern<<<(unsigned)B, kTraceThreads, smem, st>>>(a);                                             \
+        kern<<<(unsigned)B, kBatchThreads, smem, st>>>(a);                                             \
         break;                                                                                         \
     }
 
@@ -202,13 +222,14 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.cy = g->cy;
     a.area_over_s2 = g->pixel_scale * g->pixel_scale / ((double)s * (double)s);
     a.cols_per_warp = plan.cols_per_warp;
-    a.wtiles_x = plan.tiles_x; a.n_wt = (int)plan.n_wt; a.n_tiles = (int)plan.n_tiles;
+    a.wtiles_x = plan.tiles_x; a.n_wt = (int)plan.n_wt;
+    a.n_tiles = (int)((plan.n_wt + kBatchThreads / 32 - 1) / (kBatchThreads / 32));
     a.M = p->n_tnfw; a.n_src = p->n_src;
     const bool conv = p->ky > 0;
     a.ky = conv ? p->ky : 0; a.kx = conv ? p->kx : 0;
     constexpr int kBatchOY = BatchOY<T>::value;
     a.kyp = (a.ky + kBatchOY - 1) / kBatchOY * kBatchOY;
-    constexpr int TH = (kTraceThreads / 32) * kBatchOY;
+    constexpr int TH = (kBatchThreads / 32) * kBatchOY;
     const int64_t pw64 = conv ? ((int64_t)g->nx + kBatchTW - 1) / kBatchTW * kBatchTW + a.kx - 1 : 0;   // even: pair loads stay aligned
     const int64_t ph64 = conv ? ((int64_t)g->ny + TH - 1) / TH * TH + a.kyp - 1 : 0;
     if (pw64 * ph64 * (int64_t)sizeof(T) > (int64_t)kBatchMaxSmem) return JT_ERR_UNSUPPORTED;   // before any int arithmetic on it
@@ -221,8 +242,19 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.out = (T*)out;
     a.data = (const T*)data; a.sigma = (const T*)sigma; a.chi2 = chi2;
     a.dacc_off = (int)batch_smem_front(a);
-    const size_t smem = (size_t)a.dacc_off + (sizeof(T) == 4 ? (size_t)plan.R * kTraceThreads * sizeof(double2) : 0);
+    const size_t smem = (size_t)a.dacc_off + (sizeof(T) == 4 ? (size_t)plan.R * kBatchThreads * sizeof(double2) : 0);
     if (smem > kBatchMaxSmem) return JT_ERR_UNSUPPORTED;
+    if (const char* e = getenv("JT_BATCH_VAR")) {          // EXPERIMENT: variants of the R = 8 kernel
+        if (plan.R == 8) {
+            switch (100 + atoi(e)) {
+                JT_BATCH_CASE_V(100, 8, 0) JT_BATCH_CASE_V(101, 8, 1) JT_BATCH_CASE_V(102, 8, 2) JT_BATCH_CASE_V(103, 8, 3)
+                JT_BATCH_CASE_V(104, 8, 4) JT_BATCH_CASE_V(105, 8, 5) JT_BATCH_CASE_V(106, 8, 6) JT_BATCH_CASE_V(107, 8, 7)
+                default: return JT_ERR_UNSUPPORTED;
+            }
+            JT_LAUNCH_CHECK();
+            return JT_OK;
+        }
+    }
     switch (plan.R) {
         JT_BATCH_CASE(5) JT_BATCH_CASE(6) JT_BATCH_CASE(7) JT_BATCH_CASE(8) JT_BATCH_CASE(9) JT_BATCH_CASE(10)
         JT_BATCH_CASE(11) JT_BATCH_CASE(12) JT_BATCH_CASE(13) JT_BATCH_CASE(14) JT_BATCH_CASE(15) JT_BATCH_CASE(16)

@@ -69,29 +69,38 @@ __device__ __forceinline__ double t_log(double x) { return log(x); }
 //   brace = (t-1+2X^2) F(X) + c1 + S (c2 L - pi),  t = tau^2, c1 = tau pi + (t-1) ln tau, c2 = (t-1)/tau,
 //   S = sqrt(t+X^2), L = ln(X/(S+tau)).
 // ------------------------------------------------------------------------------------------------
-// The hot loops read the first nine fields (amplitude folded into the brace coefficients: one multiply per evaluation
-// less); the generic near-field forms read amp, tm1, c1.
 // Far-far field: for X >= 9 max(1, tau) (double; 8 max(1, tau) in float) the brace is summed from its expansion in
-// v = 1/X, derived with sympy from the closed form (every coefficient carries the factor (t+1)^2; the v^1 term vanishes):
-//   brace = b0 + b2 v^2 + b3 v^3 + ... ,   b0 = (t-1) ln tau - t + pi tau - 1 (the total-mass limit),
+// 1/X, derived with sympy from the closed form (every coefficient carries the factor (t+1)^2; the 1/X term vanishes):
+//   brace = b0 + b2 / X^2 + b3 / X^3 + ... ,   b0 = (t-1) ln tau - t + pi tau - 1 (the total-mass limit),
 //   b2 = -(t+1)^2/3, b3 = pi (t+1)^2/8, b4 = 2 (t+1)^2 (t-3)/15, b5 = -pi (t+1)^2 (t-2)/16, ...
-// Truncated after v^13 (double) / v^8 (float) the relative error is <= 1e-13 / 2e-8 beyond those radii for
-// tau = 0.3 ... 20 (checked against the closed form at 50 digits).  alpha = f (dx, dy), f = v^2 (a0 + v^2 (a2 + a3 v +
-// ...)), a_k = amp b_k / Rs^2: one MUFU and K + 1 multiply-adds instead of three MUFU and two polynomials.
+// Truncated after 1/X^13 (double) / 1/X^8 (float) the relative error is <= 1e-13 / 2e-8 beyond those radii (reading
+// Q9b in DESIGN.md: verified against the closed form at 50 digits for tau = 0.3 ... 1000).  With v = 1/R (NOT 1/X: the
+// powers of Rs are folded into the coefficients, a_k = amp b_k Rs^k) the deflection is alpha = f (dx, dy),
+//   f = v^2 (a_0 + v^2 (a_2 + a_3 v + ... + a_K v^(K-2))):  one MUFU and K + 1 multiply-adds per evaluation.
+// The farther the ray, the shorter the sum: three levels (K, radius in units of max(1, tau) Rs), each within the same
+// error bound (double 1e-13: 2.2e-14 / 6.0e-14 / 5e-14 worst case at tau = 1 on the radius; float 4.2e-9 / 4.0e-9 / 3.5e-9):
 template <typename T> struct FarFar;
-template <> struct FarFar<double> { static constexpr int K = 13; static constexpr double kRadius = 9.0; };
-template <> struct FarFar<float> { static constexpr int K = 8; static constexpr double kRadius = 8.0; };
-
-template <typename T>
-struct alignas(sizeof(T) * 4) SubRec {
-    T cx, cy, iRs2, thr;       // centre, 1/Rs^2, far-field threshold on X^2 (= max(10, 3t))
-    T t, a_tm1, a_c1, a_pi;    // tau^2, amp (t-1), amp c1, amp pi
-    T c_a, c_b, c_c, amp;      // amp (t-1) pi/2, amp (t+1), 2 amp; amplitude
-    T tm1, c1, thr2, a0;       // tau^2 - 1, c1 (generic near-field forms); far-far threshold on X^2; a_0
-    T ak[(FarFar<T>::K - 1 + 3) / 4 * 4];      // a_2 ... a_K, zero-padded to a multiple of 4
+template <> struct FarFar<double> {
+    static constexpr int K = 13, K1 = 9, K2 = 7;
+    static constexpr double kRadius = 9.0, kRadius1 = 20.0, kRadius2 = 44.0;
+};
+template <> struct FarFar<float> {
+    static constexpr int K = 8, K1 = 5, K2 = 4;
+    static constexpr double kRadius = 8.0, kRadius1 = 24.0, kRadius2 = 46.0;
 };
 
-// b_k / (t+1)^2 for k = 2 ... 14 as polynomials in t (sympy series of the closed form)
+// Field order = access order: the far-far loop reads the first (K + 3) values only (centre, a_0, a_2 ... a_K); the
+// classification pass reads cx, cy, thr2, iRs2, thr; the far / mid / generic forms read the rest.
+template <typename T>
+struct alignas(sizeof(T) * 4) SubRec {
+    T cx, cy, a0, thr2;        // centre; a_0; far-far threshold on X^2 (huge when the series is switched off for this record)
+    T ak[(FarFar<T>::K - 1 + 3) / 4 * 4];      // a_2 ... a_K, zero-padded to a multiple of 4
+    T iRs2, thr, t, a_tm1;     // 1/Rs^2; far-field threshold on X^2 (= max(10, 3t)); tau^2; amp (t-1)
+    T a_c1, a_pi, c_a, c_b;    // amp c1, amp pi, amp (t-1) pi/2, amp (t+1)
+    T c_c, amp, tm1, c1;       // 2 amp; amplitude; tau^2 - 1, c1 (generic near-field forms)
+};
+
+// b_k / (t+1)^2 for k = 2 ... 13 as polynomials in t (sympy series of the closed form)
 __host__ __device__ inline double farfar_coef(int k, double t) {
     const double pi = JT_PI_D;
     switch (k) {
@@ -135,17 +144,21 @@ __device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, d
     r.c1 = (T)c1;
     const double rad = FarFar<T>::kRadius * fmax(1.0, tau);
     r.thr2 = (T)(rad * rad);
-    const double sc = amp * iRs2;
-    r.a0 = (T)(sc * ((t - 1.0) * lt - t + JT_PI_D * tau - 1.0));
-    const double f = sc * (t + 1.0) * (t + 1.0);
+    r.a0 = (T)(amp * ((t - 1.0) * lt - t + JT_PI_D * tau - 1.0));
+    // a_k = amp b_k Rs^k.  A coefficient that leaves T's normal range in either direction (extreme tau, tiny Rs)
+    // switches the series off for this record: it then takes the far form, which has no such limit.
+    const double big = sizeof(T) == 4 ? 1e30 : 1e250, tiny = sizeof(T) == 4 ? 1e-30 : 1e-280;
+    bool ok = isfinite((double)r.a0);
+    double f = amp * (t + 1.0) * (t + 1.0) * Rs;
 #pragma unroll
-    for (int k = 2; k <= FarFar<T>::K; ++k) r.ak[k - 2] = (T)(f * farfar_coef(k, t));
+    for (int k = 2; k <= FarFar<T>::K; ++k) {
+        f *= Rs;
+        const double a = f * farfar_coef(k, t);
+        ok = ok && isfinite(a) && fabs(a) < big && (a == 0.0 || fabs(a) > tiny);
+        r.ak[k - 2] = (T)a;
+    }
 #pragma unroll
     for (int k = FarFar<T>::K - 1; k < (int)(sizeof(r.ak) / sizeof(T)); ++k) r.ak[k] = (T)0;
-    // extreme tau (float: beyond ~1e3): the top coefficients leave T's range -> no far-far tier for this record
-    bool ok = isfinite((double)r.a0);
-#pragma unroll
-    for (int k = 0; k < FarFar<T>::K - 1; ++k) ok = ok && isfinite((double)r.ak[k]) && fabs((double)r.ak[k]) < (sizeof(T) == 4 ? 1e30 : 1e250);
     if (!ok) {
         r.thr2 = (T)(sizeof(T) == 4 ? 3.0e38 : 1.0e300);
         r.a0 = (T)0;
@@ -154,26 +167,15 @@ __device__ __forceinline__ SubRec<T> make_rec(double cx, double cy, double Rs, d
     }
     return r;
 }
-// padding record: contributes exactly 0 and always takes the far path
-template <typename T>
-__device__ __forceinline__ SubRec<T> null_rec() {
-    SubRec<T> r;
-    r.cx = (T)1e6; r.cy = (T)1e6; r.iRs2 = (T)1; r.thr = (T)10; r.t = (T)1;
-    r.a_tm1 = (T)0; r.a_c1 = (T)0; r.a_pi = (T)0; r.c_a = (T)0; r.c_b = (T)0; r.c_c = (T)0; r.amp = (T)0;
-    r.tm1 = (T)0; r.c1 = (T)0; r.thr2 = (T)81; r.a0 = (T)0;
-#pragma unroll
-    for (int k = 0; k < (int)(sizeof(r.ak) / sizeof(T)); ++k) r.ak[k] = (T)0;
-    return r;
-}
 
-// Far-far field (see FarFar above).  Returns f with alpha = f * (dx, dy).
-template <typename T>
+// Far-far field (see FarFar above), series summed to 1/R^K.  Returns f with alpha = f * (dx, dy).
+template <typename T, int K = FarFar<T>::K>
 __device__ __forceinline__ T tnfw_farfar(T R2, const SubRec<T>& s) {
-    const T v = fast_rsqrt(R2 * s.iRs2);
+    const T v = fast_rsqrt(R2);
     const T v2 = v * v;
-    T p = s.ak[FarFar<T>::K - 2];
+    T p = s.ak[K - 2];
 #pragma unroll
-    for (int k = FarFar<T>::K - 3; k >= 0; --k) p = fma(p, v, s.ak[k]);
+    for (int k = K - 3; k >= 0; --k) p = fma(p, v, s.ak[k]);
     return v2 * fma(p, v2, s.a0);
 }
 
@@ -241,17 +243,17 @@ __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
-// far-far field on two rays at once (float)
-__device__ __forceinline__ void tnfw_farfar_pair(float R2a, float R2b, const SubRec<float>& s, float& fa, float& fb) {
-    const f32x2 X2 = mul2(pack2(R2a, R2b), bc2(s.iRs2));
-    float xa, xb;
-    unpack2(X2, xa, xb);
-    const f32x2 v = pack2(fast_rsqrt(xa), fast_rsqrt(xb));
+// far-far field on two rays at once (float): R2 = (R2a, R2b) packed
+template <int K>
+__device__ __forceinline__ f32x2 tnfw_farfar2(f32x2 R2, const SubRec<float>& s) {
+    float ra, rb;
+    unpack2(R2, ra, rb);
+    const f32x2 v = pack2(fast_rsqrt(ra), fast_rsqrt(rb));
     const f32x2 v2 = mul2(v, v);
-    f32x2 p = bc2(s.ak[FarFar<float>::K - 2]);
+    f32x2 p = bc2(s.ak[K - 2]);
 #pragma unroll
-    for (int k = FarFar<float>::K - 3; k >= 0; --k) p = fma2(p, v, bc2(s.ak[k]));
-    unpack2(mul2(v2, fma2(p, v2, bc2(s.a0))), fa, fb);
+    for (int k = K - 3; k >= 0; --k) p = fma2(p, v, bc2(s.ak[k]));
+    return mul2(v2, fma2(p, v2, bc2(s.a0)));
 }
 
 // The whole far-field form on two rays at once (same algebra as tnfw_far<float>; MUFU on the halves).

@@ -9,7 +9,7 @@
 namespace jt {
 
 constexpr int kNumSMs = 148;            // B200
-constexpr int kTraceThreads = 256;      // 8 warps per CTA in the ray-tracing kernels
+constexpr int kBatchThreads = 256;      // 8 warps per CTA in the batch kernel
 
 // thread-local last CUDA error (jt_last_cuda_error)
 void set_last_cuda_error(int e);
@@ -36,15 +36,17 @@ jt_status make_sources(const jt_sources* src, SrcSet* out);
 // ---- ray tracing (jt_trace.cu) ----
 struct TracePlan {
     int R;                 // rays per thread
+    int threads;           // threads per CTA
     int cols_per_warp;     // active lanes per warp (grid mode: floor(32/s)*s; ray mode: 32)
     int tiles_x, tiles_y;  // grid mode: warp tiles (cols_per_warp x R rays) per axis
     int64_t n_wt;          // grid mode: warp tiles in all
-    int64_t n_tiles;       // CTAs per subhalo chunk (8 warp tiles, or 8 * 32 * R rays in ray mode)
+    int64_t n_tiles;       // CTAs per subhalo chunk (threads/32 warp tiles, or threads * R rays in ray mode)
     int n_chunks;          // subhalo list split (1 = no workspace traffic)
     int64_t chunk_len;     // subhalos per chunk
     size_t partial_bytes;  // n_chunks > 1: double2 per (chunk, ray slot)
     size_t counter_bytes;  // one uint32 per tile
-    size_t tier_bytes;     // grid mode: four uint64 tier counters (jt_profile_tiers), always reserved
+    size_t tier_bytes;     // four uint64 tier counters (jt_profile_tiers), always reserved
+    size_t rec_bytes;      // derived subhalo records, written by k_make_recs at the start of every call
     size_t total_bytes;
 };
 TracePlan plan_trace_grid(jt_dtype dtype, const jt_grid* g, int64_t n_tnfw);

@@ -28,17 +28,19 @@ jt_status make_sources(const jt_sources* src, SrcSet* out) {
 // ---- plans ----
 static int rays_per_thread(int s, bool f64) {
     if (f64) {
-        switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 6; case 5: return 5; default: return s; }
+        switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 6; case 5: return 10; default: return s; }
     }
-    switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 9; case 5: return 10; default: return s; }
+    switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 6; case 5: return 10; case 7: return 14; default: return s; }   // even where it fits: rays go two to a packed instruction
 }
 
 // Split of the subhalo list over CTAs.  All CTAs of a launch do the same work, so the launch runs in waves of
 // `slots` CTAs (148 SMs x resident CTAs per SM); pick the chunk count c that minimises
 //   waves(n_tiles * c) * (records per chunk + fixed per-CTA cost in record units)
 // -- e.g. C2 (91 ray tiles, 10,000 subhalos, float): c = 13 gives 1183 CTAs = 4 full waves of 296.
+static int trace_threads(bool f64) { return f64 ? TraceCfg<double>::NT : TraceCfg<float>::NT; }
+
 static void plan_chunks(TracePlan* p, int64_t M, int R, bool f64) {
-    const int64_t slots = (int64_t)kNumSMs * (f64 ? 1 : 2);
+    const int64_t slots = (int64_t)kNumSMs * (f64 ? TraceCfg<double>::OCC : TraceCfg<float>::OCC);
     const int64_t ovh = 48, ovh_split = 24;          // prologue + epilogue; partial-sum publish + reduce
     int64_t best_c = 1;
     if (M > 0 && p->n_tiles > 0) {
@@ -56,9 +58,10 @@ static void plan_chunks(TracePlan* p, int64_t M, int R, bool f64) {
     p->chunk_len = M > 0 ? (M + best_c - 1) / best_c : 1;
     p->n_chunks = M > 0 ? (int)((M + p->chunk_len - 1) / p->chunk_len) : 1;
     if (p->n_chunks < 1) p->n_chunks = 1;
-    p->partial_bytes = p->n_chunks > 1 ? (size_t)p->n_chunks * p->n_tiles * R * kTraceThreads * sizeof(double2) : 0;
+    p->partial_bytes = p->n_chunks > 1 ? (size_t)p->n_chunks * p->n_tiles * R * p->threads * sizeof(double2) : 0;
     p->counter_bytes = p->n_chunks > 1 ? align_up((size_t)p->n_tiles * sizeof(unsigned int), 256) : 0;
-    p->total_bytes = p->partial_bytes + p->counter_bytes + p->tier_bytes;
+    p->rec_bytes = align_up((size_t)M * (f64 ? sizeof(SubRec<double>) : sizeof(SubRec<float>)), 256);
+    p->total_bytes = p->partial_bytes + p->counter_bytes + p->tier_bytes + p->rec_bytes;
 }
 
 // Ray ownership: a warp tile is cols_per_warp ray columns x R ray rows; the warp tiles of the grid are numbered
@@ -72,8 +75,9 @@ static TracePlan plan_trace_grid_t(const jt_grid* g, int64_t n_tnfw, bool f64) {
     p.tiles_x = (NX + p.cols_per_warp - 1) / p.cols_per_warp;       // warp tiles per row of warp tiles
     p.tiles_y = (NY + p.R - 1) / p.R;
     p.n_wt = (int64_t)p.tiles_x * p.tiles_y;
-    p.n_tiles = (p.n_wt + kTraceThreads / 32 - 1) / (kTraceThreads / 32);
-    p.tier_bytes = 64;
+    p.threads = trace_threads(f64);
+    p.n_tiles = (p.n_wt + p.threads / 32 - 1) / (p.threads / 32);
+    p.tier_bytes = 256;
     plan_chunks(&p, n_tnfw, p.R, f64);
     return p;
 }
@@ -84,28 +88,53 @@ TracePlan plan_trace_rays(jt_dtype d, int64_t n_rays, int64_t n_tnfw) {
     p.R = 8;
     p.cols_per_warp = 32;
     p.tiles_x = 1; p.tiles_y = 1;
-    p.n_tiles = (n_rays + (int64_t)p.R * kTraceThreads - 1) / ((int64_t)p.R * kTraceThreads);
+    p.threads = trace_threads(d == JT_F64);
+    p.n_tiles = (n_rays + (int64_t)p.R * p.threads - 1) / ((int64_t)p.R * p.threads);
+    p.tier_bytes = 0;
     plan_chunks(&p, n_tnfw, p.R, d == JT_F64);
     return p;
 }
 
+// records per shared-memory tile: what fits kStages times beside the float mode's accumulator columns with
+// TraceCfg<T>::OCC CTAs per SM, at most 256 (more only delays the first tile), a multiple of 32
 template <typename T>
-static void fill_lens(TraceArgs<T>& a, const jt_lens* lens, const TracePlan& plan, void* workspace) {
+static int pick_tile_recs(int R, int64_t chunk_len) {
+    const size_t budget = (size_t)227 * 1024 / TraceCfg<T>::OCC - 2048;
+    const size_t dacc = sizeof(T) == 4 ? (size_t)R * TraceCfg<T>::NT * sizeof(double2) : 0;
+    const size_t per = kStages * sizeof(SubRec<T>) + (TraceCfg<T>::NT / 32) * 2 * sizeof(unsigned short);
+    int64_t tr = budget > dacc + 32 * per ? (int64_t)((budget - dacc) / per) / 32 * 32 : 32;
+    if (tr > 256) tr = 256;
+    const int64_t need = (chunk_len < 1 ? 1 : chunk_len + 31) / 32 * 32;       // the whole chunk in one tile when it is short
+    return (int)(need < tr ? (need < 32 ? 32 : need) : tr);
+}
+
+// Fills the lens part of the arguments and enqueues k_make_recs (derived records, zeroed counters).
+template <typename T>
+static jt_status fill_lens(TraceArgs<T>& a, const jt_lens* lens, const TracePlan& plan, void* workspace, bool count_tiers,
+                           cudaStream_t st) {
     a.m = make_macro(lens);
     a.M = lens->n_tnfw;
     a.tn[0] = (const T*)lens->tnfw_cx; a.tn[1] = (const T*)lens->tnfw_cy; a.tn[2] = (const T*)lens->tnfw_Rs;
     a.tn[3] = (const T*)lens->tnfw_alpha_Rs; a.tn[4] = (const T*)lens->tnfw_r_trunc;
     a.n_chunks = plan.n_chunks;
     a.chunk_len = plan.chunk_len;
-    // records per staging round: the whole chunk when it fits (one barrier pair per CTA), else the largest tile that
-    // leaves room for 2 CTAs/SM (float: 96 B records + 32-64 KB of double sums) or 1 CTA/SM (double: 224 B records)
-    const int64_t cap = sizeof(T) == 8 ? 768 : 512;
-    int64_t tr = plan.chunk_len < cap ? plan.chunk_len : cap;
-    if (a.M < tr) tr = a.M;
-    a.tile_recs = (int)((tr < 1 ? 1 : tr) + 31) / 32 * 32;
+    a.tile_recs = pick_tile_recs<T>(plan.R, plan.chunk_len);
     a.n_tiles = plan.n_tiles;
     a.partial = (double2*)workspace;
     a.counter = (unsigned int*)((char*)workspace + plan.partial_bytes);
+    a.tier_counts = count_tiers ? (unsigned long long*)trace_tier_counters(plan, workspace) : nullptr;
+    a.recs = (const SubRec<T>*)((char*)workspace + plan.partial_bytes + plan.counter_bytes + plan.tier_bytes);
+    if (a.M > 0) {
+        const int n_counter = plan.n_chunks > 1 ? (int)plan.n_tiles : 0;
+        const int64_t n = a.M > n_counter ? a.M : n_counter;
+        const RawTn<T> raw = {{a.tn[0], a.tn[1], a.tn[2], a.tn[3], a.tn[4]}};
+        k_make_recs<T><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a.M, raw, const_cast<SubRec<T>*>(a.recs), a.counter, n_counter,
+                                                                   a.tier_counts);
+        JT_LAUNCH_CHECK();
+    } else if (count_tiers) {
+        JT_CUDA_TRY(cudaMemsetAsync(a.tier_counts, 0, kTiers * sizeof(unsigned long long), st));
+    }
+    return JT_OK;
 }
 
 template <typename T>
@@ -121,14 +150,10 @@ static jt_status trace_grid_t(const jt_grid* g, const jt_lens* lens, const SrcSe
     a.cols_per_warp = plan.cols_per_warp;
     a.wtiles_x = plan.tiles_x;
     a.n_wt = plan.n_wt;
-    fill_lens(a, lens, plan, workspace);
+    const jt_status fs = fill_lens(a, lens, plan, workspace, count_tiers, st);
+    if (fs != JT_OK) return fs;
     a.out = (T*)pre_psf;
     a.src = src;
-    if (plan.n_chunks > 1) JT_CUDA_TRY(cudaMemsetAsync(a.counter, 0, plan.counter_bytes, st));
-    if (count_tiers) {
-        a.tier_counts = (unsigned long long*)trace_tier_counters(plan, workspace);
-        JT_CUDA_TRY(cudaMemsetAsync(a.tier_counts, 0, 4 * sizeof(unsigned long long), st));
-    }
     return launch_trace_t<T, true>(a, plan.R, st);
 }
 
@@ -148,8 +173,8 @@ static jt_status trace_rays_t(int64_t n, const void* tx, const void* ty, const j
     TraceArgs<T> a = {};
     a.n_rays = n;
     a.tx = (const T*)tx; a.ty = (const T*)ty; a.bx = (T*)bx; a.by = (T*)by;
-    fill_lens(a, lens, plan, workspace);
-    if (plan.n_chunks > 1) JT_CUDA_TRY(cudaMemsetAsync(a.counter, 0, plan.counter_bytes, st));
+    const jt_status fs = fill_lens(a, lens, plan, workspace, false, st);
+    if (fs != JT_OK) return fs;
     return launch_trace_t<T, false>(a, plan.R, st);
 }
 

@@ -81,7 +81,9 @@ def test_workspace_queries_are_consistent(jt):
     big = jt.simulate_image_workspace_bytes("f32", g, 10000, 21, 21, "direct")
     small = jt.simulate_image_workspace_bytes("f32", g, 0, 21, 21, "direct")
     assert big > small >= 200 * 200 * 4
-    assert jt.ray_shoot_workspace_bytes("f64", 10 ** 7, 100) == 0        # enough ray tiles: no split, no scratch
+    assert jt.ray_shoot_workspace_bytes("f64", 10 ** 7, 0) == 0          # no subhalos: no records, no split, no scratch
+    rec = jt.ray_shoot_workspace_bytes("f64", 10 ** 7, 100)              # enough ray tiles: no split, only the derived records
+    assert 100 * 8 * 16 <= rec <= 100 * 8 * 32 + 256
     assert jt.ray_shoot_workspace_bytes("f64", 1000, 10 ** 5) > 0
 
 
