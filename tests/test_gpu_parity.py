@@ -378,6 +378,38 @@ def test_image_edge_cases(jt, orc, dtype):
     _check_image(jt, orc, wn, method="auto")
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("s", [1, 2, 5])
+def test_image_series_levels_and_cores(jt, orc, dtype, s):
+    """jt_simulate_image's per-warp-tile sort: a few VERY strong subhalos (alpha_Rs = 0.5-2 arcsec,
+    hundreds of times the priors') whose three far-far radii (9 / 20 / 44 max(1, tau) Rs in double, 8 / 24 / 46 in float),
+    far and near zones all fall inside the grid, so that every warp tile puts some of them in every class; two of them
+    sit exactly on a ray and exactly between rays.  The source is broad and shallow (n = 1), so max|img| does not dwarf
+    the pixels the subhalos act on.  The float64 tolerance here is 1e-12, a hundred times tighter than the north-star
+    bar: the series' truncation bound is 1e-13 of each deflection (measured: 3e-15 ... 7e-15 on this case), while a
+    series shortened one level too early (K = 7 from the K = 13 radius on -- tried as a mutation) gives 1.2e-11 ... 7.8e-11."""
+    nx, ny, h = 96, 64, 0.05
+    tn = np.array([  # cx, cy, Rs, alpha_Rs, r_trunc
+        [0.31, -0.22, 0.010, 2.00, 0.010],       # tau = 1: radii 0.09, 0.20, 0.44
+        [-1.20, 0.45, 0.004, 2.00, 0.020],       # tau = 5: 0.18, 0.40, 0.88
+        [1.05, 0.90, 0.020, 1.00, 0.010],        # tau = 0.5 (max(1, tau) = 1): 0.18, 0.40, 0.88
+        [-0.60, -1.10, 0.002, 1.00, 0.040],      # tau = 20: 0.36, 0.80, 1.76
+        [0.0, 0.0, 0.006, 0.50, 0.030],          # moved onto a ray below
+        [0.0, 0.0, 0.006, 0.50, 0.030],          # moved between four rays below
+    ]).T.copy()
+    w = workloads.config_c4(nx=nx, n_tnfw=6, K=9, dtype="f64")
+    w.ny, w.supersample, w.pixel_scale, w.cx, w.cy = ny, s, h, 0.0, 0.0
+    hs = h / s
+    x0 = -(nx * s - 1) / 2 * hs
+    y0 = -(ny * s - 1) / 2 * hs
+    tn[0, 4], tn[1, 4] = x0 + 37 * hs, y0 + 21 * hs                  # exactly on ray (J = 21, I = 37)
+    tn[0, 5], tn[1, 5] = x0 + 60.5 * hs, y0 + 40.5 * hs              # centre of a ray cell
+    w.tnfw = tn
+    w.sources = np.array([[3.0, 0.8, 1.0, 0.0, 0.1, -0.3, 0.2]])
+    w = w.as_dtype(dtype)
+    _check_image(jt, orc, w, method="direct", tol=1e-12 if dtype == "f64" else None)
+
+
 @pytest.mark.parametrize("seed", range(16))
 def test_image_random_shapes(jt, orc, seed):
     """Seeded random configurations of the fused call: grid shape and offset, supersampling, subhalo count (around the
