@@ -36,11 +36,14 @@ if ROOT not in sys.path:
 METRIC = "ray_deflector_evals_per_s"
 UNIT = "evals/s"
 SM_COUNT = 148
-# Algorithmic work per evaluation on the binding unit, counted in the SASS of each warp-uniform
-# tier loop (loop head + body) divided by its 8 rays; f32: FP32-pipe lane operations (a packed FFMA2 / FMUL2 / FADD2
-# counts as two); f64: FP64-pipe instructions.  Order: far-far series, far form, mid form, cold path (counted as far).
-# The mix of tiers is measured per run with jt_profile_tiers.
-TIER_COST = {"f32": (14.5, 14.5, 14.5, 29.6, 47.0, 29.6), "f64": (25.2, 25.2, 25.2, 50.6, 80.0, 50.6)}
+# Algorithmic work per evaluation on the binding unit, counted in the SASS of each class loop
+# (`python -m paper_2606_01547_b200.sass_loops`, output and the arithmetic in profiles/r02_sass_loops.md): loop body count
+# of the pipe's opcodes / (records per iteration x rays per thread).  f32: FP32-pipe lane operations (a packed FFMA2 /
+# FMUL2 / FADD2 counts as two: it holds the pipe for two cycles); f64: FP64-pipe instructions.  Order: far-far series at
+# its three lengths (longest first), far form, near form on a warp tile outside / inside X^2 = 2 (both run the mid form
+# on every ray; the per-ray generic fix-up inside is not counted).  The mix of classes is measured per run with
+# jt_profile_tiers.
+TIER_COST = {"f32": (13.25, 10.25, 9.25, 29.6, 36.0, 36.0), "f64": (23.25, 19.25, 17.25, 50.6, 77.0, 77.0)}
 TIER_NAMES = ("far_far_long", "far_far_mid", "far_far_short", "far", "mid", "cold")
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu --set full captures in
 # profiles/r01d_ncu_{c2f64,c2f32,c3f32}.txt (the kernels are ALU-bound: compulsory traffic is parameters in, image out)
@@ -222,10 +225,27 @@ class BatchRunner:
         self.jt.simulate_batch(self.grid, *self.d, out=self.out)
 
     def step_e2e(self):
-        for d, h in zip(self.d, self.h):
-            d.copy_(h, non_blocking=True)
-        self.step()
-        self.h_out.copy_(self.out, non_blocking=True)
+        """Pinned host -> device -> kernel -> pinned host, the batch cut into slices dealt to two streams so that the
+        67 MB of images of slice i go back over PCIe while slice i + 1 is being simulated (systems are independent:
+        a slice is just a smaller jt_simulate_batch call on views of the same buffers)."""
+        import torch
+        if not hasattr(self, "streams"):
+            self.streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+            n = min(8, self.w.B)
+            edges = [round(i * self.w.B / n) for i in range(n + 1)]
+            self.slices = [(a, b) for a, b in zip(edges[:-1], edges[1:]) if b > a]
+        cur = torch.cuda.current_stream()
+        for st in self.streams:
+            st.wait_stream(cur)
+        for i, (a, b) in enumerate(self.slices):
+            st = self.streams[i % 2]
+            with torch.cuda.stream(st):
+                for d, h in zip(self.d, self.h):
+                    d[a:b].copy_(h[a:b], non_blocking=True)
+                self.jt.simulate_batch(self.grid, *[d[a:b] for d in self.d], out=self.out[a:b], stream=st)
+                self.h_out[a:b].copy_(self.out[a:b], non_blocking=True)
+        for st in self.streams:
+            cur.wait_stream(st)
 
 
 # ------------------------------------------------------------------ the oracle on the host cores
@@ -392,6 +412,26 @@ def conv_block(torch, jt, w, peaks, probes):
     return blk
 
 
+def latency_block(torch, jt):
+    """The launch-latency-bound configs C0 and C1 (parity configs, roofline fractions not
+    meaningful): microseconds per image, device time from a CUDA-graph replay of 20 jt_simulate_image calls, and wall
+    time per call through the Python binding (ctypes marshalling included)."""
+    out = {}
+    for name in ("C0-f64", "C1-f64"):
+        r = ImageRunner(jt, make_workload(name, 0), "auto")
+        us = graph_time(torch, r.step)
+        for _ in range(20):
+            r.step()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(200):
+            r.step()
+        torch.cuda.synchronize()
+        out[name] = {"device_us_per_image_graph_replay": us, "python_call_us_per_image": 1e6 * (time.perf_counter() - t0) / 200,
+                     "evals": int(r.w.evals)}
+    return out
+
+
 def measure(torch, jt, name, args, rank, world, sample_clocks=False):
     """Both timed legs and the roofline record of one workload.  Returns a dict (rank 0) or None."""
     w = make_workload(name, rank)
@@ -530,6 +570,8 @@ def run_ours(args, rank, world, local_rank):
         meas = probes["ffma"] if r["dtype"] == "f32" else probes["dfma"]
         r["roofline"]["frac_of_measured_alu_rate"] = r["roofline"]["achieved"] * 1e12 / meas
     line["conv"] = conv_block(torch, jt, w, peaks, probes)
+    if world == 1 and not args.no_per_config:
+        line["latency_configs"] = latency_block(torch, jt)
     if per_config:
         line["per_config"] = per_config
     if not args.no_cpu_baseline:
@@ -567,7 +609,7 @@ def run_conv_sweep(args, rank):
                 img = torch.as_tensor(rng.uniform(0, 1, (B, n, n)), dtype=tdt, device="cuda")
                 out = torch.empty_like(img)
                 row = {"dtype": dtype, "n": n, "K": k, "B": B}
-                for method in ("direct", "fft", "auto") if B == 1 else ("direct", "auto"):
+                for method in ("direct", "fft", "auto"):
                     try:
                         nb = jt.psf_convolve_batch_workspace_bytes(dtype, B, n, n, k, k, method)
                         ws = torch.empty(max(nb, 1), dtype=torch.uint8, device="cuda")

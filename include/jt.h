@@ -128,7 +128,8 @@ JT_API jt_status jt_psf_convolve(jt_dtype dtype, int32_t ny, int32_t nx, const v
 
 /* The same on B images with ONE kernel in one call (the batched form of the paper's convolution benchmark,
  * PAPER.md:112-114; SURVEY.md section 8(d) D4 "batch B in {1, 1024} images").  images, out: device [B][ny][nx].
- * DIRECT runs all images in one launch (B x tiles x row bands CTAs); FFT transforms them one after the other. */
+ * DIRECT runs all images in one launch (B x tiles x row bands CTAs); FFT transforms the kernel once and the images
+ * in groups whose spectra fit 2 GiB of workspace (four launches per group). */
 JT_API size_t    jt_psf_convolve_batch_workspace_bytes(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
                                                 jt_conv_method method);
 JT_API jt_status jt_psf_convolve_batch(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, const void *images,

@@ -47,27 +47,21 @@ jt_conv_method resolve_conv_method(jt_dtype dtype, int64_t B, int ny, int nx, in
     if (m == JT_CONV_DIRECT || m == JT_CONV_FFT) return m;
     if (!conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_CONV_FFT;
     if (!conv_fft_supported(dtype, ny, nx, ky, kx)) return JT_CONV_DIRECT;
-    return (double)B * conv_fft_estimate_us(dtype, ny, nx, ky, kx) < conv_direct_estimate_us(dtype, B, ny, nx, ky, kx) ? JT_CONV_FFT
+    return conv_fft_estimate_us(dtype, B, ny, nx, ky, kx) < conv_direct_estimate_us(dtype, B, ny, nx, ky, kx) ? JT_CONV_FFT
                                                                                                                      : JT_CONV_DIRECT;
 }
 
 static size_t conv_ws(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx, jt_conv_method method) {
     const jt_conv_method m = resolve_conv_method(dtype, B, ny, nx, ky, kx, method);
-    return m == JT_CONV_DIRECT ? conv_direct_workspace_bytes(dtype, B, ny, nx, ky, kx) : fft_conv_workspace_bytes(dtype, ny, nx, ky, kx);
+    return m == JT_CONV_DIRECT ? conv_direct_workspace_bytes(dtype, B, ny, nx, ky, kx) : fft_conv_workspace_bytes(dtype, B, ny, nx, ky, kx);
 }
 
-// B images [B][ny][nx] with one kernel.  The FFT path transforms the images one after the other (one plane of workspace).
+// B images [B][ny][nx] with one kernel
 static jt_status conv_dispatch(jt_dtype dtype, int64_t B, int ny, int nx, const void* image, int ky, int kx, const void* kernel,
                                jt_conv_method method, void* workspace, void* out, cudaStream_t st) {
     const jt_conv_method m = resolve_conv_method(dtype, B, ny, nx, ky, kx, method);
     if (m == JT_CONV_DIRECT) return launch_conv_direct(dtype, B, ny, nx, image, ky, kx, kernel, workspace, out, st);
-    const size_t img_bytes = (size_t)ny * nx * dtype_size(dtype);
-    for (int64_t b = 0; b < B; ++b) {
-        const jt_status s = launch_conv_fft(dtype, ny, nx, (const char*)image + b * img_bytes, ky, kx, kernel, workspace,
-                                            (char*)out + b * img_bytes, st);
-        if (s != JT_OK) return s;
-    }
-    return JT_OK;
+    return launch_conv_fft(dtype, B, ny, nx, image, ky, kx, kernel, workspace, out, st);
 }
 
 }  // namespace jt

@@ -8,7 +8,6 @@
 //   direct convolution (definition P) out of that shared image with the register-window sweep of jt_conv.cuh
 //   one coalesced HBM write of the final image.
 // HBM traffic per system is its parameters in and its image out; nothing intermediate leaves the SM.
-#include <stdlib.h>
 #include "jt_conv.cuh"
 #include "jt_trace.cuh"
 
@@ -196,10 +195,9 @@ static size_t batch_smem_front(const BatchArgs<T>& a) {
     return align_up((size_t)a.rec_cap * sizeof(SubRec<T>) + ((size_t)a.img_elems + (size_t)4 * ((a.kx + 1) / 2) * a.kyp) * sizeof(T), 16);
 }
 
-#define JT_BATCH_CASE(RR) JT_BATCH_CASE_V(RR, RR, kBatchVar)
-#define JT_BATCH_CASE_V(TAG, RR, VV)                                                                   \
-    case TAG: {                                                                                        \
-        auto kern = k_batch<T, RR, VV>;                                                                \
+#define JT_BATCH_CASE(RR)                                                                              \
+    case RR: {                                                                                         \
+        auto kern = k_batch<T, RR, kBatchVar>;                                                         \
         static bool attr_set = false;   /* once per instantiation: allow the full dynamic shared memory */ \
         if (!attr_set) {                                                                               \
             JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBatchMaxSmem)); \
@@ -244,17 +242,6 @@ static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_b
     a.dacc_off = (int)batch_smem_front(a);
     const size_t smem = (size_t)a.dacc_off + (sizeof(T) == 4 ? (size_t)plan.R * kBatchThreads * sizeof(double2) : 0);
     if (smem > kBatchMaxSmem) return JT_ERR_UNSUPPORTED;
-    if (const char* e = getenv("JT_BATCH_VAR")) {          // EXPERIMENT: variants of the R = 8 kernel
-        if (plan.R == 8) {
-            switch (100 + atoi(e)) {
-                JT_BATCH_CASE_V(100, 8, 0) JT_BATCH_CASE_V(101, 8, 1) JT_BATCH_CASE_V(102, 8, 2) JT_BATCH_CASE_V(103, 8, 3)
-                JT_BATCH_CASE_V(104, 8, 4) JT_BATCH_CASE_V(105, 8, 5) JT_BATCH_CASE_V(106, 8, 6) JT_BATCH_CASE_V(107, 8, 7)
-                default: return JT_ERR_UNSUPPORTED;
-            }
-            JT_LAUNCH_CHECK();
-            return JT_OK;
-        }
-    }
     switch (plan.R) {
         JT_BATCH_CASE(5) JT_BATCH_CASE(6) JT_BATCH_CASE(7) JT_BATCH_CASE(8) JT_BATCH_CASE(9) JT_BATCH_CASE(10)
         JT_BATCH_CASE(11) JT_BATCH_CASE(12) JT_BATCH_CASE(13) JT_BATCH_CASE(14) JT_BATCH_CASE(15) JT_BATCH_CASE(16)

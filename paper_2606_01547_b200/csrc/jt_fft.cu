@@ -150,7 +150,9 @@ struct FftArgs {
     int n_cta_img;                   // rows_fwd: CTAs that transform image row pairs (the rest take kernel rows)
     Radices rx, ry;
     double scale;                    // 1 / (Px Py)
-    Cd *SA, *SB, *SC;                // planes [ny][Ph], [ky][Ph], [ny][Ph]
+    int B;                           // images sharing the one kernel
+    Cd *SA, *SB, *SC;                // planes [B][ny][Ph], [ky][Ph], [B][ny][Ph]
+    Cd *SBF;                         // B > 1: the kernel's full 2-D spectrum [Py][Ph], scaled, transformed once
 };
 
 // ---- rows forward: pairs of real rows -> half spectra ----
@@ -164,11 +166,13 @@ __global__ void __launch_bounds__(kFftMaxThreads) k_fft_rows_fwd(const __grid_co
     Cd* tw = y + (size_t)a.nb * P;
     cudaTriggerProgrammaticLaunchCompletion();                 // lets k_fft_cols start its twiddle set-up once every CTA here runs
     make_twiddles(tw, P, tid, nthr);
-    const bool is_img = (int)blockIdx.x < a.n_cta_img;
-    const T* src = is_img ? img : ker;
+    const int n_img_ctas = a.n_cta_img * a.B;
+    const bool is_img = (int)blockIdx.x < n_img_ctas;
+    const int b_img = is_img ? (int)blockIdx.x / a.n_cta_img : 0;
+    const T* src = is_img ? img + (size_t)b_img * a.ny * a.nx : ker;
     const int rows = is_img ? a.ny : a.ky, width = is_img ? a.nx : a.kx;
-    Cd* plane = is_img ? a.SA : a.SB;
-    const int pair0 = (is_img ? (int)blockIdx.x : (int)blockIdx.x - a.n_cta_img) * a.nb;
+    Cd* plane = is_img ? a.SA + (size_t)b_img * a.ny * a.Ph : a.SB;
+    const int pair0 = (is_img ? (int)blockIdx.x - b_img * a.n_cta_img : (int)blockIdx.x - n_img_ctas) * a.nb;
     for (int idx = tid; idx < a.nb * P; idx += nthr) {
         const int b = idx / P, i = idx - b * P;
         const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
@@ -192,34 +196,46 @@ __global__ void __launch_bounds__(kFftMaxThreads) k_fft_rows_fwd(const __grid_co
 }
 
 // ---- columns: forward FFTs of tc image and tc kernel spectrum columns, product, inverse FFT, crop ----
+// KER_READY (batches): the kernel's columns were transformed once by k_fft_cols_ker; the product reads SBF.
+template <bool KER_READY>
 __global__ void __launch_bounds__(kFftMaxThreads) k_fft_cols(const __grid_constant__ FftArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int P = a.Py, tc = a.tc, tid = threadIdx.x, nthr = blockDim.x;
-    Cd* x = reinterpret_cast<Cd*>(smem_raw);                   // [2 tc][P]: image columns, then kernel columns
-    Cd* y = x + (size_t)2 * tc * P;
-    Cd* tw = y + (size_t)2 * tc * P;
+    constexpr int NSET = KER_READY ? 1 : 2;
+    Cd* x = reinterpret_cast<Cd*>(smem_raw);                   // [NSET tc][P]: image columns, then kernel columns
+    Cd* y = x + (size_t)NSET * tc * P;
+    Cd* tw = y + (size_t)NSET * tc * P;
     make_twiddles(tw, P, tid, nthr);
-    cudaGridDependencySynchronize();                           // the planes SA, SB of k_fft_rows_fwd are complete
+    cudaGridDependencySynchronize();                           // the planes of the previous kernel are complete
     cudaTriggerProgrammaticLaunchCompletion();
     const int k0 = blockIdx.x * tc;
     const int ncol = min(tc, a.Ph - k0);
+    const Cd* SA = a.SA + (size_t)blockIdx.y * a.ny * a.Ph;
+    Cd* SC = a.SC + (size_t)blockIdx.y * a.ny * a.Ph;
     for (int idx = tid; idx < P * tc; idx += nthr) {
         const int r = idx / tc, c = idx - r * tc;
         Cd va = {0.0, 0.0}, vb = {0.0, 0.0};
         if (c < ncol) {
-            if (r < a.ny) va = __ldcg(&a.SA[(size_t)r * a.Ph + k0 + c]);
-            if (r < a.ky) vb = __ldcg(&a.SB[(size_t)r * a.Ph + k0 + c]);
+            if (r < a.ny) va = __ldcg(&SA[(size_t)r * a.Ph + k0 + c]);
+            if (!KER_READY && r < a.ky) vb = __ldcg(&a.SB[(size_t)r * a.Ph + k0 + c]);
         }
         x[c * P + r] = va;
-        x[(tc + c) * P + r] = vb;
+        if (!KER_READY) x[(tc + c) * P + r] = vb;
     }
     __syncthreads();
-    Cd* X = stockham<-1>(x, y, tw, P, a.ry, 2 * tc, P, tid, nthr);
+    Cd* X = stockham<-1>(x, y, tw, P, a.ry, NSET * tc, P, tid, nthr);
     Cd* Y = (X == x) ? y : x;
     for (int idx = tid; idx < tc * P; idx += nthr) {
-        Cd c = cmul(X[idx], X[tc * P + idx]);
-        c.x *= a.scale;
-        c.y *= a.scale;
+        Cd c;
+        if (KER_READY) {
+            const int col = idx / P, r = idx - col * P;
+            const Cd kf = col < ncol ? __ldcg(&a.SBF[(size_t)r * a.Ph + k0 + col]) : Cd{0.0, 0.0};
+            c = cmul(X[idx], kf);
+        } else {
+            c = cmul(X[idx], X[tc * P + idx]);
+            c.x *= a.scale;
+            c.y *= a.scale;
+        }
         X[idx] = c;
     }
     __syncthreads();
@@ -227,7 +243,38 @@ __global__ void __launch_bounds__(kFftMaxThreads) k_fft_cols(const __grid_consta
     const int row0 = a.ky / 2;
     for (int idx = tid; idx < a.ny * tc; idx += nthr) {
         const int j = idx / tc, c = idx - j * tc;
-        if (c < ncol) a.SC[(size_t)j * a.Ph + k0 + c] = C[c * P + row0 + j];
+        if (c < ncol) SC[(size_t)j * a.Ph + k0 + c] = C[c * P + row0 + j];
+    }
+}
+
+// ---- batches: column FFTs of the kernel's row spectra, once -> SBF [Py][Ph] with the 1 / (Px Py) scale ----
+__global__ void __launch_bounds__(kFftMaxThreads) k_fft_cols_ker(const __grid_constant__ FftArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int P = a.Py, tc = a.tc, tid = threadIdx.x, nthr = blockDim.x;
+    Cd* x = reinterpret_cast<Cd*>(smem_raw);
+    Cd* y = x + (size_t)tc * P;
+    Cd* tw = y + (size_t)tc * P;
+    make_twiddles(tw, P, tid, nthr);
+    cudaGridDependencySynchronize();                           // plane SB of k_fft_rows_fwd is complete
+    cudaTriggerProgrammaticLaunchCompletion();
+    const int k0 = blockIdx.x * tc;
+    const int ncol = min(tc, a.Ph - k0);
+    for (int idx = tid; idx < P * tc; idx += nthr) {
+        const int r = idx / tc, c = idx - r * tc;
+        Cd vb = {0.0, 0.0};
+        if (c < ncol && r < a.ky) vb = __ldcg(&a.SB[(size_t)r * a.Ph + k0 + c]);
+        x[c * P + r] = vb;
+    }
+    __syncthreads();
+    const Cd* X = stockham<-1>(x, y, tw, P, a.ry, tc, P, tid, nthr);
+    for (int idx = tid; idx < P * tc; idx += nthr) {
+        const int r = idx / tc, c = idx - r * tc;
+        if (c < ncol) {
+            Cd v = X[c * P + r];
+            v.x *= a.scale;
+            v.y *= a.scale;
+            a.SBF[(size_t)r * a.Ph + k0 + c] = v;
+        }
     }
 }
 
@@ -242,6 +289,8 @@ __global__ void __launch_bounds__(kFftMaxThreads) k_fft_rows_inv(const __grid_co
     make_twiddles(tw, P, tid, nthr);
     cudaGridDependencySynchronize();                           // plane SC of k_fft_cols is complete
     const int pair0 = blockIdx.x * a.nb;
+    const Cd* SC = a.SC + (size_t)blockIdx.y * a.ny * a.Ph;
+    out += (size_t)blockIdx.y * a.ny * a.nx;
     for (int idx = tid; idx < a.nb * P; idx += nthr) {
         const int b = idx / P, k = idx - b * P;
         const int r0 = 2 * (pair0 + b), r1 = r0 + 1;
@@ -249,9 +298,9 @@ __global__ void __launch_bounds__(kFftMaxThreads) k_fft_rows_inv(const __grid_co
         if (r0 < a.ny) {
             const bool mirror = k >= a.Ph;                     // C_k = conj C_{P-k} for k > P/2
             const int kk = mirror ? P - k : k;
-            Cd ca = __ldcg(&a.SC[(size_t)r0 * a.Ph + kk]);
+            Cd ca = __ldcg(&SC[(size_t)r0 * a.Ph + kk]);
             Cd cb = {0.0, 0.0};
-            if (r1 < a.ny) cb = __ldcg(&a.SC[(size_t)r1 * a.Ph + kk]);
+            if (r1 < a.ny) cb = __ldcg(&SC[(size_t)r1 * a.Ph + kk]);
             if (mirror) { ca.y = -ca.y; cb.y = -cb.y; }
             v = {ca.x - cb.y, ca.y + cb.x};                    // C_a + i C_b
         }
@@ -302,7 +351,7 @@ struct FftPlan {
     bool ok;
 };
 
-static FftPlan plan_fft(int ny, int nx, int ky, int kx) {
+static FftPlan plan_fft(int ny, int nx, int ky, int kx, int64_t B = 1) {
     FftPlan p = {};
     p.ok = false;
     if ((int64_t)ny + ky - 1 > kFftMaxP || (int64_t)nx + kx - 1 > kFftMaxP) return p;
@@ -318,7 +367,9 @@ static FftPlan plan_fft(int ny, int nx, int ky, int kx) {
     // row kernels: enough butterflies per CTA for 256 threads, enough CTAs for 148 SMs
     const int pairs_img = (ny + 1) / 2, pairs_ker = (ky + 1) / 2;
     int nb = 1;
-    while (nb < 8 && nb * a.Px < 1024 && (pairs_img + pairs_ker) / (2 * nb) >= 2 * kNumSMs) nb *= 2;
+    const int64_t pairs_all = (int64_t)pairs_img * B + pairs_ker;
+    // one image: short transforms share a CTA; a batch: as many row pairs per CTA as keep 4 CTAs per SM busy
+    while (nb < 8 && (B > 1 || nb * a.Px < 1024) && pairs_all / (2 * nb) >= (B > 1 ? 4 : 2) * kNumSMs) nb *= 2;
     a.nb = nb;
     p.smem_rows = ((size_t)2 * nb * a.Px + a.Px) * csz;
     a.n_cta_img = (pairs_img + nb - 1) / nb;
@@ -326,17 +377,17 @@ static FftPlan plan_fft(int ny, int nx, int ky, int kx) {
     p.grid_rows_inv = a.n_cta_img;
     // column kernel: 2 columns per CTA (one 32-byte sector per plane row); 4 when the transform is short
     int tc = 2;
-    while (tc < 8 && tc * a.Py < 512 && (a.Ph + 2 * tc - 1) / (2 * tc) >= kNumSMs) tc *= 2;
-    while (tc > 1 && ((size_t)4 * tc * a.Py + a.Py) * csz > kFftMaxSmem) tc /= 2;
+    while (tc < 8 && (B > 1 || tc * a.Py < 512) && (int64_t)((a.Ph + 2 * tc - 1) / (2 * tc)) * B >= (B > 1 ? 4 : 1) * kNumSMs) tc *= 2;
+    while (tc > 1 && ((size_t)4 * tc * a.Py + a.Py) * csz > (B > 1 ? kFftMaxSmem / 2 : kFftMaxSmem)) tc /= 2;
     a.tc = tc;
-    p.smem_cols = ((size_t)4 * tc * a.Py + a.Py) * csz;
+    p.smem_cols = ((size_t)(B > 1 ? 2 : 4) * tc * a.Py + a.Py) * csz;     // batches: the kernel's columns are not in the CTA
     p.grid_cols = (a.Ph + tc - 1) / tc;
     if (p.smem_rows > kFftMaxSmem || p.smem_cols > kFftMaxSmem) return p;
     // CTA sizes: about one radix-4 butterfly per thread and pass, capped where more warps only lengthen the barriers
     // (measured on B200: rows 256, columns 384-512 are best from 60^2 to 1000^2)
     auto pick_threads = [](int butterflies, int cap) { int t = (butterflies + 31) / 32 * 32; return t < 128 ? 128 : (t > cap ? cap : t); };
     p.thr_rows = pick_threads(nb * a.Px / 4, 256);
-    p.thr_cols = pick_threads(2 * tc * a.Py / 4, 512);
+    p.thr_cols = pick_threads((B > 1 ? 1 : 2) * tc * a.Py / 4, 512);
     p.plane_a = align_up((size_t)ny * a.Ph * csz, 256);
     p.plane_b = align_up((size_t)ky * a.Ph * csz, 256);
     p.plane_c = align_up((size_t)ny * a.Ph * csz, 256);
@@ -346,24 +397,39 @@ static FftPlan plan_fft(int ny, int nx, int ky, int kx) {
 
 bool conv_fft_supported(jt_dtype, int ny, int nx, int ky, int kx) { return plan_fft(ny, nx, ky, kx).ok; }
 
-// Time model behind JT_CONV_AUTO, calibrated on B200 with bench.py --conv-sweep: three dependent
-// launches plus the planes' trips through L2.
-double conv_fft_estimate_us(jt_dtype, int ny, int nx, int ky, int kx) {
-    const FftPlan p = plan_fft(ny, nx, ky, kx);
+// A batch is transformed in groups of G images (all of it when its planes fit kFftGroupBytes of workspace).
+constexpr size_t kFftGroupBytes = (size_t)2 << 30;
+static int64_t fft_group(const FftPlan& p, int64_t B) {
+    const size_t per = p.plane_a + p.plane_c;
+    int64_t G = (int64_t)(kFftGroupBytes / (per ? per : 1));
+    if (G < 1) G = 1;
+    if (G > 65535) G = 65535;                       // gridDim.y
+    return B < G ? B : G;
+}
+static size_t fft_plane_bf(const FftPlan& p, int64_t B) { return B > 1 ? align_up((size_t)p.a.Py * p.a.Ph * sizeof(Cd), 256) : 0; }
+
+// Time model behind JT_CONV_AUTO, calibrated on B200 with bench.py --conv-sweep: dependent
+// launches plus the planes' trips through L2 (one image) or HBM (a batch: the kernel's spectrum is formed once).
+double conv_fft_estimate_us(jt_dtype, int64_t B, int ny, int nx, int ky, int kx) {
+    const FftPlan p = plan_fft(ny, nx, ky, kx, B);
     if (!p.ok) return 1e30;
     const double mb = (double)(p.plane_a + p.plane_b + p.plane_c) * 2.0 / 1048576.0;
-    return 9.0 + 1.2 * mb;
+    if (B <= 1) return 9.0 + 1.2 * mb;
+    const double mb_img = (double)(p.plane_a + p.plane_c) * 2.0 / 1048576.0;
+    return 14.0 + 1.2 * mb + (double)(B - 1) * 1.3 * mb_img;   // measured: 0.77 TB/s of plane traffic (FP64 butterflies in shared memory)
 }
 
-size_t fft_conv_workspace_bytes(jt_dtype, int ny, int nx, int ky, int kx) {
-    const FftPlan p = plan_fft(ny, nx, ky, kx);
-    return p.ok ? p.plane_a + p.plane_b + p.plane_c : 0;
+size_t fft_conv_workspace_bytes(jt_dtype, int64_t B, int ny, int nx, int ky, int kx) {
+    const FftPlan p = plan_fft(ny, nx, ky, kx, B);
+    if (!p.ok) return 0;
+    const int64_t G = fft_group(p, B);
+    return (size_t)G * (p.plane_a + p.plane_c) + p.plane_b + fft_plane_bf(p, B);
 }
 
 template <typename K, typename... Args>
-static jt_status launch_fft_kernel(K kern, int grid, int threads, size_t smem, bool dependent, cudaStream_t st, Args... args) {
+static jt_status launch_fft_kernel(K kern, dim3 grid, int threads, size_t smem, bool dependent, cudaStream_t st, Args... args) {
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)grid);
+    cfg.gridDim = grid;
     cfg.blockDim = dim3((unsigned)threads);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
@@ -377,35 +443,60 @@ static jt_status launch_fft_kernel(K kern, int grid, int threads, size_t smem, b
     return JT_OK;
 }
 
+// workspace: [SA: G images][SC: G images][SB][SBF (batches)]
 template <typename T>
-static jt_status conv_fft_t(FftPlan& p, const T* img, const T* ker, void* workspace, T* out, cudaStream_t st) {
+static jt_status conv_fft_t(FftPlan& p, int64_t B, const T* img, const T* ker, void* workspace, T* out, cudaStream_t st) {
     FftArgs& a = p.a;
+    const int64_t G = fft_group(p, B);
     a.SA = (Cd*)workspace;
-    a.SB = (Cd*)((char*)workspace + p.plane_a);
-    a.SC = (Cd*)((char*)workspace + p.plane_a + p.plane_b);
+    a.SC = (Cd*)((char*)workspace + (size_t)G * p.plane_a);
+    a.SB = (Cd*)((char*)workspace + (size_t)G * (p.plane_a + p.plane_c));
+    a.SBF = (Cd*)((char*)a.SB + p.plane_b);
     auto k1 = k_fft_rows_fwd<T>;
-    auto k2 = k_fft_cols;
+    auto k2 = k_fft_cols<false>;
+    auto k2r = k_fft_cols<true>;
+    auto k2k = k_fft_cols_ker;
     auto k3 = k_fft_rows_inv<T>;
     static bool attr_set = false;                  // once per instantiation: allow the full dynamic shared memory
     if (!attr_set) {
         JT_CUDA_TRY(cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         JT_CUDA_TRY(cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
+        JT_CUDA_TRY(cudaFuncSetAttribute(k2r, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
+        JT_CUDA_TRY(cudaFuncSetAttribute(k2k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         JT_CUDA_TRY(cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         attr_set = true;
     }
-    jt_status s = launch_fft_kernel(k1, p.grid_rows_fwd, p.thr_rows, p.smem_rows, false, st, a, img, ker);
-    if (s != JT_OK) return s;
-    s = launch_fft_kernel(k2, p.grid_cols, p.thr_cols, p.smem_cols, true, st, a);
-    if (s != JT_OK) return s;
-    return launch_fft_kernel(k3, p.grid_rows_inv, p.thr_rows, p.smem_rows, true, st, a, out);
+    const int ker_ctas = p.grid_rows_fwd - a.n_cta_img;
+    const size_t img_elems = (size_t)a.ny * a.nx;
+    for (int64_t b0 = 0; b0 < B; b0 += G) {
+        const int g = (int)(B - b0 < G ? B - b0 : G);
+        a.B = g;
+        // the kernel's rows ride the first group's row pass (its CTAs come after the images'); later groups reuse SB / SBF
+        const int rows_grid = a.n_cta_img * g + (b0 == 0 ? ker_ctas : 0);
+        jt_status s = launch_fft_kernel(k1, dim3((unsigned)rows_grid), p.thr_rows, p.smem_rows, false, st, a, img + b0 * img_elems, ker);
+        if (s != JT_OK) return s;
+        if (B > 1) {
+            if (b0 == 0) {
+                s = launch_fft_kernel(k2k, dim3((unsigned)p.grid_cols), p.thr_cols, p.smem_cols, true, st, a);
+                if (s != JT_OK) return s;
+            }
+            s = launch_fft_kernel(k2r, dim3((unsigned)p.grid_cols, (unsigned)g), p.thr_cols, p.smem_cols, true, st, a);
+        } else {
+            s = launch_fft_kernel(k2, dim3((unsigned)p.grid_cols, 1u), p.thr_cols, p.smem_cols, true, st, a);
+        }
+        if (s != JT_OK) return s;
+        s = launch_fft_kernel(k3, dim3((unsigned)p.grid_rows_inv, (unsigned)g), p.thr_rows, p.smem_rows, true, st, a, out + b0 * img_elems);
+        if (s != JT_OK) return s;
+    }
+    return JT_OK;
 }
 
-jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker, void* workspace,
-                          void* out, cudaStream_t st) {
-    FftPlan p = plan_fft(ny, nx, ky, kx);
+jt_status launch_conv_fft(jt_dtype dtype, int64_t B, int ny, int nx, const void* img, int ky, int kx, const void* ker,
+                          void* workspace, void* out, cudaStream_t st) {
+    FftPlan p = plan_fft(ny, nx, ky, kx, B);
     if (!p.ok) return JT_ERR_UNSUPPORTED;
-    return dtype == JT_F32 ? conv_fft_t<float>(p, (const float*)img, (const float*)ker, workspace, (float*)out, st)
-                           : conv_fft_t<double>(p, (const double*)img, (const double*)ker, workspace, (double*)out, st);
+    return dtype == JT_F32 ? conv_fft_t<float>(p, B, (const float*)img, (const float*)ker, workspace, (float*)out, st)
+                           : conv_fft_t<double>(p, B, (const double*)img, (const double*)ker, workspace, (double*)out, st);
 }
 
 }  // namespace jt

@@ -65,13 +65,13 @@ jt_conv_method resolve_conv_method(jt_dtype dtype, int64_t B, int ny, int nx, in
 bool      conv_direct_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
 size_t    conv_direct_workspace_bytes(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
 double    conv_direct_estimate_us(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
-double    conv_fft_estimate_us(jt_dtype dtype, int ny, int nx, int ky, int kx);
+double    conv_fft_estimate_us(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
 jt_status launch_conv_direct(jt_dtype dtype, int64_t B, int ny, int nx, const void* img, int ky, int kx, const void* ker,
                              void* workspace, void* out, cudaStream_t st);   // B images [B][ny][nx], one kernel
 bool      conv_fft_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
-size_t    fft_conv_workspace_bytes(jt_dtype dtype, int ny, int nx, int ky, int kx);
-jt_status launch_conv_fft(jt_dtype dtype, int ny, int nx, const void* img, int ky, int kx, const void* ker,
-                          void* workspace, void* out, cudaStream_t st);
+size_t    fft_conv_workspace_bytes(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
+jt_status launch_conv_fft(jt_dtype dtype, int64_t B, int ny, int nx, const void* img, int ky, int kx, const void* ker,
+                          void* workspace, void* out, cudaStream_t st);   // B images [B][ny][nx], one kernel
 
 // ---- batch (jt_batch.cu); data / sigma / chi2 non-null: chi^2 accumulated in the kernel, out may then be null ----
 jt_status launch_batch(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
