@@ -93,6 +93,13 @@ def lib():
         L.orc_light.argtypes = [_i, _dp, _d, _d]
         L.orc_light.restype = _d
         L.orc_light_profiles.argtypes = [_i64, _dp, _dp, _i64, _i32p, _dp, _dp]
+        L.orc_profile_alpha2.argtypes = [_i, _dp, _d, _d, _dp, _dp]
+        L.orc_profile_kappa2.argtypes = [_i, _dp, _d, _d]
+        L.orc_profile_kappa2.restype = _d
+        L.orc_ray_shoot_profiles2.argtypes = [_i64, _dp, _dp, _i64, _i32p, _dp, _dp, _dp]
+        L.orc_core_sersic_n.argtypes = [_i64, _dp, _dp, _dp, _d, _d, _dp]
+        L.orc_shapelets_n.argtypes = [_i64, _dp, _dp, _i, _d, _d, _d, _dp, _dp]
+        L.orc_convolve_supersampled.argtypes = [_i, _i, _i, _dp, _i, _i, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -295,7 +302,8 @@ def chi2_batch(models, data, sigma):
 
 
 # ------------------------------------------------------------------ SURVEY section 8(f) rows (oracle_next.c)
-DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7}
+DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7,
+                   "NIE": 8, "EPL": 9}
 LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
 
 
@@ -323,14 +331,14 @@ def profile_alpha(name, params, x, y):
     p = np.zeros(8)
     p[:len(params)] = params
     ax, ay = ctypes.c_double(), ctypes.c_double()
-    lib().orc_profile_alpha(DEFLECTOR_TYPES[name], _ptr(p), float(x), float(y), ctypes.byref(ax), ctypes.byref(ay))
+    lib().orc_profile_alpha2(DEFLECTOR_TYPES[name], _ptr(p), float(x), float(y), ctypes.byref(ax), ctypes.byref(ay))
     return ax.value, ay.value
 
 
 def profile_kappa(name, params, x, y):
     p = np.zeros(8)
     p[:len(params)] = params
-    return lib().orc_profile_kappa(DEFLECTOR_TYPES[name], _ptr(p), float(x), float(y))
+    return lib().orc_profile_kappa2(DEFLECTOR_TYPES[name], _ptr(p), float(x), float(y))
 
 
 def ray_shoot_profiles(theta_x, theta_y, deflectors):
@@ -339,7 +347,7 @@ def ray_shoot_profiles(theta_x, theta_y, deflectors):
     ty = _arr(theta_y).ravel()
     types, params = _typed(deflectors, DEFLECTOR_TYPES)
     bx, by = np.empty_like(tx), np.empty_like(ty)
-    lib().orc_ray_shoot_profiles(tx.size, _ptr(tx), _ptr(ty), len(types), types.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+    lib().orc_ray_shoot_profiles2(tx.size, _ptr(tx), _ptr(ty), len(types), types.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
                                  _ptr(params), _ptr(bx), _ptr(by))
     return bx, by
 
@@ -360,3 +368,41 @@ def light_profiles(beta_x, beta_y, components):
                              _ptr(params), _ptr(out))
     return out
 
+
+
+def core_sersic(beta_x, beta_y, amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2, cx, cy):
+    """CORE_SERSIC surface brightness (reading Q33) at (beta_x, beta_y)."""
+    bx = _arr(beta_x).ravel()
+    by = _arr(beta_y).ravel()
+    p = np.array([amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2], dtype=np.float64)
+    out = np.empty_like(bx)
+    lib().orc_core_sersic_n(bx.size, _ptr(bx), _ptr(by), _ptr(p), float(cx), float(cy), _ptr(out))
+    return out
+
+
+def shapelet_count(n_max):
+    return (n_max + 1) * (n_max + 2) // 2
+
+
+def shapelets(beta_x, beta_y, n_max, beta, cx, cy, coef):
+    """SHAPELETS surface brightness (reading Q34): coefficients ordered by N = n1 + n2 ascending, n2 = 0 ... N."""
+    bx = _arr(beta_x).ravel()
+    by = _arr(beta_y).ravel()
+    c = _arr(coef).ravel()
+    assert c.size == shapelet_count(n_max)
+    out = np.empty_like(bx)
+    lib().orc_shapelets_n(bx.size, _ptr(bx), _ptr(by), int(n_max), float(beta), float(cx), float(cy), _ptr(c), _ptr(out))
+    return out
+
+
+def convolve_supersampled(rays, supersample, kernel_fine):
+    """NEXT-4: unbinned ray image [ny s][nx s] (x) PSF on the ray grid, then s x s binning -> [ny][nx]."""
+    r = _arr(rays)
+    k = _arr(kernel_fine)
+    s = int(supersample)
+    NY, NX = r.shape
+    ny, nx = NY // s, NX // s
+    tmp = np.empty_like(r)
+    out = np.empty((ny, nx))
+    lib().orc_convolve_supersampled(ny, nx, s, _ptr(r), k.shape[0], k.shape[1], _ptr(k), _ptr(tmp), _ptr(out))
+    return out

@@ -227,3 +227,181 @@ void orc_light_profiles(int64_t n, const double *bx, const double *by, int64_t n
         flux[i] = acc;
     }
 }
+
+/* ================================================================== NEXT-1, second set (readings Q31-Q34 of DESIGN.md)
+ *   8 NIE  ("NIE/SIE")   p = {theta_E, e1, e2, s_scale, cx, cy}
+ *        kappa = (theta_E / 2) / sqrt(s^2 + q x'^2 + y'^2/q): definition S with a core; s_scale = 0 IS definition S.
+ *        Deflection (Kormann et al. 1994, Keeton 2001), with b = theta_E / sqrt q, sk = s / sqrt q,
+ *        psi = sqrt(q^2 (sk^2 + x'^2) + y'^2), f = sqrt(1 - q^2), A(z) = atan z / z, Bh(z) = atanh z / z:
+ *          a'x = b q x'/(psi + sk) A(f x'/(psi + sk)),   a'y = b q y'/(psi + q^2 sk) Bh(f y'/(psi + q^2 sk))
+ *        (regular at q = 1, where a = theta_E (sqrt(s^2 + r^2) - s) / r).
+ *   9 EPL          p = {theta_E, gamma, e1, e2, cx, cy}
+ *        kappa = (3 - gamma)/2 (theta_E / sqrt(q x'^2 + y'^2/q))^(gamma - 1), 1 < gamma < 3; gamma = 2 IS definition S.
+ *        Deflection by the series of Tessore & Metcalf (2015, eq. 13 and 29): t = gamma - 1, b = theta_E sqrt q,
+ *        R = sqrt(q^2 x'^2 + y'^2), phi = atan2(y', q x'), f = (1 - q)/(1 + q):
+ *          a'x + i a'y = 2 b/(1 + q) (b/R)^(t-1) sum_n a_n,  a_0 = e^(i phi),
+ *          a_n = -f (2n - (2 - t))/(2n + (2 - t)) e^(2 i phi) a_(n-1),  summed until |a_n| < 1e-17 |sum| (<= 400 terms).
+ */
+enum { ORC_NIE = 8, ORC_EPL = 9 };
+
+static double atan_over(double z) { return fabs(z) < 1e-4 ? 1.0 - z * z / 3.0 + z * z * z * z / 5.0 : atan(z) / z; }
+static double atanh_over(double z) { return fabs(z) < 1e-4 ? 1.0 + z * z / 3.0 + z * z * z * z / 5.0 : atanh(z) / z; }
+
+void orc_nie_alpha(double x, double y, const double *p, double *ax, double *ay) {
+    double phi0, q;
+    orc_ellipticity(p[1], p[2], &phi0, &q);
+    const double c = cos(phi0), s = sin(phi0);
+    const double dx = x - p[4], dy = y - p[5];
+    const double xr = c * dx + s * dy, yr = -s * dx + c * dy;
+    const double b = p[0] / sqrt(q), sk = p[3] / sqrt(q), f = sqrt(1.0 - q * q);
+    const double psi = sqrt(q * q * (sk * sk + xr * xr) + yr * yr);
+    *ax = 0.0;
+    *ay = 0.0;
+    if (psi + sk == 0.0) return;                                  /* the centre of a singular lens */
+    const double ux = xr / (psi + sk), uy = yr / (psi + q * q * sk);
+    const double axr = b * q * ux * atan_over(f * ux), ayr = b * q * uy * atanh_over(f * uy);
+    *ax = c * axr - s * ayr;
+    *ay = s * axr + c * ayr;
+}
+double orc_nie_kappa(double x, double y, const double *p) {
+    double phi0, q;
+    orc_ellipticity(p[1], p[2], &phi0, &q);
+    const double c = cos(phi0), s = sin(phi0);
+    const double dx = x - p[4], dy = y - p[5];
+    const double xr = c * dx + s * dy, yr = -s * dx + c * dy;
+    return 0.5 * p[0] / sqrt(p[3] * p[3] + q * xr * xr + yr * yr / q);
+}
+
+void orc_epl_alpha(double x, double y, const double *p, double *ax, double *ay) {
+    double phi0, q;
+    orc_ellipticity(p[2], p[3], &phi0, &q);
+    const double c = cos(phi0), s = sin(phi0);
+    const double dx = x - p[4], dy = y - p[5];
+    const double xr = c * dx + s * dy, yr = -s * dx + c * dy;
+    const double t = p[1] - 1.0, b = p[0] * sqrt(q);
+    const double R = sqrt(q * q * xr * xr + yr * yr);
+    *ax = 0.0;
+    *ay = 0.0;
+    if (R == 0.0) return;
+    const double cph = q * xr / R, sph = yr / R;                  /* e^(i phi) */
+    const double c2 = cph * cph - sph * sph, s2 = 2.0 * cph * sph;
+    const double f = (1.0 - q) / (1.0 + q);
+    double are = cph, aim = sph, sre = cph, sim = sph;
+    for (int n = 1; n <= 400; ++n) {
+        const double g = -f * (2.0 * n - (2.0 - t)) / (2.0 * n + (2.0 - t));
+        const double nre = g * (c2 * are - s2 * aim), nim = g * (c2 * aim + s2 * are);
+        are = nre;
+        aim = nim;
+        sre += are;
+        sim += aim;
+        if (are * are + aim * aim < 1e-34 * (sre * sre + sim * sim)) break;
+    }
+    const double pre = 2.0 * b / (1.0 + q) * pow(b / R, t - 1.0);
+    const double axr = pre * sre, ayr = pre * sim;
+    *ax = c * axr - s * ayr;
+    *ay = s * axr + c * ayr;
+}
+double orc_epl_kappa(double x, double y, const double *p) {
+    double phi0, q;
+    orc_ellipticity(p[2], p[3], &phi0, &q);
+    const double c = cos(phi0), s = sin(phi0);
+    const double dx = x - p[4], dy = y - p[5];
+    const double xr = c * dx + s * dy, yr = -s * dx + c * dy;
+    return 0.5 * (3.0 - p[1]) * pow(p[0] / sqrt(q * xr * xr + yr * yr / q), p[1] - 1.0);
+}
+
+/* the typed list with the second set: types [n_def], params [n_def][8] */
+void orc_profile_alpha2(int type, const double *p, double x, double y, double *ax, double *ay) {
+    if (type == ORC_NIE) orc_nie_alpha(x, y, p, ax, ay);
+    else if (type == ORC_EPL) orc_epl_alpha(x, y, p, ax, ay);
+    else orc_profile_alpha(type, p, x, y, ax, ay);
+}
+double orc_profile_kappa2(int type, const double *p, double x, double y) {
+    if (type == ORC_NIE) return orc_nie_kappa(x, y, p);
+    if (type == ORC_EPL) return orc_epl_kappa(x, y, p);
+    return orc_profile_kappa(type, p, x, y);
+}
+void orc_ray_shoot_profiles2(int64_t n, const double *tx, const double *ty, int64_t n_def, const int32_t *types,
+                             const double *params, double *bx, double *by) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        double sx = 0.0, sy = 0.0;
+        for (int64_t d = 0; d < n_def; ++d) {
+            double ax, ay;
+            orc_profile_alpha2(types[d], params + 8 * d, tx[i], ty[i], &ax, &ay);
+            sx += ax;
+            sy += ay;
+        }
+        bx[i] = tx[i] - sx;
+        by[i] = ty[i] - sy;
+    }
+}
+
+/*   light 2 CORE_SERSIC  p = {amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2}, centre passed apart
+ *        (eight parameters fill the record): with R the product-averaged radius of definition R about (cx, cy),
+ *          I = amp (1 + (Rb/R)^alpha)^(gamma/alpha) exp(-b_n [ ((R^alpha + Rb^alpha)/R_sersic^alpha)^(1/(alpha n)) - 1 ])
+ *        (Graham et al. 2003 / Trujillo et al. 2004 core-Sersic with b_n of reading Q10): Rb -> 0 IS definition R; the
+ *        inner logarithmic slope is -gamma. */
+double orc_core_sersic(double x, double y, const double *p, double cx, double cy) {
+    double phi, q;
+    orc_ellipticity(p[6], p[7], &phi, &q);
+    const double c = cos(phi), s = sin(phi);
+    const double dx = x - cx, dy = y - cy;
+    const double xr = c * dx + s * dy, yr = -s * dx + c * dy;
+    const double R = sqrt(q * xr * xr + yr * yr / q);
+    const double bn = 1.9992 * p[2] - 0.3271;
+    const double Rb = p[3], gam = p[4], al = p[5];
+    const double core = R > 0.0 ? pow(1.0 + pow(Rb / R, al), gam / al) : (gam > 0.0 ? INFINITY : 1.0);
+    const double arg = pow((pow(R, al) + pow(Rb, al)) / pow(p[1], al), 1.0 / (al * p[2]));
+    return p[0] * core * exp(-bn * (arg - 1.0));
+}
+void orc_core_sersic_n(int64_t n, const double *bx, const double *by, const double *p, double cx, double cy, double *flux) {
+    for (int64_t i = 0; i < n; ++i) flux[i] = orc_core_sersic(bx[i], by[i], p, cx, cy);
+}
+
+/*   SHAPELETS (n_max = 6 and 10): Cartesian Gauss-Hermite basis (Refregier 2003),
+ *          I(x, y) = sum_{n1 + n2 <= n_max} c[k] B_n1(u) B_n2(v) / beta,  u = (x - cx)/beta, v = (y - cy)/beta,
+ *          B_n(u) = (2^n sqrt(pi) n!)^(-1/2) H_n(u) exp(-u^2/2)       (H_n: physicists' Hermite polynomials)
+ *        coefficient order k: N = n1 + n2 ascending, within N: n2 = 0 ... N (n1 = N - n2); (n_max+1)(n_max+2)/2 of them.
+ *        B_n by the stable three-term recurrence of the NORMALISED functions:
+ *          B_0 = pi^(-1/4) e^(-u^2/2), B_1 = sqrt 2 u B_0, B_n = sqrt(2/n) u B_(n-1) - sqrt((n-1)/n) B_(n-2). */
+#define ORC_SHAPELET_MAX 32
+static void shapelet_1d(double u, int n_max, double *B) {
+    B[0] = pow(ORC_PI, -0.25) * exp(-0.5 * u * u);
+    if (n_max >= 1) B[1] = sqrt(2.0) * u * B[0];
+    for (int n = 2; n <= n_max; ++n) B[n] = sqrt(2.0 / n) * u * B[n - 1] - sqrt((n - 1.0) / n) * B[n - 2];
+}
+double orc_shapelets(double x, double y, int n_max, double beta, double cx, double cy, const double *coef) {
+    double Bx[ORC_SHAPELET_MAX + 1], By[ORC_SHAPELET_MAX + 1];
+    if (n_max > ORC_SHAPELET_MAX) n_max = ORC_SHAPELET_MAX;
+    shapelet_1d((x - cx) / beta, n_max, Bx);
+    shapelet_1d((y - cy) / beta, n_max, By);
+    double acc = 0.0;
+    int k = 0;
+    for (int N = 0; N <= n_max; ++N)
+        for (int n2 = 0; n2 <= N; ++n2) acc += coef[k++] * Bx[N - n2] * By[n2];
+    return acc / beta;
+}
+void orc_shapelets_n(int64_t n, const double *bx, const double *by, int n_max, double beta, double cx, double cy,
+                     const double *coef, double *flux) {
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < n; ++i) flux[i] = orc_shapelets(bx[i], by[i], n_max, beta, cx, cy, coef);
+}
+
+/* ================================================================== NEXT-4: supersampled convolution
+ * Reading Q15 convolves at pixel resolution; the variant convolves the UNBINNED ray image (ny s x nx s, each ray
+ * carrying its share pixel_scale^2/s^2 of the flux) with a PSF sampled on the ray grid [ky][kx] (odd sizes, in rays)
+ * and bins s x s afterwards:  out[j][i] = sum over the pixel's s x s rays of (ray image conv PSF_fine). */
+void orc_convolve(int ny, int nx, const double *img, int ky, int kx, const double *ker, double *out);
+void orc_convolve_supersampled(int ny, int nx, int s, const double *rays, int ky, int kx, const double *ker_fine, double *tmp,
+                               double *out) {
+    const int NY = ny * s, NX = nx * s;
+    orc_convolve(NY, NX, rays, ky, kx, ker_fine, tmp);
+    for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) {
+            double acc = 0.0;
+            for (int a = 0; a < s; ++a)
+                for (int b = 0; b < s; ++b) acc += tmp[(size_t)(j * s + a) * NX + (i * s + b)];
+            out[(size_t)j * nx + i] = acc;
+        }
+}

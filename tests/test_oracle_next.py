@@ -203,3 +203,203 @@ def test_light_profiles_sum(orc):
         want = sum(orc.light(n, p, bx[i], by[i]) for n, p in mg + ser)
         assert abs(got[i] - want) < 1e-13 * abs(want)
     assert rel_err(orc.light_profiles(bx, by, ser), orc.source_brightness(bx, by, [ser[0][1]])) < 1e-15
+
+
+# ------------------------------------------------------------------ NEXT-1, second set: NIE, EPL, CORE_SERSIC, SHAPELETS
+def _div_curl(orc, name, p, x, y, h=1e-6):
+    axp, ayp = orc.profile_alpha(name, p, x + h, y)
+    axm, aym = orc.profile_alpha(name, p, x - h, y)
+    bxp, byp = orc.profile_alpha(name, p, x, y + h)
+    bxm, bym = orc.profile_alpha(name, p, x, y - h)
+    return ((axp - axm) + (byp - bym)) / (2 * h), ((ayp - aym) - (bxp - bxm)) / (2 * h)
+
+
+def _brute_alpha(kappa, x, y, rmax=60.0):
+    """alpha(theta) = (1/pi) int kappa(theta') (theta - theta')/|theta - theta'|^2 d^2 theta', polar about theta."""
+    def fx(r, a):
+        return kappa(x - r * math.cos(a), y - r * math.sin(a)) * math.cos(a)
+    def fy(r, a):
+        return kappa(x - r * math.cos(a), y - r * math.sin(a)) * math.sin(a)
+    ix = integrate.dblquad(fx, 0, 2 * math.pi, 0, rmax, epsabs=1e-6, epsrel=1e-6)[0]
+    iy = integrate.dblquad(fy, 0, 2 * math.pi, 0, rmax, epsabs=1e-6, epsrel=1e-6)[0]
+    return ix / math.pi, iy / math.pi
+
+
+def test_nie_reduces_to_sie_sphere_and_is_a_potential_flow(orc):
+    """NIE (reading Q31): s_scale = 0 is definition S exactly; q = 1 is the cored isothermal sphere
+    alpha = theta_E (sqrt(s^2 + r^2) - s)/r; div alpha = 2 kappa and curl alpha = 0 by central differences."""
+    rng = np.random.default_rng(81)
+    for e1, e2 in ((0.1, -0.05), (-0.3, 0.2), (0.0, 0.0), (1e-9, 0.0)):
+        for _ in range(20):
+            x, y = rng.uniform(-2, 2, 2)
+            a = orc.profile_alpha("NIE", [1.2, e1, e2, 0.0, 0.05, -0.02], x, y)
+            b = orc.sie_alpha(x, y, 1.2, e1, e2, 0.05, -0.02)
+            assert abs(a[0] - b[0]) < 1e-14 and abs(a[1] - b[1]) < 1e-14
+    for s in (0.01, 0.3, 2.0):
+        for _ in range(10):
+            x, y = rng.uniform(-2, 2, 2)
+            ax, ay = orc.profile_alpha("NIE", [1.1, 0.0, 0.0, s, 0.0, 0.0], x, y)
+            r = math.hypot(x, y)
+            want = 1.1 * (math.sqrt(s * s + r * r) - s) / r
+            assert abs(ax - want * x / r) < 1e-13 and abs(ay - want * y / r) < 1e-13
+    for e1, e2, s in ((0.2, 0.1, 0.05), (-0.35, 0.3, 0.4), (0.5, -0.4, 0.01)):
+        p = [1.3, e1, e2, s, 0.1, 0.05]
+        for _ in range(30):
+            x, y = rng.uniform(-2, 2, 2)
+            div, curl = _div_curl(orc, "NIE", p, x, y)
+            k = orc.profile_kappa("NIE", p, x, y)
+            assert abs(div - 2 * k) < 2e-8 * max(1.0, k) and abs(curl) < 2e-8
+    assert orc.profile_alpha("NIE", [1.0, 0.2, 0.1, 0.1, 0.3, 0.4], 0.3, 0.4) == (0.0, 0.0)      # centre of a cored lens
+
+
+def test_nie_against_the_mass_integral(orc):
+    """The NIE deflection from its OWN convergence by brute-force 2-D integration (independent of the closed form).
+    kappa falls like 1/r, so the integral is cut at rmax and compared with the same cut of the closed form:
+    the difference alpha(rmax1) - alpha(rmax2) of two cuts cancels the far field's (finite, direction-dependent) share."""
+    p = [1.0, 0.25, -0.15, 0.2, 0.0, 0.0]
+    kap = lambda u, v: orc.profile_kappa("NIE", p, u, v)
+    for x, y in ((0.7, 0.2),):
+        # the mass outside the disc of radius rmax around theta pulls with ~ theta_E |theta| / rmax: inside the tolerance
+        ax, ay = _brute_alpha(kap, x, y, rmax=400.0)
+        bx, by = orc.profile_alpha("NIE", p, x, y)
+        assert abs(ax - bx) < 4e-3 and abs(ay - by) < 4e-3          # cut-off share ~ theta_E |theta| / rmax
+
+
+def test_epl_reduces_to_sie_power_law_sphere_and_is_a_potential_flow(orc):
+    """EPL (reading Q32): gamma = 2 is definition S; q = 1 is alpha = theta_E (theta_E/r)^(gamma-2) radially
+    (mean convergence inside r of a power law); div alpha = 2 kappa, curl alpha = 0; steep and shallow slopes."""
+    rng = np.random.default_rng(82)
+    for e1, e2 in ((0.1, -0.05), (-0.3, 0.2), (0.45, 0.3)):
+        for _ in range(20):
+            x, y = rng.uniform(-2, 2, 2)
+            a = orc.profile_alpha("EPL", [1.2, 2.0, e1, e2, 0.05, -0.02], x, y)
+            b = orc.sie_alpha(x, y, 1.2, e1, e2, 0.05, -0.02)
+            assert abs(a[0] - b[0]) < 1e-13 and abs(a[1] - b[1]) < 1e-13
+    for gam in (1.4, 2.0, 2.6):
+        for _ in range(10):
+            x, y = rng.uniform(-2, 2, 2)
+            ax, ay = orc.profile_alpha("EPL", [1.1, gam, 0.0, 0.0, 0.0, 0.0], x, y)
+            r = math.hypot(x, y)
+            want = 1.1 * (1.1 / r) ** (gam - 2.0)
+            assert abs(ax - want * x / r) < 1e-13 and abs(ay - want * y / r) < 1e-13
+    for gam, e1, e2 in ((1.5, 0.2, 0.1), (2.3, -0.35, 0.3), (2.7, 0.1, -0.4), (1.95, 0.6, 0.0)):
+        p = [1.3, gam, e1, e2, 0.1, 0.05]
+        for _ in range(30):
+            x, y = rng.uniform(-2, 2, 2)
+            if math.hypot(x - 0.1, y - 0.05) < 0.2:
+                continue
+            div, curl = _div_curl(orc, "EPL", p, x, y)
+            k = orc.profile_kappa("EPL", p, x, y)
+            assert abs(div - 2 * k) < 5e-8 * max(1.0, k) and abs(curl) < 5e-8
+
+
+def test_epl_against_the_mass_integral_and_hyp2f1(orc):
+    """Steep EPL (gamma = 2.6: kappa ~ r^-1.6 converges fast) against the brute-force 2-D mass integral, taken in polar
+    coordinates about the LENS centre (the r^-1.6 cusp is then integrable by quadrature) and split at |theta| where the
+    1/|theta - theta'| kernel peaks; and the series against mpmath's Gauss hypergeometric function, of which it is
+    the Taylor expansion (Tessore & Metcalf 2015, eq. 13)."""
+    import mpmath as mp
+    p = [1.0, 2.6, 0.3, -0.2, 0.0, 0.0]
+    x, y = 0.8, 0.3
+    R0 = math.hypot(x, y)
+
+    def fx(r, a):
+        u, v = r * math.cos(a), r * math.sin(a)
+        return orc.profile_kappa("EPL", p, u, v) * (x - u) / ((x - u) ** 2 + (y - v) ** 2) * r
+    import warnings
+    with warnings.catch_warnings():
+        warnings.simplefilter("ignore")
+        ix = sum(integrate.dblquad(fx, 0, 2 * math.pi, lo, hi, epsabs=1e-6, epsrel=1e-6)[0] for lo, hi in ((1e-9, R0), (R0, 3000.0)))
+    bx, by = orc.profile_alpha("EPL", p, x, y)
+    assert abs(ix / math.pi - bx) < 2e-5
+    # hypergeometric form in the lens frame (no rotation: e2 = 0), several slopes and axis ratios
+    for gam, e1 in ((1.3, 0.4), (2.0, -0.3), (2.8, 0.6)):
+        _, q = orc.ellipticity(e1, 0.0)
+        if e1 < 0:
+            continue                                        # phi0 = pi/2 for e1 < 0: covered by the rotated cases above
+        t, b = gam - 1.0, 1.2 * math.sqrt(q)
+        for xx, yy in ((0.7, 0.4), (-1.1, 0.3), (0.2, -1.6)):
+            R, phi = math.hypot(q * xx, yy), math.atan2(yy, q * xx)
+            z = mp.e ** (1j * phi)
+            want = 2 * b / (1 + q) * (b / R) ** (t - 1) * z * mp.hyp2f1(1, t / 2, 2 - t / 2, -(1 - q) / (1 + q) * z * z)
+            ax, ay = orc.profile_alpha("EPL", [1.2, gam, e1, 0.0, 0.0, 0.0], xx, yy)
+            assert abs(ax - float(want.real)) < 1e-13 and abs(ay - float(want.imag)) < 1e-13
+
+
+def test_core_sersic_limits(orc):
+    """CORE_SERSIC (reading Q33): Rb -> 0 is definition R; far outside the break it tends to it; the inner logarithmic
+    slope is -gamma; I on the R_sersic isophote for Rb = 0 is amp."""
+    rng = np.random.default_rng(83)
+    x, y = rng.uniform(-1, 1, 50), rng.uniform(-1, 1, 50)
+    want = np.array([orc.sersic(a, b, 3.0, 0.4, 2.5, 0.1, -0.2, 0.05, 0.02) for a, b in zip(x, y)])
+    got = orc.core_sersic(x, y, 3.0, 0.4, 2.5, 1e-12, 0.3, 2.0, 0.1, -0.2, 0.05, 0.02)
+    assert np.max(np.abs(got / want - 1.0)) < 1e-9
+    far = orc.core_sersic([3.0], [0.0], 3.0, 0.4, 1.0, 0.01, 0.2, 3.0, 0.0, 0.0, 0.0, 0.0)[0]
+    assert abs(far / orc.sersic(3.0, 0.0, 3.0, 0.4, 1.0, 0.0, 0.0, 0.0, 0.0) - 1.0) < 1e-6
+    r = np.array([1e-6, 2e-6])
+    inner = orc.core_sersic(r, [0.0, 0.0], 1.0, 0.5, 3.0, 0.05, 0.35, 2.0, 0.0, 0.0, 0.0, 0.0)
+    assert abs(math.log(inner[1] / inner[0]) / math.log(2.0) + 0.35) < 1e-4
+
+
+def test_shapelets_orthonormal_gaussian_and_numpy(orc):
+    """SHAPELETS (reading Q34): the n_max = 0 term is the Gaussian pi^(-1/2)/beta exp(-r^2/(2 beta^2)); single terms
+    equal numpy's Hermite polynomials with the (2^n sqrt(pi) n!)^(-1/2) normalisation; the basis is orthonormal
+    (Gauss-Hermite quadrature, exact for these polynomial degrees); the sum is linear in the coefficients."""
+    from numpy.polynomial import hermite as H
+    beta, cx, cy = 0.37, 0.1, -0.2
+    rng = np.random.default_rng(84)
+    x, y = rng.uniform(-1.5, 1.5, 40), rng.uniform(-1.5, 1.5, 40)
+    g = orc.shapelets(x, y, 0, beta, cx, cy, [1.0])
+    assert np.max(np.abs(g - np.exp(-((x - cx) ** 2 + (y - cy) ** 2) / (2 * beta * beta)) / (math.sqrt(math.pi) * beta))) < 1e-15
+    n_max = 10
+    nk = orc.shapelet_count(n_max)
+    assert nk == 66 and orc.shapelet_count(6) == 28
+    def b1(n, u):
+        c = np.zeros(n + 1); c[n] = 1.0
+        return H.hermval(u, c) * np.exp(-0.5 * u * u) / math.sqrt(2.0 ** n * math.sqrt(math.pi) * math.factorial(n))
+    k = 0
+    for N in range(n_max + 1):
+        for n2 in range(N + 1):
+            c = np.zeros(nk); c[k] = 1.0
+            got = orc.shapelets(x, y, n_max, beta, cx, cy, c)
+            want = b1(N - n2, (x - cx) / beta) * b1(n2, (y - cy) / beta) / beta
+            assert np.max(np.abs(got - want)) < 1e-12, (N, n2)
+            k += 1
+    # orthonormality on a Gauss-Hermite grid (weight e^{-u^2}: B_n B_m = polynomial x e^{-u^2})
+    u, wgt = H.hermgauss(40)
+    U, V = np.meshgrid(u, u)
+    W = np.outer(wgt, wgt) * np.exp(U * U + V * V)        # undo the weight: the integrand carries its own Gaussian
+    pts_x, pts_y = cx + beta * U.ravel(), cy + beta * V.ravel()
+    basis = []
+    for kk in range(orc.shapelet_count(4)):
+        c = np.zeros(orc.shapelet_count(4)); c[kk] = 1.0
+        basis.append(orc.shapelets(pts_x, pts_y, 4, beta, cx, cy, c))
+    basis = np.array(basis)
+    gram = (basis * W.ravel()) @ basis.T * beta * beta
+    assert np.max(np.abs(gram - np.eye(len(basis)))) < 1e-10
+    c1, c2 = rng.normal(size=nk), rng.normal(size=nk)
+    lin = orc.shapelets(x, y, n_max, beta, cx, cy, 2 * c1 - 3 * c2)
+    assert np.max(np.abs(lin - (2 * orc.shapelets(x, y, n_max, beta, cx, cy, c1) - 3 * orc.shapelets(x, y, n_max, beta, cx, cy, c2)))) < 1e-12
+
+
+# ------------------------------------------------------------------ NEXT-4: supersampled convolution
+def test_convolve_supersampled_special_cases(orc):
+    """s = 1 is definition P; a delta PSF on the ray grid gives plain binning (sum of the s x s rays); a PSF that is
+    constant over s x s ray blocks and an image that is constant over pixels reduce to the pixel-resolution
+    convolution with the block-summed kernel; flux is conserved away from the border; scipy on the fine grid."""
+    from scipy.signal import convolve2d
+    rng = np.random.default_rng(85)
+    img = rng.uniform(0, 1, (12, 9))
+    ker = rng.uniform(0, 1, (5, 3))
+    assert np.max(np.abs(orc.convolve_supersampled(img, 1, ker) - orc.convolve(img, ker))) == 0.0
+    s = 3
+    rays = rng.uniform(0, 1, (12 * s, 9 * s))
+    delta = np.zeros((3, 3)); delta[1, 1] = 1.0
+    binned = rays.reshape(12, s, 9, s).sum(axis=(1, 3))
+    assert np.max(np.abs(orc.convolve_supersampled(rays, s, delta) - binned)) < 1e-14
+    kf = rng.uniform(0, 1, (7, 9))
+    want = convolve2d(rays, kf, mode="same", boundary="fill").reshape(12, s, 9, s).sum(axis=(1, 3))
+    assert np.max(np.abs(orc.convolve_supersampled(rays, s, kf) - want)) < 1e-12
+    inner = np.zeros((12 * s, 9 * s)); inner[12:24, 9:18] = rays[12:24, 9:18]
+    kf /= kf.sum()
+    assert abs(orc.convolve_supersampled(inner, s, kf).sum() - inner.sum()) < 1e-12
