@@ -199,13 +199,15 @@ JT_API jt_status jt_lensing_maps(jt_dtype dtype, int64_t n, const void *theta_x,
  *   JT_DEFL_SIE         (:80)           theta_E, e1, e2, cx, cy       definition S
  *   JT_DEFL_SHEAR       (:85)           gamma1, gamma2                definition H
  *   JT_DEFL_TNFW        (:87)           Rs, alpha_Rs, r_trunc, cx, cy definition T
+ *   JT_DEFL_NIE         (:80)           theta_E, e1, e2, s_scale, cx, cy   definition S with a core (reading Q31)
+ *   JT_DEFL_EPL         (:66-70)        theta_E, gamma, e1, e2, cx, cy     elliptical power law, 1 < gamma < 3 (Q32)
  *   light
  *   JT_LIGHT_SERSIC_ELLIPSE   (:103)    amp, R_sersic, n_sersic, e1, e2, cx, cy      definition R
  *   JT_LIGHT_GAUSSIAN_ELLIPSE (:98-101) amp (total flux), sigma, e1, e2, cx, cy; GAUSSIAN is e1 = e2 = 0,
  *                                       MULTI_GAUSSIAN(_ELLIPSE) is several records
  * Formulas: DESIGN.md readings Q26-Q30.  Unknown types contribute nothing. */
 typedef enum { JT_DEFL_CONVERGENCE = 0, JT_DEFL_SIS = 1, JT_DEFL_NFW = 2, JT_DEFL_HERNQUIST = 3, JT_DEFL_PJAFFE = 4,
-               JT_DEFL_SIE = 5, JT_DEFL_SHEAR = 6, JT_DEFL_TNFW = 7 } jt_deflector_type;
+               JT_DEFL_SIE = 5, JT_DEFL_SHEAR = 6, JT_DEFL_TNFW = 7, JT_DEFL_NIE = 8, JT_DEFL_EPL = 9 } jt_deflector_type;
 typedef enum { JT_LIGHT_SERSIC_ELLIPSE = 0, JT_LIGHT_GAUSSIAN_ELLIPSE = 1 } jt_light_type;
 typedef struct { int32_t type; int32_t reserved; double p[8]; } jt_profile;
 /* beta = theta - sum of the n_def deflectors.  theta, beta: device [n]; deflectors: device [n_def]. */
@@ -214,6 +216,29 @@ JT_API jt_status jt_ray_shoot_profiles(jt_dtype dtype, int64_t n, const void *th
 /* flux[i] = sum of the n_comp light components at (beta_x[i], beta_y[i]) (surface brightness). */
 JT_API jt_status jt_light_profiles(jt_dtype dtype, int64_t n, const void *beta_x, const void *beta_y, int64_t n_comp,
                             const jt_profile *components, void *flux, void *stream);
+
+/* CORE_SERSIC (reading Q33): params (HOST, 10 doubles) = amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2,
+ * cx, cy;  I = amp (1 + (Rb/R)^alpha)^(gamma/alpha) exp(-b_n [((R^alpha + Rb^alpha)/R_sersic^alpha)^(1/(alpha n)) - 1]),
+ * R the product-averaged radius of definition R.  beta_x, beta_y, flux: device [n]. */
+JT_API jt_status jt_light_core_sersic(jt_dtype dtype, int64_t n, const void *beta_x, const void *beta_y, const double *params,
+                               void *flux, void *stream);
+/* SHAPELETS (n_max = 6 and 10; reading Q34): Cartesian Gauss-Hermite basis of scale beta about
+ * (cx, cy); coef: device [(n_max+1)(n_max+2)/2] of the call's dtype, ordered by N = n1 + n2 ascending and, within N, by
+ * n2 = 0 ... N;  flux[i] = sum_k coef[k] B_n1(u) B_n2(v) / beta.  n_max <= JT_MAX_SHAPELET_ORDER. */
+#define JT_MAX_SHAPELET_ORDER 12
+JT_API jt_status jt_light_shapelets(jt_dtype dtype, int64_t n, const void *beta_x, const void *beta_y, int32_t n_max, double beta,
+                             double cx, double cy, const void *coef, void *flux, void *stream);
+
+/* NEXT-4 (not in the paper): jt_simulate_image with the convolution done at RAY resolution --
+ * the unbinned ray image [ny s][nx s] (each ray carrying pixel_scale^2/s^2 of surface brightness) is convolved with a
+ * PSF sampled on the ray grid, kernel_fine: device [ky][kx] (odd sizes, in rays), and binned s x s afterwards.
+ * out: device [ny][nx].  workspace >= jt_simulate_image_supersampled_psf_workspace_bytes(...). */
+JT_API size_t    jt_simulate_image_supersampled_psf_workspace_bytes(jt_dtype dtype, const jt_grid *grid, int64_t n_tnfw, int32_t ky,
+                                                             int32_t kx, jt_conv_method method);
+JT_API jt_status jt_simulate_image_supersampled_psf(jt_dtype dtype, const jt_grid *grid, const jt_lens *lens,
+                                             const jt_sources *sources, int32_t ky, int32_t kx, const void *kernel_fine,
+                                             jt_conv_method method, void *workspace, size_t workspace_bytes, void *out,
+                                             void *stream);
 
 /* Measurement aid (bench.py's roofline leg).  jt_profile_enable(1) makes every following
  * jt_simulate_image call on this host thread record CUDA events on its stream before the ray-tracing kernel, between it

@@ -11,6 +11,9 @@ from .binding import (  # noqa: F401
     lensing_maps,
     ray_shoot_profiles,
     light_profiles,
+    light_core_sersic,
+    light_shapelets,
+    simulate_image_supersampled_psf,
     profile_records,
     DEFLECTOR_TYPES,
     LIGHT_TYPES,

@@ -107,6 +107,12 @@ def lib():
         L.jt_lensing_maps.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Lens), vp, vp, vp, vp, vp]
         L.jt_ray_shoot_profiles.argtypes = [ctypes.c_int, i64, vp, vp, i64, vp, vp, vp, vp]
         L.jt_light_profiles.argtypes = [ctypes.c_int, i64, vp, vp, i64, vp, vp, vp]
+        L.jt_light_core_sersic.argtypes = [ctypes.c_int, i64, vp, vp, dbl, vp, vp]
+        L.jt_light_shapelets.argtypes = [ctypes.c_int, i64, vp, vp, i32, ctypes.c_double, ctypes.c_double, ctypes.c_double, vp, vp, vp]
+        L.jt_simulate_image_supersampled_psf_workspace_bytes.restype = sz
+        L.jt_simulate_image_supersampled_psf_workspace_bytes.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), i64, i32, i32, ctypes.c_int]
+        L.jt_simulate_image_supersampled_psf.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), ctypes.POINTER(_Lens),
+                                                         ctypes.POINTER(_Sources), i32, i32, vp, ctypes.c_int, vp, sz, vp, vp]
         del dbl
         L.jt_kernel_launches.restype = ctypes.c_uint64
         L.jt_profile_enable.argtypes = [ctypes.c_int]
@@ -442,7 +448,8 @@ def lensing_maps(theta_x, theta_y, sie=None, shear=None, tnfw=None, stream=None)
     return tuple(out)
 
 
-DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7}
+DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7,
+                   "NIE": 8, "EPL": 9}
 LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
 _PROFILE_DT = np.dtype([("type", np.int32), ("reserved", np.int32), ("p", np.float64, 8)])     # jt_profile, 72 bytes
 
@@ -477,3 +484,44 @@ def light_profiles(beta_x, beta_y, components, stream=None):
     _check(lib().jt_light_profiles(code, beta_x.numel(), _ptr(beta_x), _ptr(beta_y), recs.numel() // 72,
                                    _ptr(recs) if recs.numel() else None, _ptr(flux), _stream(stream)), "jt_light_profiles")
     return flux
+
+
+def light_core_sersic(beta_x, beta_y, params, stream=None):
+    """jt_light_core_sersic: params = (amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2, cx, cy)."""
+    _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y")
+    p = (ctypes.c_double * 10)(*[float(v) for v in params])
+    flux = torch.empty_like(beta_x)
+    _check(lib().jt_light_core_sersic(_dt(beta_x), beta_x.numel(), _ptr(beta_x), _ptr(beta_y), p, _ptr(flux), _stream(stream)),
+           "jt_light_core_sersic")
+    return flux
+
+
+def light_shapelets(beta_x, beta_y, n_max, beta, cx, cy, coef, stream=None):
+    """jt_light_shapelets: coef is a device tensor [(n_max+1)(n_max+2)/2] of the call's dtype (N ascending, n2 = 0..N)."""
+    _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y"), _dev(coef, "coef")
+    if _dt(coef) != _dt(beta_x) or coef.numel() != (n_max + 1) * (n_max + 2) // 2:
+        raise TypeError("coef: wrong dtype or length")
+    flux = torch.empty_like(beta_x)
+    _check(lib().jt_light_shapelets(_dt(beta_x), beta_x.numel(), _ptr(beta_x), _ptr(beta_y), int(n_max), float(beta), float(cx),
+                                    float(cy), _ptr(coef), _ptr(flux), _stream(stream)), "jt_light_shapelets")
+    return flux
+
+
+def simulate_image_supersampled_psf(grid, sie, shear, tnfw, sources, psf_fine, dtype=None, method="auto", workspace=None, out=None,
+                                    stream=None):
+    """jt_simulate_image_supersampled_psf (NEXT-4): psf_fine is sampled on the RAY grid [ky][kx]."""
+    _dev(psf_fine, "psf_fine")
+    code = _code(dtype) if dtype is not None else _dt(psf_fine)
+    g = grid._c()
+    L = _lens(code, sie, shear, tnfw)
+    S, keep = _sources(sources)
+    ky, kx = psf_fine.shape
+    nb = int(lib().jt_simulate_image_supersampled_psf_workspace_bytes(code, ctypes.byref(g), L.n_tnfw, ky, kx, _METHODS[method]))
+    ws, wsb = _workspace(nb, psf_fine.device, workspace, stream)
+    if out is None:
+        out = torch.empty((grid.ny, grid.nx), dtype=_torch_dtype(code), device=psf_fine.device)
+    _check(lib().jt_simulate_image_supersampled_psf(code, ctypes.byref(g), ctypes.byref(L), ctypes.byref(S), ky, kx, _ptr(psf_fine),
+                                                    _METHODS[method], _ptr(ws), wsb, _ptr(out), _stream(stream)),
+           "jt_simulate_image_supersampled_psf")
+    del keep
+    return out

@@ -343,4 +343,60 @@ jt_status jt_light_profiles(jt_dtype dtype, int64_t n, const void* beta_x, const
     return launch_light_profiles(dtype, n, beta_x, beta_y, n_comp, components, flux, (cudaStream_t)stream);
 }
 
+jt_status jt_light_core_sersic(jt_dtype dtype, int64_t n, const void* beta_x, const void* beta_y, const double* params, void* flux,
+                               void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (n < 0 || !params || !(params[1] > 0.0) || !(params[2] > 0.0) || !(params[3] > 0.0) || !(params[5] > 0.0))
+        return JT_ERR_INVALID_VALUE;
+    if (n == 0) return JT_OK;
+    if (!beta_x || !beta_y || !flux || flux == beta_x || flux == beta_y) return JT_ERR_INVALID_VALUE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_core_sersic(dtype, n, beta_x, beta_y, params, flux, (cudaStream_t)stream);
+}
+
+jt_status jt_light_shapelets(jt_dtype dtype, int64_t n, const void* beta_x, const void* beta_y, int32_t n_max, double beta, double cx,
+                             double cy, const void* coef, void* flux, void* stream) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (n < 0 || n_max < 0 || n_max > JT_MAX_SHAPELET_ORDER || !(beta > 0.0) || !coef) return JT_ERR_INVALID_VALUE;
+    if (n == 0) return JT_OK;
+    if (!beta_x || !beta_y || !flux || flux == beta_x || flux == beta_y) return JT_ERR_INVALID_VALUE;
+    jt_status s = check_device();
+    if (s != JT_OK) return s;
+    return launch_shapelets(dtype, n, beta_x, beta_y, n_max, beta, cx, cy, coef, flux, (cudaStream_t)stream);
+}
+
+// NEXT-4: the ray grid is a grid of its own with supersample 1: [jt_simulate_image workspace on it][fine output]
+static jt_grid fine_grid(const jt_grid* g) {
+    jt_grid f = *g;
+    f.nx = g->nx * g->supersample;
+    f.ny = g->ny * g->supersample;
+    f.pixel_scale = g->pixel_scale / (double)g->supersample;
+    f.supersample = 1;
+    return f;
+}
+
+size_t jt_simulate_image_supersampled_psf_workspace_bytes(jt_dtype dtype, const jt_grid* grid, int64_t n_tnfw, int32_t ky, int32_t kx,
+                                                          jt_conv_method method) {
+    if (!valid_dtype(dtype) || !valid_method(method) || !valid_grid(grid) || n_tnfw < 0 || !valid_kernel_size(ky, kx)) return 0;
+    const jt_grid f = fine_grid(grid);
+    const size_t inner = jt_simulate_image_workspace_bytes(dtype, &f, n_tnfw, ky, kx, method);
+    return align_up(inner, 256) + align_up((size_t)f.nx * f.ny * dtype_size(dtype), 256);
+}
+
+jt_status jt_simulate_image_supersampled_psf(jt_dtype dtype, const jt_grid* grid, const jt_lens* lens, const jt_sources* sources,
+                                             int32_t ky, int32_t kx, const void* kernel_fine, jt_conv_method method, void* workspace,
+                                             size_t workspace_bytes, void* out, void* stream) {
+    if (!valid_dtype(dtype) || !valid_method(method)) return JT_ERR_UNSUPPORTED;
+    if (!valid_grid(grid) || !valid_lens(lens) || !out || !kernel_fine || !valid_kernel_size(ky, kx)) return JT_ERR_INVALID_VALUE;
+    const size_t need = jt_simulate_image_supersampled_psf_workspace_bytes(dtype, grid, lens->n_tnfw, ky, kx, method);
+    if (!workspace || workspace_bytes < need) return JT_ERR_WORKSPACE;
+    const jt_grid f = fine_grid(grid);
+    const size_t inner = align_up(jt_simulate_image_workspace_bytes(dtype, &f, lens->n_tnfw, ky, kx, method), 256);
+    void* fine_out = (char*)workspace + inner;
+    jt_status s = jt_simulate_image(dtype, &f, lens, sources, ky, kx, kernel_fine, method, workspace, inner, fine_out, stream);
+    if (s != JT_OK) return s;
+    return launch_bin_sum(dtype, grid->ny, grid->nx, grid->supersample, fine_out, out, (cudaStream_t)stream);
+}
+
 }  // extern "C"

@@ -87,4 +87,10 @@ jt_status launch_ray_shoot_profiles(jt_dtype dtype, int64_t n, const void* tx, c
 jt_status launch_light_profiles(jt_dtype dtype, int64_t n, const void* bx, const void* by, int64_t n_comp,
                                 const jt_profile* comps, void* flux, cudaStream_t st);
 
+jt_status launch_core_sersic(jt_dtype dtype, int64_t n, const void* bx, const void* by, const double* params10, void* flux,
+                             cudaStream_t st);
+jt_status launch_shapelets(jt_dtype dtype, int64_t n, const void* bx, const void* by, int n_max, double beta, double cx, double cy,
+                           const void* coef, void* flux, cudaStream_t st);
+jt_status launch_bin_sum(jt_dtype dtype, int ny, int nx, int s, const void* fine, void* out, cudaStream_t st);
+
 }  // namespace jt

@@ -186,6 +186,43 @@ __device__ __forceinline__ void profile_alpha(const jt_profile& d, double x, dou
             ax += mx; ay += my;
             return;
         }
+        case JT_DEFL_NIE: {                                    // reading Q31: definition S with a core s_scale
+            double c, sn, q;
+            ellipticity(p[1], p[2], &c, &sn, &q);
+            const double dx = x - p[4], dy = y - p[5];
+            const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+            const double isq = fast_rsqrt(q), b = p[0] * isq, sk = p[3] * isq, f2 = 1.0 - q * q;
+            const double psi = sqrt(q * q * (sk * sk + xr * xr) + yr * yr);
+            if (psi + sk == 0.0) return;
+            const double ux = xr / (psi + sk), uy = yr / (psi + q * q * sk);
+            const double axr = b * q * ux * atan_over(f2 * ux * ux), ayr = b * q * uy * atanh_over(f2 * uy * uy);
+            ax += c * axr - sn * ayr;
+            ay += sn * axr + c * ayr;
+            return;
+        }
+        case JT_DEFL_EPL: {                                    // reading Q32: Tessore & Metcalf (2015) series
+            double c, sn, q;
+            ellipticity(p[2], p[3], &c, &sn, &q);
+            const double dx = x - p[4], dy = y - p[5];
+            const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+            const double t = p[1] - 1.0, b = p[0] * sqrt(q);
+            const double R2 = q * q * xr * xr + yr * yr;
+            if (R2 == 0.0) return;
+            const double R = sqrt(R2), cph = q * xr / R, sph = yr / R;
+            const double c2 = cph * cph - sph * sph, s2 = 2.0 * cph * sph, f = (1.0 - q) / (1.0 + q);
+            double are = cph, aim = sph, sre = cph, sim = sph;
+            for (int n = 1; n <= 400; ++n) {
+                const double g = -f * (2.0 * n - (2.0 - t)) / (2.0 * n + (2.0 - t));
+                const double nre = g * (c2 * are - s2 * aim), nim = g * (c2 * aim + s2 * are);
+                are = nre; aim = nim;
+                sre += are; sim += aim;
+                if (are * are + aim * aim < 1e-34 * (sre * sre + sim * sim)) break;
+            }
+            const double pre = 2.0 * b / (1.0 + q) * pow(b / R, t - 1.0);
+            ax += pre * (c * sre - sn * sim);
+            ay += pre * (sn * sre + c * sim);
+            return;
+        }
         case JT_DEFL_TNFW: {
             const TnfwRaw s = {p[3], p[4], p[0], p[1], p[2]};
             double f, kap;
@@ -301,6 +338,113 @@ jt_status launch_light_profiles(jt_dtype dtype, int64_t n, const void* bx, const
         k_light_profiles<float><<<(unsigned)blocks, kNextThreads, 0, st>>>(n, (const float*)bx, (const float*)by, n_comp, comps, (float*)flux);
     else
         k_light_profiles<double><<<(unsigned)blocks, kNextThreads, 0, st>>>(n, (const double*)bx, (const double*)by, n_comp, comps, (double*)flux);
+    JT_LAUNCH_CHECK();
+    return JT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- NEXT-1: CORE_SERSIC, SHAPELETS
+struct CoreSersic { double amp, iRs, n, Rb, gam, al, c, s, q, cx, cy, bn; };
+
+template <typename T>
+__global__ void __launch_bounds__(kNextThreads) k_core_sersic(int64_t n, const T* __restrict__ bx, const T* __restrict__ by,
+                                                              const __grid_constant__ CoreSersic P, T* __restrict__ flux) {
+    const int64_t i = (int64_t)blockIdx.x * kNextThreads + threadIdx.x;
+    if (i >= n) return;
+    const double dx = (double)bx[i] - P.cx, dy = (double)by[i] - P.cy;
+    const double xr = P.c * dx + P.s * dy, yr = -P.s * dx + P.c * dy;
+    const double R = sqrt(P.q * xr * xr + yr * yr / P.q);
+    const double core = R > 0.0 ? pow(1.0 + pow(P.Rb / R, P.al), P.gam / P.al) : (P.gam > 0.0 ? INFINITY : 1.0);
+    const double arg = pow((pow(R, P.al) + pow(P.Rb, P.al)) * pow(P.iRs, P.al), 1.0 / (P.al * P.n));
+    flux[i] = (T)(P.amp * core * exp(-P.bn * (arg - 1.0)));
+}
+
+jt_status launch_core_sersic(jt_dtype dtype, int64_t n, const void* bx, const void* by, const double* p, void* flux, cudaStream_t st) {
+    CoreSersic P;
+    P.amp = p[0]; P.iRs = 1.0 / p[1]; P.n = p[2]; P.Rb = p[3]; P.gam = p[4]; P.al = p[5];
+    ellipticity(p[6], p[7], &P.c, &P.s, &P.q);
+    P.cx = p[8]; P.cy = p[9];
+    P.bn = 1.9992 * p[2] - 0.3271;                             // reading Q10
+    const int64_t blocks = (n + kNextThreads - 1) / kNextThreads;
+    if (blocks > 0x7fffffffLL) return JT_ERR_UNSUPPORTED;
+    if (dtype == JT_F32) k_core_sersic<float><<<(unsigned)blocks, kNextThreads, 0, st>>>(n, (const float*)bx, (const float*)by, P, (float*)flux);
+    else k_core_sersic<double><<<(unsigned)blocks, kNextThreads, 0, st>>>(n, (const double*)bx, (const double*)by, P, (double*)flux);
+    JT_LAUNCH_CHECK();
+    return JT_OK;
+}
+
+// Shapelets (reading Q34): the coefficient triangle sits in shared memory, pre-multiplied by the recurrence's
+// normalisation; a thread runs the two 1-D recurrences in registers (n_max <= JT_MAX_SHAPELET_ORDER, unrolled) and
+// contracts them with the triangle: (n_max+1)(n_max+2)/2 multiply-adds per ray.  A dense contraction only in name --
+// one 66-vector per ray against basis values that exist nowhere but in that ray's registers -- so no tensor cores.
+template <typename T>
+__global__ void __launch_bounds__(kNextThreads) k_shapelets(int64_t n, const T* __restrict__ bx, const T* __restrict__ by, int n_max,
+                                                            double ibeta, double cx, double cy, const T* __restrict__ coef,
+                                                            T* __restrict__ flux) {
+    __shared__ double s_c[(JT_MAX_SHAPELET_ORDER + 1) * (JT_MAX_SHAPELET_ORDER + 2) / 2];
+    __shared__ double s_a[JT_MAX_SHAPELET_ORDER + 1], s_b[JT_MAX_SHAPELET_ORDER + 1];
+    const int nk = (n_max + 1) * (n_max + 2) / 2;
+    for (int k = threadIdx.x; k < nk; k += kNextThreads) s_c[k] = (double)coef[k];
+    for (int m = threadIdx.x; m <= n_max; m += kNextThreads) {
+        s_a[m] = m > 0 ? sqrt(2.0 / m) : 0.0;                  // B_m = a_m u B_(m-1) - b_m B_(m-2)
+        s_b[m] = m > 0 ? sqrt((m - 1.0) / m) : 0.0;
+    }
+    __syncthreads();
+    const int64_t i = (int64_t)blockIdx.x * kNextThreads + threadIdx.x;
+    if (i >= n) return;
+    const double u = ((double)bx[i] - cx) * ibeta, v = ((double)by[i] - cy) * ibeta;
+    double Bx[JT_MAX_SHAPELET_ORDER + 1], By[JT_MAX_SHAPELET_ORDER + 1];
+    const double g0 = 0.75112554446494248285870300477623;     // pi^(-1/4)
+    Bx[0] = g0 * exp(-0.5 * u * u);
+    By[0] = g0 * exp(-0.5 * v * v);
+#pragma unroll
+    for (int m = 1; m <= JT_MAX_SHAPELET_ORDER; ++m) {
+        Bx[m] = m <= n_max ? s_a[m] * u * Bx[m - 1] - (m > 1 ? s_b[m] * Bx[m - 2] : 0.0) : 0.0;
+        By[m] = m <= n_max ? s_a[m] * v * By[m - 1] - (m > 1 ? s_b[m] * By[m - 2] : 0.0) : 0.0;
+    }
+    double acc = 0.0;
+#pragma unroll
+    for (int N = 0; N <= JT_MAX_SHAPELET_ORDER; ++N) {
+        if (N <= n_max) {
+#pragma unroll
+            for (int n2 = 0; n2 <= N; ++n2) acc = fma(s_c[N * (N + 1) / 2 + n2], Bx[N - n2] * By[n2], acc);
+        }
+    }
+    flux[i] = (T)(acc * ibeta);
+}
+
+jt_status launch_shapelets(jt_dtype dtype, int64_t n, const void* bx, const void* by, int n_max, double beta, double cx, double cy,
+                           const void* coef, void* flux, cudaStream_t st) {
+    const int64_t blocks = (n + kNextThreads - 1) / kNextThreads;
+    if (blocks > 0x7fffffffLL) return JT_ERR_UNSUPPORTED;
+    if (dtype == JT_F32)
+        k_shapelets<float><<<(unsigned)blocks, kNextThreads, 0, st>>>(n, (const float*)bx, (const float*)by, n_max, 1.0 / beta, cx, cy,
+                                                                      (const float*)coef, (float*)flux);
+    else
+        k_shapelets<double><<<(unsigned)blocks, kNextThreads, 0, st>>>(n, (const double*)bx, (const double*)by, n_max, 1.0 / beta, cx, cy,
+                                                                       (const double*)coef, (double*)flux);
+    JT_LAUNCH_CHECK();
+    return JT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------- NEXT-4: s x s binning
+// out[j][i] = sum of the s x s block of the ray-resolution image (summed in double, fixed order)
+template <typename T>
+__global__ void __launch_bounds__(kNextThreads) k_bin_sum(int ny, int nx, int s, const T* __restrict__ fine, T* __restrict__ out) {
+    const int64_t p = (int64_t)blockIdx.x * kNextThreads + threadIdx.x;
+    if (p >= (int64_t)ny * nx) return;
+    const int j = (int)(p / nx), i = (int)(p - (int64_t)j * nx);
+    const int64_t NX = (int64_t)nx * s;
+    double acc = 0.0;
+    for (int a = 0; a < s; ++a)
+        for (int b = 0; b < s; ++b) acc += (double)fine[((int64_t)j * s + a) * NX + ((int64_t)i * s + b)];
+    out[p] = (T)acc;
+}
+
+jt_status launch_bin_sum(jt_dtype dtype, int ny, int nx, int s, const void* fine, void* out, cudaStream_t st) {
+    const int64_t blocks = ((int64_t)ny * nx + kNextThreads - 1) / kNextThreads;
+    if (blocks > 0x7fffffffLL) return JT_ERR_UNSUPPORTED;
+    if (dtype == JT_F32) k_bin_sum<float><<<(unsigned)blocks, kNextThreads, 0, st>>>(ny, nx, s, (const float*)fine, (float*)out);
+    else k_bin_sum<double><<<(unsigned)blocks, kNextThreads, 0, st>>>(ny, nx, s, (const double*)fine, (double*)out);
     JT_LAUNCH_CHECK();
     return JT_OK;
 }

@@ -158,3 +158,69 @@ def test_light_profiles(jt, orc, dtype):
     a = jt.source_brightness(to_dev(bx, "f64"), to_dev(by, "f64"), [ser[0][1]])
     b = jt.light_profiles(to_dev(bx, "f64"), to_dev(by, "f64"), ser)
     assert float((a - b).abs().max()) < 1e-12 * float(a.abs().max())
+
+
+# ------------------------------------------------------------------ NEXT-1, second set
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_ray_shoot_profiles_nie_epl(jt, orc, dtype):
+    """NIE (readings Q31) and EPL (Q32: the Tessore-Metcalf series, summed to the same tolerance on both sides) in a
+    typed list with members of the first set; includes s_scale = 0, gamma = 2, round lenses and a ray on a centre."""
+    rng = np.random.default_rng(91)
+    n = 3000
+    tx, ty = rng.uniform(-2, 2, n), rng.uniform(-2, 2, n)
+    tx[0], ty[0] = 0.3, -0.1                                   # on the centre of the first NIE
+    defl = [("NIE", [1.1, 0.2, -0.1, 0.15, 0.3, -0.1]), ("NIE", [0.4, 0.0, 0.0, 0.05, -0.8, 0.6]),
+            ("NIE", [0.7, -0.3, 0.25, 0.0, 1.2, 1.1]), ("EPL", [1.0, 2.0, 0.15, 0.1, -0.2, 0.3]),
+            ("EPL", [0.8, 1.45, -0.35, 0.3, 0.9, -0.7]), ("EPL", [0.5, 2.7, 0.5, -0.2, -1.1, -1.2]),
+            ("EPL", [0.6, 2.3, 0.0, 0.0, 0.1, 1.4]), ("SHEAR", [0.03, -0.02]), ("SIS", [0.2, 1.5, -1.5])]
+    if dtype == "f32":
+        tx, ty = _f32r(tx), _f32r(ty)
+    bx, by = jt.ray_shoot_profiles(to_dev(tx, dtype), to_dev(ty, dtype), defl)
+    wx, wy = orc.ray_shoot_profiles(tx, ty, defl)
+    tol = 2e-12 if dtype == "f64" else 6e-7
+    assert np.max(np.abs(bx.double().cpu().numpy() - wx)) < tol
+    assert np.max(np.abs(by.double().cpu().numpy() - wy)) < tol
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_light_core_sersic_and_shapelets(jt, orc, dtype):
+    """CORE_SERSIC (Q33) and SHAPELETS (Q34) at n_max = 0, 6, 10 (the paper's two orders, 28 and 66 coefficients) and 12."""
+    rng = np.random.default_rng(92)
+    n = 5000
+    bx, by = rng.uniform(-1.5, 1.5, n), rng.uniform(-1.5, 1.5, n)
+    if dtype == "f32":
+        bx, by = _f32r(bx), _f32r(by)
+    p = [3.0, 0.4, 2.5, 0.05, 0.3, 2.0, 0.1, -0.2, 0.05, 0.02]
+    got = jt.light_core_sersic(to_dev(bx, dtype), to_dev(by, dtype), p).double().cpu().numpy()
+    want = orc.core_sersic(bx, by, *p)
+    assert np.max(np.abs(got / want - 1.0)) < (1e-12 if dtype == "f64" else 2e-6)
+    for n_max in (0, 6, 10, 12):
+        coef = rng.normal(size=orc.shapelet_count(n_max))
+        if dtype == "f32":
+            coef = _f32r(coef)
+        got = jt.light_shapelets(to_dev(bx, dtype), to_dev(by, dtype), n_max, 0.37, 0.1, -0.2, to_dev(coef, dtype)).double().cpu().numpy()
+        want = orc.shapelets(bx, by, n_max, 0.37, 0.1, -0.2, coef)
+        assert np.max(np.abs(got - want)) < (1e-12 if dtype == "f64" else 2e-6) * np.max(np.abs(want)), n_max
+
+
+# ------------------------------------------------------------------ NEXT-4
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("s,method", [(1, "direct"), (2, "direct"), (3, "fft"), (4, "auto")])
+def test_simulate_image_supersampled_psf(jt, orc, dtype, s, method):
+    """Convolution at ray resolution, then s x s binning = the oracle's composition (its ray image is the s = 1 pre-PSF
+    image on the ray grid; PSF sampled on that grid, asymmetric on purpose)."""
+    nx = 36
+    w = workloads.config_c2(nx=nx, supersample=s, n_tnfw=300, K=9, dtype=dtype)
+    rng = np.random.default_rng(93 + s)
+    kf = rng.uniform(0, 1, (4 * s + 1, 2 * s + 3))
+    kf /= kf.sum()
+    if dtype == "f32":
+        kf = _f32r(kf)
+    fine = workloads.config_c2(nx=nx, supersample=s, n_tnfw=300, K=9, dtype=dtype)
+    fine.nx, fine.ny, fine.pixel_scale, fine.supersample = nx * s, nx * s, w.pixel_scale / s, 1
+    rays, _ = orc.simulate_image(fine)
+    want = orc.convolve_supersampled(rays, s, kf)
+    g = jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample)
+    got = jt.simulate_image_supersampled_psf(g, w.sie, w.shear, to_dev(w.tnfw, dtype), w.sources, to_dev(kf, dtype), dtype=dtype,
+                                             method=method).double().cpu().numpy()
+    assert rel_err(got, want) < (1e-10 if dtype == "f64" else 2e-4)
