@@ -59,7 +59,7 @@ static void plan_chunks(TracePlan* p, int64_t M, int R, bool f64) {
     p->n_chunks = M > 0 ? (int)((M + p->chunk_len - 1) / p->chunk_len) : 1;
     if (p->n_chunks < 1) p->n_chunks = 1;
     p->partial_bytes = p->n_chunks > 1 ? (size_t)p->n_chunks * p->n_tiles * R * p->threads * sizeof(double2) : 0;
-    p->counter_bytes = p->n_chunks > 1 ? align_up((size_t)p->n_tiles * sizeof(unsigned int), 256) : 0;
+    p->counter_bytes = p->n_chunks > 1 ? align_up((size_t)p->n_tiles * (p->threads / 32) * sizeof(unsigned int), 256) : 0;   // one per warp tile
     p->rec_bytes = align_up((size_t)M * (f64 ? sizeof(SubRec<double>) : sizeof(SubRec<float>)), 256);
     p->total_bytes = p->partial_bytes + p->counter_bytes + p->tier_bytes + p->rec_bytes;
 }
@@ -125,10 +125,10 @@ static jt_status fill_lens(TraceArgs<T>& a, const jt_lens* lens, const TracePlan
     a.tier_counts = count_tiers ? (unsigned long long*)trace_tier_counters(plan, workspace) : nullptr;
     a.recs = (const SubRec<T>*)((char*)workspace + plan.partial_bytes + plan.counter_bytes + plan.tier_bytes);
     if (a.M > 0) {
-        const int n_counter = plan.n_chunks > 1 ? (int)plan.n_tiles : 0;
+        const int64_t n_counter = plan.n_chunks > 1 ? plan.n_tiles * (plan.threads / 32) : 0;
         const int64_t n = a.M > n_counter ? a.M : n_counter;
         const RawTn<T> raw = {{a.tn[0], a.tn[1], a.tn[2], a.tn[3], a.tn[4]}};
-        k_make_recs<T><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a.M, raw, const_cast<SubRec<T>*>(a.recs), a.counter, n_counter,
+        k_make_recs<T><<<(unsigned)((n + 127) / 128), 128, 0, st>>>(a.M, raw, const_cast<SubRec<T>*>(a.recs), a.counter, (int)n_counter,
                                                                    a.tier_counts);
         JT_LAUNCH_CHECK();
     } else if (count_tiers) {

@@ -25,8 +25,8 @@
 // bounding box) votes per record on the rays themselves.  float runs the far-far and far forms on two rays at once
 // with packed f32x2 instructions (FFMA2 / FMUL2 / FADD2).
 // When there are too few ray tiles to fill the SMs the subhalo list is split into chunks (wave-aware choice in
-// jt_trace.cu); every (tile, chunk) CTA writes double partial sums to the workspace and the last CTA to arrive for
-// a tile adds them in chunk order (deterministic) and runs the epilogue.
+// jt_trace.cu); every (tile, chunk) CTA writes double partial sums to the workspace and, warp by warp, the last to
+// arrive for a warp tile adds them in chunk order (deterministic) and runs that warp tile's epilogue.
 #pragma once
 #include "jt_internal.h"
 
@@ -563,7 +563,6 @@ template <> struct TraceCfg<float> { static constexpr int NT = 256, OCC = 2, VAR
 template <typename T, int R, bool GRID>
 __global__ void __launch_bounds__(TraceCfg<T>::NT, TraceCfg<T>::OCC) k_trace(const __grid_constant__ TraceArgs<T> a) {
     constexpr int NT = TraceCfg<T>::NT, NW = NT / 32;
-    __shared__ int s_last;
     extern __shared__ __align__(32) unsigned char dacc_raw[];
     SubRec<T>* ring = reinterpret_cast<SubRec<T>*>(dacc_raw + dacc_smem_bytes<T, R, NT>());
     unsigned short* lists = reinterpret_cast<unsigned short*>(ring + (size_t)kStages * a.tile_recs);
@@ -665,20 +664,20 @@ __global__ void __launch_bounds__(TraceCfg<T>::NT, TraceCfg<T>::OCC) k_trace(con
         for (int k = 0; k < kTiers; ++k) atomicAdd(&a.tier_counts[k], (unsigned long long)tiers.n[k]);
     }
 
-    // ---- split subhalo list: publish partial sums; the last CTA of the tile reduces them in chunk order ----
+    // ---- split subhalo list: publish partial sums; the last WARP to arrive for a warp tile (over the chunks) adds them
+    // in chunk order and runs that warp tile's epilogue.  Per warp, not per CTA: a CTA-wide barrier here kept the warps
+    // that had finished waiting for the one with subhalo cores in its rays (ncu: 9-12 % of all warp samples).
     if (a.n_chunks > 1) {
         const int64_t slot0 = ((int64_t)chunk * a.n_tiles + tile) * R;
 #pragma unroll
         for (int r = 0; r < R; ++r)
             __stcg(&a.partial[(slot0 + r) * NT + tid], make_double2(axd[r], ayd[r]));
         __threadfence();
-        __syncthreads();
-        if (tid == 0) {
-            const unsigned int old = atomicAdd(&a.counter[tile], 1u);
-            s_last = (old == (unsigned int)(a.n_chunks - 1));
-        }
-        __syncthreads();
-        if (!s_last) return;
+        __syncwarp();
+        unsigned int old = 0u;
+        if (lane == 0) old = atomicAdd(&a.counter[tile * NW + warp], 1u);
+        old = __shfl_sync(0xffffffffu, old, 0);
+        if (old != (unsigned int)(a.n_chunks - 1)) return;
         __threadfence();
 #pragma unroll
         for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
