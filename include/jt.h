@@ -32,7 +32,8 @@
  *
  * Error codes: JT_ERR_INVALID_VALUE  null pointer where data is required, negative count,
  *              nx/ny < 1, supersample < 1 or > JT_MAX_SUPERSAMPLE, pixel_scale <= 0,
- *              even or < 1 kernel size, n_src < 0 or > JT_MAX_SOURCES, in == out;
+ *              even or < 1 kernel size, n_src < 0 or > JT_MAX_SOURCES, in == out, a workspace that is not
+ *              16-byte aligned;
  *              JT_ERR_UNSUPPORTED    unknown dtype / method, device is not compute capability 10.x;
  *              JT_ERR_WORKSPACE      workspace_bytes smaller than the matching *_workspace_bytes query
  *                                    (or workspace NULL when the query is non-zero);

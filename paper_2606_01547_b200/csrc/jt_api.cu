@@ -99,6 +99,7 @@ jt_status jt_ray_shoot(jt_dtype dtype, int64_t n_rays, const void* theta_x, cons
     if (theta_x == beta_x || theta_y == beta_y || theta_x == beta_y || theta_y == beta_x) return JT_ERR_INVALID_VALUE;
     const TracePlan plan = plan_trace_rays(dtype, n_rays, lens->n_tnfw);
     if (plan.total_bytes > 0 && (!workspace || workspace_bytes < plan.total_bytes)) return JT_ERR_WORKSPACE;
+    if ((uintptr_t)workspace & 15) return JT_ERR_INVALID_VALUE;              // the records are fetched by 16-byte bulk copies
     jt_status s = check_device();
     if (s != JT_OK) return s;
     return launch_trace_rays(dtype, n_rays, theta_x, theta_y, lens, plan, workspace, beta_x, beta_y, (cudaStream_t)stream);
@@ -192,6 +193,7 @@ jt_status jt_simulate_image(jt_dtype dtype, const jt_grid* grid, const jt_lens* 
         return JT_ERR_UNSUPPORTED;
     const size_t need = jt_simulate_image_workspace_bytes(dtype, grid, lens->n_tnfw, conv ? ky : 0, conv ? kx : 0, method);
     if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
+    if ((uintptr_t)workspace & 15) return JT_ERR_INVALID_VALUE;              // the records are fetched by 16-byte bulk copies
     s = check_device();
     if (s != JT_OK) return s;
     const TracePlan plan = plan_trace_grid(dtype, grid, lens->n_tnfw);

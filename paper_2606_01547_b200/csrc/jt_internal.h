@@ -40,6 +40,9 @@ struct TracePlan {
     int cols_per_warp;     // active lanes per warp (grid mode: floor(32/s)*s; ray mode: 32)
     int tiles_x, tiles_y;  // grid mode: warp tiles (cols_per_warp x R rays) per axis
     int64_t n_wt;          // grid mode: warp tiles in all
+    bool wide;             // grid mode, single-image kernel: CTA-wide tiles (s does not divide 32)
+    int cols_per_cta, ctiles_x;
+    int64_t n_tiles_wide;
     int64_t n_tiles;       // CTAs per subhalo chunk (threads/32 warp tiles, or threads * R rays in ray mode)
     int n_chunks;          // subhalo list split (1 = no workspace traffic)
     int64_t chunk_len;     // subhalos per chunk

@@ -77,7 +77,14 @@ static TracePlan plan_trace_grid_t(const jt_grid* g, int64_t n_tnfw, bool f64) {
     p.n_wt = (int64_t)p.tiles_x * p.tiles_y;
     p.threads = trace_threads(f64);
     p.n_tiles = (p.n_wt + p.threads / 32 - 1) / (p.threads / 32);
+    // s does not divide 32 (3, 5, 6, 7, 9 ...): 2-4 lanes of every warp tile would idle (s = 5: 30 of 32).  The
+    // single-image kernel then gives a CTA floor(threads/s)*s adjacent columns and bins through shared memory.
+    p.wide = (32 % s) != 0;
+    p.cols_per_cta = (p.threads / s) * s;
+    p.ctiles_x = (NX + p.cols_per_cta - 1) / p.cols_per_cta;
+    p.n_tiles_wide = (int64_t)p.ctiles_x * p.tiles_y;
     p.tier_bytes = 256;
+    if (p.wide) p.n_tiles = p.n_tiles_wide;          // the batch kernel keeps warp tiles (n_wt, tiles_x, cols_per_warp)
     plan_chunks(&p, n_tnfw, p.R, f64);
     return p;
 }
@@ -150,6 +157,9 @@ static jt_status trace_grid_t(const jt_grid* g, const jt_lens* lens, const SrcSe
     a.cols_per_warp = plan.cols_per_warp;
     a.wtiles_x = plan.tiles_x;
     a.n_wt = plan.n_wt;
+    a.wide = plan.wide ? 1 : 0;
+    a.cols_per_cta = plan.cols_per_cta;
+    a.ctiles_x = plan.ctiles_x;
     const jt_status fs = fill_lens(a, lens, plan, workspace, count_tiers, st);
     if (fs != JT_OK) return fs;
     a.out = (T*)pre_psf;

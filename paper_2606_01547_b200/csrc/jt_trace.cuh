@@ -41,6 +41,7 @@ struct TraceArgs {
     double hh, cx, cy, area_over_s2;      // half ray spacing, grid centre
     int cols_per_warp, wtiles_x;
     int64_t n_wt;                         // warp tiles of the grid, dealt to CTAs NT/32 at a time
+    int wide, cols_per_cta, ctiles_x;     // s does not divide 32: a CTA owns floor(NT/s)*s adjacent columns x R rows and bins through shared memory
     // ray mode
     int64_t n_rays;
     const T *tx, *ty;
@@ -550,6 +551,28 @@ __device__ __forceinline__ void grid_epilogue(const MacroLens& m, const SrcSet& 
     }
 }
 
+// The same O(rays) work for the CTA-wide tiles: the surface brightness of this thread's R rays -> dst[r * pitch]
+// (0 for rays outside the grid and for the spare threads of the tile).
+template <typename T, int R>
+__device__ __forceinline__ void grid_brightness(const MacroLens& m, const SrcSet& src, const RayGeom& g, bool active,
+                                                const double (&axd)[R], const double (&ayd)[R], double* dst, int pitch) {
+    double sx[R], sy[R];                        // dynamically indexed below -> local memory, once per ray
+#pragma unroll
+    for (int r = 0; r < R; ++r) { sx[r] = axd[r]; sy[r] = ayd[r]; }
+    const double xd = g.xd();
+#pragma unroll 1
+    for (int r = 0; r < R; ++r) {
+        double v = 0.0;
+        if (active && g.I < g.NX && g.J0 + r < g.NY) {
+            const double yd = g.yd(r);
+            double mx, my;
+            macro_alpha(m, xd, yd, mx, my);
+            v = sersic_sum<T>(src, xd - mx - sx[r], yd - my - sy[r]);
+        }
+        dst[r * pitch] = v;
+    }
+}
+
 // shared-memory footprint of k_trace: [float mode: DAcc columns][kStages record tiles][NT/32 x 2 index lists][barriers]
 template <typename T, int R, int NT>
 __host__ __device__ constexpr size_t trace_smem_bytes(int tile_recs) {
@@ -588,7 +611,11 @@ __global__ void __launch_bounds__(TraceCfg<T>::NT, TraceCfg<T>::OCC) k_trace(con
     T xs[R], ys[R];
     if constexpr (GRID) {
         const int64_t wt = tile * NW + warp;
-        if (wt < a.n_wt) {
+        if (a.wide) {                              // CTA tile: cols_per_cta columns x R rows; the spare threads shadow
+            // the tile's last column (their rays must not widen the warp's bounding box) and store nothing
+            g.I = (int)(tile % a.ctiles_x) * a.cols_per_cta + min(tid, a.cols_per_cta - 1);
+            g.J0 = (int)(tile / a.ctiles_x) * R;
+        } else if (wt < a.n_wt) {
             g.I = (int)(wt % a.wtiles_x) * a.cols_per_warp + lane;
             g.J0 = (int)(wt / a.wtiles_x) * R;
         } else {                                   // idle warp of the last CTA: clamped coordinates, no stores
@@ -673,11 +700,19 @@ __global__ void __launch_bounds__(TraceCfg<T>::NT, TraceCfg<T>::OCC) k_trace(con
         for (int r = 0; r < R; ++r)
             __stcg(&a.partial[(slot0 + r) * NT + tid], make_double2(axd[r], ayd[r]));
         __threadfence();
-        __syncwarp();
-        unsigned int old = 0u;
-        if (lane == 0) old = atomicAdd(&a.counter[tile * NW + warp], 1u);
-        old = __shfl_sync(0xffffffffu, old, 0);
-        if (old != (unsigned int)(a.n_chunks - 1)) return;
+        if (GRID && a.wide) {                      // the CTA bins together: CTA-wide completion
+            __shared__ int s_last;
+            __syncthreads();
+            if (tid == 0) s_last = atomicAdd(&a.counter[tile], 1u) == (unsigned int)(a.n_chunks - 1);
+            __syncthreads();
+            if (!s_last) return;
+        } else {
+            __syncwarp();
+            unsigned int old = 0u;
+            if (lane == 0) old = atomicAdd(&a.counter[tile * NW + warp], 1u);
+            old = __shfl_sync(0xffffffffu, old, 0);
+            if (old != (unsigned int)(a.n_chunks - 1)) return;
+        }
         __threadfence();
 #pragma unroll
         for (int r = 0; r < R; ++r) { axd[r] = 0.0; ayd[r] = 0.0; }
@@ -695,8 +730,26 @@ __global__ void __launch_bounds__(TraceCfg<T>::NT, TraceCfg<T>::OCC) k_trace(con
     if constexpr (GRID) {
         T* out = a.out;
         const int nx = a.nx;
-        grid_epilogue<T, R>(a.m, a.src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
-                            [out, nx](int j, int i, double v) { out[(int64_t)j * nx + i] = (T)v; });
+        if (a.wide) {
+            // ray brightness -> shared memory (the accumulator columns in float mode, the record ring in double: both
+            // are free once every warp has left the loop), then one thread per pixel sums its s x s rays in fixed order
+            __syncthreads();
+            double* sB = sizeof(T) == 4 ? reinterpret_cast<double*>(dacc_raw) : reinterpret_cast<double*>(ring);
+            grid_brightness<T, R>(a.m, a.src, g, tid < a.cols_per_cta, axd, ayd, sB + tid, NT);
+            __syncthreads();
+            const int s = a.s, n_px = a.cols_per_cta / s, n_py = R / s;
+            const int i0 = (int)(tile % a.ctiles_x) * n_px, j0 = (int)(tile / a.ctiles_x) * n_py;
+            for (int p = tid; p < n_px * n_py; p += NT) {
+                const int py = p / n_px, px = p - py * n_px;
+                double tot = 0.0;
+                for (int u = 0; u < s; ++u)
+                    for (int v = 0; v < s; ++v) tot += sB[(py * s + u) * NT + px * s + v];
+                if (i0 + px < a.nx && j0 + py < a.ny) out[(int64_t)(j0 + py) * nx + i0 + px] = (T)(tot * a.area_over_s2);
+            }
+        } else {
+            grid_epilogue<T, R>(a.m, a.src, g, a.s, a.cols_per_warp, a.area_over_s2, lane, axd, ayd,
+                                [out, nx](int j, int i, double v) { out[(int64_t)j * nx + i] = (T)v; });
+        }
     } else {
         double sx[R], sy[R];
 #pragma unroll
