@@ -211,7 +211,7 @@ template <typename T>
 static jt_status batch_t(jt_dtype dtype, int64_t B, const jt_grid* g, const jt_batch_params* p, void* out,
                          const void* data, const void* sigma, double* chi2, cudaStream_t st) {
     if (B > 0x7fffffffLL) return JT_ERR_UNSUPPORTED;
-    const TracePlan plan = plan_trace_grid(dtype, g, 0);
+    const TracePlan plan = plan_trace_grid(dtype, g, 1 << 20);      // warp-tile geometry with the register-blocked ray count
     BatchArgs<T> a = {};
     const int s = g->supersample;
     a.nx = g->nx; a.ny = g->ny; a.s = s; a.NX = g->nx * s; a.NY = g->ny * s;

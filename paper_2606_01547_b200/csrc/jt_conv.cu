@@ -28,7 +28,7 @@
 #include <stdlib.h>
 #include <stdio.h>
 #include <math.h>
-#include "jt_internal.h"
+#include "jt_conv.cuh"
 
 namespace jt {
 
@@ -403,12 +403,102 @@ static ConvPlan plan_conv(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx)
     return best;
 }
 
+// ------------------------------------------------------------------------------------------------ small problems
+// Launch-latency-bound shapes (C0: 60 x 60 (x) 11 x 11 is 0.4 M FMAs; the paper's 60 x 60 sweep): ONE launch instead of
+// tap kernel + constant-bank copy + sweep kernel.  A CTA of 64 threads owns a 64 x 8 output tile, stages the packed
+// taps (jt_conv.cuh) and its halo tile in shared memory itself and runs the register-window sweep of the batch kernel.
+// The taps do not depend on the image, so they are staged BEFORE the grid dependency is awaited: launched as a
+// programmatic dependent of the ray-tracing kernel, this part overlaps its tail.
+constexpr int kSmallOY = 4, kSmallNW = 2, kSmallTH = kSmallOY * kSmallNW;
+constexpr size_t kSmallMaxSmem = 96 * 1024;
+constexpr double kSmallMaxFma = 2.0e7;
+
+template <typename T>
+__global__ void __launch_bounds__(kSmallNW * 32) k_conv_small(int ny, int nx, int ky, int kx, int kyp, int tws, int ths,
+                                                              const T* __restrict__ img, const T* __restrict__ ker,
+                                                              T* __restrict__ out) {
+    extern __shared__ __align__(128) unsigned char smem_small[];   // (its own name: `smem_raw` is the TMA kernel's, 128-byte aligned)
+    const int npairs = (kx + 1) / 2, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    T* Kq = reinterpret_cast<T*>(smem_small);
+    T* tile = Kq + (size_t)npairs * kyp * 4;
+    stage_taps<T>(Kq, ker, ky, kx, kyp, 0, npairs, tid, kSmallNW * 32);
+    cudaGridDependencySynchronize();                           // the image of the previous kernel is complete
+    const int i0 = blockIdx.x * kConvTW, j0 = blockIdx.y * kSmallTH, hy = ky / 2, hx = kx / 2;
+    for (int idx = tid; idx < ths * tws; idx += kSmallNW * 32) {
+        const int r = idx / tws, c = idx - r * tws;
+        const int gj = j0 - hy + r, gi = i0 - hx + c;
+        tile[idx] = (gj >= 0 && gj < ny && gi >= 0 && gi < nx) ? __ldg(&img[(size_t)gj * nx + gi]) : (T)0;
+    }
+    __syncthreads();
+    ConvAcc<T, kSmallOY> acc;
+    acc.zero();
+    acc.template sweep<false>(tile + (size_t)(warp * kSmallOY) * tws + 2 * lane, tws, Kq, kyp, npairs);
+    const int i = i0 + 2 * lane;
+#pragma unroll
+    for (int r = 0; r < kSmallOY; ++r) {
+        const int j = j0 + warp * kSmallOY + r;
+        if (j < ny) {
+            if (i < nx) out[(size_t)j * nx + i] = acc.col0(r);
+            if (i + 1 < nx) out[(size_t)j * nx + i + 1] = acc.col1(r);
+        }
+    }
+}
+
+struct SmallPlan { int kyp, tws, ths; size_t smem; double est_us; bool ok; };
+static SmallPlan plan_small(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx) {
+    SmallPlan p = {};
+    const size_t sz = dtype_size(d);
+    p.kyp = (ky + kSmallOY - 1) / kSmallOY * kSmallOY;
+    p.tws = kConvTW + kx - 1;                                  // even (kx odd): pair loads stay aligned
+    p.ths = kSmallTH + p.kyp - 1;
+    p.smem = ((size_t)((kx + 1) / 2) * p.kyp * 4 + (size_t)p.tws * p.ths) * sz;
+    p.ok = B == 1 && (double)ny * nx * ky * kx <= kSmallMaxFma && p.smem <= kSmallMaxSmem;
+    // measured on B200 (conv sweep, 60^2 ... 200^2): 3 us + a CTA's FMAs at 12.8 (double) / 24 (float) per clock, per wave
+    const double ctas = (double)((nx + kConvTW - 1) / kConvTW) * ((ny + kSmallTH - 1) / kSmallTH);
+    const double per_cta = (double)kConvTW * kSmallTH * ((kx + 1) / 2 * 2) * p.kyp;
+    p.est_us = 3.0 + ceil(ctas / (kNumSMs * 2.0)) * per_cta * (d == JT_F64 ? 4.1e-5 : 2.2e-5);
+    return p;
+}
+// the one-launch kernel when it is expected to beat the constant-bank kernel (tiny kernels on small images)
+static bool use_small(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx, SmallPlan* sp);
+
+template <typename T>
+static jt_status conv_small_t(const SmallPlan& p, int ny, int nx, const T* img, int ky, int kx, const T* ker, T* out, cudaStream_t st) {
+    auto kern = k_conv_small<T>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmallMaxSmem));
+        attr_set = true;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((nx + kConvTW - 1) / kConvTW), (unsigned)((ny + kSmallTH - 1) / kSmallTH));
+    cfg.blockDim = dim3(kSmallNW * 32);
+    cfg.dynamicSmemBytes = p.smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    JT_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, ny, nx, ky, kx, p.kyp, p.tws, p.ths, img, ker, out));
+    JT_LAUNCH_CHECK();
+    return JT_OK;
+}
+
 bool conv_direct_supported(jt_dtype d, int ny, int nx, int ky, int kx) { return plan_conv(d, 1, ny, nx, ky, kx).ok; }
 size_t conv_direct_workspace_bytes(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx) {
     const ConvPlan p = plan_conv(d, B, ny, nx, ky, kx);
     return p.ok ? p.table_bytes + p.counter_bytes + p.partial_bytes : 0;
 }
+static bool use_small(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx, SmallPlan* sp) {
+    *sp = plan_small(d, B, ny, nx, ky, kx);
+    if (!sp->ok) return false;
+    const ConvPlan p = plan_conv(d, B, ny, nx, ky, kx);
+    return !p.ok || sp->est_us < p.est_us;
+}
 double conv_direct_estimate_us(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx) {
+    SmallPlan sp;
+    if (use_small(d, B, ny, nx, ky, kx, &sp)) return sp.est_us;
     const ConvPlan p = plan_conv(d, B, ny, nx, ky, kx);
     return p.ok ? p.est_us : 1e30;
 }
@@ -528,6 +618,10 @@ static jt_status conv_direct_t(jt_dtype d, int64_t B, int ny, int nx, const T* i
 
 jt_status launch_conv_direct(jt_dtype dtype, int64_t B, int ny, int nx, const void* img, int ky, int kx, const void* ker,
                              void* workspace, void* out, cudaStream_t st) {
+    SmallPlan sp;
+    if (use_small(dtype, B, ny, nx, ky, kx, &sp))
+        return dtype == JT_F32 ? conv_small_t<float>(sp, ny, nx, (const float*)img, ky, kx, (const float*)ker, (float*)out, st)
+                               : conv_small_t<double>(sp, ny, nx, (const double*)img, ky, kx, (const double*)ker, (double*)out, st);
     return dtype == JT_F32 ? conv_direct_t<float>(dtype, B, ny, nx, (const float*)img, ky, kx, (const float*)ker, workspace, (float*)out, st)
                            : conv_direct_t<double>(dtype, B, ny, nx, (const double*)img, ky, kx, (const double*)ker, workspace, (double*)out, st);
 }

@@ -26,7 +26,10 @@ jt_status make_sources(const jt_sources* src, SrcSet* out) {
 }
 
 // ---- plans ----
-static int rays_per_thread(int s, bool f64) {
+static int rays_per_thread(int s, bool f64, int64_t M) {
+    // next to no subhalos: nothing to amortise over a thread's rays, and the O(rays) epilogue runs ray after ray -- one
+    // pixel row per thread puts the most warps on it (C0: 29 CTAs instead of 4, C1: 235 instead of 118)
+    if (M <= 16 && s <= 4) return s;
     if (f64) {
         switch (s) { case 1: case 2: case 4: case 8: return 8; case 3: return 6; case 5: return 10; default: return s; }
     }
@@ -69,7 +72,7 @@ static void plan_chunks(TracePlan* p, int64_t M, int R, bool f64) {
 static TracePlan plan_trace_grid_t(const jt_grid* g, int64_t n_tnfw, bool f64) {
     TracePlan p = {};
     const int s = g->supersample;
-    p.R = rays_per_thread(s, f64);
+    p.R = rays_per_thread(s, f64, n_tnfw);
     p.cols_per_warp = (32 / s) * s;
     const int NX = g->nx * s, NY = g->ny * s;
     p.tiles_x = (NX + p.cols_per_warp - 1) / p.cols_per_warp;       // warp tiles per row of warp tiles

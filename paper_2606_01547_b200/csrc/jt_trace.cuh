@@ -599,6 +599,7 @@ __global__ void __launch_bounds__(TraceCfg<T>::NT, TraceCfg<T>::OCC) k_trace(con
     const int64_t j_end = min(a.M, j_begin + a.chunk_len);
     const int n_rounds = j_end > j_begin ? (int)((j_end - j_begin + a.tile_recs - 1) / a.tile_recs) : 0;
 
+    cudaTriggerProgrammaticLaunchCompletion();     // a dependent launch (the small convolution) may stage its taps now
     if (tid == 0) {
 #pragma unroll
         for (int s = 0; s < kStages; ++s) { mbar_init(&full[s], 1); done[s] = 0u; }
@@ -802,6 +803,7 @@ jt_status launch_trace_impl(const TraceArgs<T>& a, int R, cudaStream_t st) {
     cfg.numAttrs = a.M > 0 ? 1 : 0;
     if constexpr (GRID) {
         switch (R) {
+            JT_TRACE_CASE(1) JT_TRACE_CASE(2) JT_TRACE_CASE(3) JT_TRACE_CASE(4)
             JT_TRACE_CASE(5) JT_TRACE_CASE(6) JT_TRACE_CASE(7) JT_TRACE_CASE(8) JT_TRACE_CASE(9) JT_TRACE_CASE(10) JT_TRACE_CASE(11)
             JT_TRACE_CASE(12) JT_TRACE_CASE(13) JT_TRACE_CASE(14) JT_TRACE_CASE(15) JT_TRACE_CASE(16)
             default: return JT_ERR_UNSUPPORTED;
