@@ -97,6 +97,8 @@ def lib():
         L.orc_profile_kappa2.argtypes = [_i, _dp, _d, _d]
         L.orc_profile_kappa2.restype = _d
         L.orc_ray_shoot_profiles2.argtypes = [_i64, _dp, _dp, _i64, _i32p, _dp, _dp, _dp]
+        L.orc_multipole_potential.argtypes = [_d, _d, _dp]
+        L.orc_multipole_potential.restype = _d
         L.orc_core_sersic_n.argtypes = [_i64, _dp, _dp, _dp, _d, _d, _dp]
         L.orc_shapelets_n.argtypes = [_i64, _dp, _dp, _i, _d, _d, _d, _dp, _dp]
         L.orc_convolve_supersampled.argtypes = [_i, _i, _i, _dp, _i, _i, _dp, _dp, _dp]
@@ -303,7 +305,7 @@ def chi2_batch(models, data, sigma):
 
 # ------------------------------------------------------------------ SURVEY section 8(f) rows (oracle_next.c)
 DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7,
-                   "NIE": 8, "EPL": 9}
+                   "NIE": 8, "EPL": 9, "MULTIPOLE": 10}
 LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
 
 
@@ -406,3 +408,8 @@ def convolve_supersampled(rays, supersample, kernel_fine):
     out = np.empty((ny, nx))
     lib().orc_convolve_supersampled(ny, nx, s, _ptr(r), k.shape[0], k.shape[1], _ptr(k), _ptr(tmp), _ptr(out))
     return out
+
+
+def multipole_potential(x, y, m, a_m, phi_m, cx=0.0, cy=0.0):
+    p = np.array([m, a_m, phi_m, cx, cy, 0, 0, 0], dtype=np.float64)
+    return lib().orc_multipole_potential(float(x), float(y), _ptr(p))

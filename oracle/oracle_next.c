@@ -242,7 +242,7 @@ void orc_light_profiles(int64_t n, const double *bx, const double *by, int64_t n
  *          a'x + i a'y = 2 b/(1 + q) (b/R)^(t-1) sum_n a_n,  a_0 = e^(i phi),
  *          a_n = -f (2n - (2 - t))/(2n + (2 - t)) e^(2 i phi) a_(n-1),  summed until |a_n| < 1e-17 |sum| (<= 400 terms).
  */
-enum { ORC_NIE = 8, ORC_EPL = 9 };
+enum { ORC_NIE = 8, ORC_EPL = 9, ORC_MULTIPOLE = 10 };
 
 static double atan_over(double z) { return fabs(z) < 1e-4 ? 1.0 - z * z / 3.0 + z * z * z * z / 5.0 : atan(z) / z; }
 static double atanh_over(double z) { return fabs(z) < 1e-4 ? 1.0 + z * z / 3.0 + z * z * z * z / 5.0 : atanh(z) / z; }
@@ -310,15 +310,40 @@ double orc_epl_kappa(double x, double y, const double *p) {
     return 0.5 * (3.0 - p[1]) * pow(p[0] / sqrt(q * xr * xr + yr * yr / q), p[1] - 1.0);
 }
 
+/*  10 MULTIPOLE  p = {m, a_m, phi_m, cx, cy}, integer m >= 2 (reading Q36): the potential
+ *        psi = r a_m/(1 - m^2) cos(m (phi - phi_m)), whose Laplacian gives kappa = a_m cos(m (phi - phi_m))/(2 r);
+ *        alpha_r = dpsi/dr = a_m/(1 - m^2) cos(m (phi - phi_m)), alpha_phi = (1/r) dpsi/dphi = -m a_m/(1 - m^2) sin(m (phi - phi_m)),
+ *        (alpha_x, alpha_y) = (alpha_r cos phi - alpha_phi sin phi, alpha_r sin phi + alpha_phi cos phi); alpha(0) = 0. */
+double orc_multipole_potential(double x, double y, const double *p) {
+    const double dx = x - p[3], dy = y - p[4], m = p[0];
+    return sqrt(dx * dx + dy * dy) * p[1] / (1.0 - m * m) * cos(m * (atan2(dy, dx) - p[2]));
+}
+void orc_multipole_alpha(double x, double y, const double *p, double *ax, double *ay) {
+    const double dx = x - p[3], dy = y - p[4], m = p[0];
+    *ax = 0.0;
+    *ay = 0.0;
+    if (dx == 0.0 && dy == 0.0) return;
+    const double phi = atan2(dy, dx);
+    const double ar = p[1] / (1.0 - m * m) * cos(m * (phi - p[2])), aphi = -m * p[1] / (1.0 - m * m) * sin(m * (phi - p[2]));
+    *ax = ar * cos(phi) - aphi * sin(phi);
+    *ay = ar * sin(phi) + aphi * cos(phi);
+}
+double orc_multipole_kappa(double x, double y, const double *p) {
+    const double dx = x - p[3], dy = y - p[4];
+    return 0.5 * p[1] * cos(p[0] * (atan2(dy, dx) - p[2])) / sqrt(dx * dx + dy * dy);
+}
+
 /* the typed list with the second set: types [n_def], params [n_def][8] */
 void orc_profile_alpha2(int type, const double *p, double x, double y, double *ax, double *ay) {
     if (type == ORC_NIE) orc_nie_alpha(x, y, p, ax, ay);
     else if (type == ORC_EPL) orc_epl_alpha(x, y, p, ax, ay);
+    else if (type == ORC_MULTIPOLE) orc_multipole_alpha(x, y, p, ax, ay);
     else orc_profile_alpha(type, p, x, y, ax, ay);
 }
 double orc_profile_kappa2(int type, const double *p, double x, double y) {
     if (type == ORC_NIE) return orc_nie_kappa(x, y, p);
     if (type == ORC_EPL) return orc_epl_kappa(x, y, p);
+    if (type == ORC_MULTIPOLE) return orc_multipole_kappa(x, y, p);
     return orc_profile_kappa(type, p, x, y);
 }
 void orc_ray_shoot_profiles2(int64_t n, const double *tx, const double *ty, int64_t n_def, const int32_t *types,

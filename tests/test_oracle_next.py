@@ -326,6 +326,29 @@ def test_epl_against_the_mass_integral_and_hyp2f1(orc):
             assert abs(ax - float(want.real)) < 1e-13 and abs(ay - float(want.imag)) < 1e-13
 
 
+def test_multipole_is_the_gradient_of_its_potential(orc):
+    """MULTIPOLE (reading Q36), m = 2, 3, 4: alpha = grad psi by central differences of the potential; div alpha = 2 kappa
+    with the closed-form kappa = a_m cos(m (phi - phi_m))/(2 r); curl alpha = 0; |alpha| does not depend on r;
+    rotating the point by 2 pi / m leaves the radial component unchanged."""
+    rng = np.random.default_rng(86)
+    for m in (2, 3, 4):
+        p = [float(m), 0.07, 0.3, 0.1, -0.05]
+        for _ in range(25):
+            x, y = rng.uniform(-2, 2, 2)
+            if math.hypot(x - 0.1, y + 0.05) < 0.2:
+                continue
+            h = 1e-6
+            gx = (orc.multipole_potential(x + h, y, *p) - orc.multipole_potential(x - h, y, *p)) / (2 * h)
+            gy = (orc.multipole_potential(x, y + h, *p) - orc.multipole_potential(x, y - h, *p)) / (2 * h)
+            ax, ay = orc.profile_alpha("MULTIPOLE", p, x, y)
+            assert abs(ax - gx) < 1e-9 and abs(ay - gy) < 1e-9
+            div, curl = _div_curl(orc, "MULTIPOLE", p, x, y)
+            assert abs(div - 2 * orc.profile_kappa("MULTIPOLE", p, x, y)) < 2e-8 and abs(curl) < 2e-8
+            a2 = orc.profile_alpha("MULTIPOLE", p, 0.1 + 3 * (x - 0.1), -0.05 + 3 * (y + 0.05))
+            assert abs(a2[0] - ax) < 1e-14 and abs(a2[1] - ay) < 1e-14
+    assert orc.profile_alpha("MULTIPOLE", [3.0, 0.05, 0.1, 0.2, 0.3], 0.2, 0.3) == (0.0, 0.0)
+
+
 def test_core_sersic_limits(orc):
     """CORE_SERSIC (reading Q33): Rb -> 0 is definition R; far outside the break it tends to it; the inner logarithmic
     slope is -gamma; I on the R_sersic isophote for Rb = 0 is amp."""
