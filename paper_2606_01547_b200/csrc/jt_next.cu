@@ -200,6 +200,18 @@ __device__ __forceinline__ void profile_alpha(const jt_profile& d, double x, dou
             ay += sn * axr + c * ayr;
             return;
         }
+        case JT_DEFL_MULTIPOLE: {                              // reading Q36: psi = r a_m/(1 - m^2) cos(m (phi - phi_m)), m >= 2
+            const double dx = x - p[3], dy = y - p[4], m = p[0];
+            if (dx == 0.0 && dy == 0.0) return;
+            const double phi = atan2(dy, dx), amp = p[1] / (1.0 - m * m);
+            double sm, cm, sp, cp;
+            sincos(m * (phi - p[2]), &sm, &cm);
+            sincos(phi, &sp, &cp);
+            const double ar = amp * cm, aphi = -m * amp * sm;
+            ax += ar * cp - aphi * sp;
+            ay += ar * sp + aphi * cp;
+            return;
+        }
         case JT_DEFL_EPL: {                                    // reading Q32: Tessore & Metcalf (2015) series
             double c, sn, q;
             ellipticity(p[2], p[3], &c, &sn, &q);

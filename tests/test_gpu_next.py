@@ -163,8 +163,9 @@ def test_light_profiles(jt, orc, dtype):
 # ------------------------------------------------------------------ NEXT-1, second set
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_ray_shoot_profiles_nie_epl(jt, orc, dtype):
-    """NIE (readings Q31) and EPL (Q32: the Tessore-Metcalf series, summed to the same tolerance on both sides) in a
-    typed list with members of the first set; includes s_scale = 0, gamma = 2, round lenses and a ray on a centre."""
+    """NIE (readings Q31), EPL (Q32: the Tessore-Metcalf series, summed to the same tolerance on both sides) and
+    MULTIPOLE (Q36; EPL + m = 3, 4 about one centre is the paper's EPL_MULTIPOLE row without its m = 1 term) in a typed
+    list with members of the first set; includes s_scale = 0, gamma = 2, round lenses and a ray on a centre."""
     rng = np.random.default_rng(91)
     n = 3000
     tx, ty = rng.uniform(-2, 2, n), rng.uniform(-2, 2, n)
@@ -172,7 +173,9 @@ def test_ray_shoot_profiles_nie_epl(jt, orc, dtype):
     defl = [("NIE", [1.1, 0.2, -0.1, 0.15, 0.3, -0.1]), ("NIE", [0.4, 0.0, 0.0, 0.05, -0.8, 0.6]),
             ("NIE", [0.7, -0.3, 0.25, 0.0, 1.2, 1.1]), ("EPL", [1.0, 2.0, 0.15, 0.1, -0.2, 0.3]),
             ("EPL", [0.8, 1.45, -0.35, 0.3, 0.9, -0.7]), ("EPL", [0.5, 2.7, 0.5, -0.2, -1.1, -1.2]),
-            ("EPL", [0.6, 2.3, 0.0, 0.0, 0.1, 1.4]), ("SHEAR", [0.03, -0.02]), ("SIS", [0.2, 1.5, -1.5])]
+            ("EPL", [0.6, 2.3, 0.0, 0.0, 0.1, 1.4]), ("SHEAR", [0.03, -0.02]), ("SIS", [0.2, 1.5, -1.5]),
+            ("MULTIPOLE", [3.0, 0.04, 0.2, -0.2, 0.3]), ("MULTIPOLE", [4.0, -0.03, 1.1, -0.2, 0.3]),
+            ("MULTIPOLE", [2.0, 0.02, -0.4, 0.3, -0.1])]                # the last one centred on ray 0
     if dtype == "f32":
         tx, ty = _f32r(tx), _f32r(ty)
     bx, by = jt.ray_shoot_profiles(to_dev(tx, dtype), to_dev(ty, dtype), defl)
