@@ -25,8 +25,6 @@
 #include <cuda.h>
 #include <cudaTypedefs.h>
 #include <mutex>
-#include <stdlib.h>
-#include <stdio.h>
 #include <math.h>
 #include "jt_conv.cuh"
 
@@ -340,26 +338,20 @@ static ConvPlan plan_conv(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx)
     int L_min = 1;
     while (L_min <= ky && tap_elems_per_launch(npairs, (ky + L_min - 1) / L_min) * sz > (size_t)kTapBytes) ++L_min;
     if (L_min > ky) return best;                                // one kernel row does not fit the constant bank
-    int fOY = 0, fNW = 0, fL = 0, fZ = 0;                       // DEBUG: JT_CONV_FORCE=OY,NW,launches,Z
-    if (const char* f = getenv("JT_CONV_FORCE")) sscanf(f, "%d,%d,%d,%d", &fOY, &fNW, &fL, &fZ);
     for (int OY : kOYs) {
-        if (fOY && OY != fOY) continue;
         if (d == JT_F64 && OY > kMaxOYf64) continue;
         for (int NW = 8; NW >= 2; NW -= 2) {                    // even: odd warp counts measured 5-15 % slower
-            if (fNW && NW != fNW) continue;
             const int TH = NW * OY;
             const int tiles_x = (nx + xoff + kConvTW - 1) / kConvTW, tiles_y = (ny + TH - 1) / TH;
             const int64_t tiles = (int64_t)tiles_x * tiles_y * B;
             if ((int64_t)tiles_y * B > 0x7fffffffLL || tiles_x > 65535) continue;
             for (int L = L_min; L <= L_min + 2 && L <= ky; ++L) {
-                if (fL && L != fL) continue;
                 const int kb = (ky + L - 1) / L;
                 if (L > L_min && (ky + kb - 1) / kb != L) continue;
                 const int ths = TH + kb - 1;
                 if (ths > 256) continue;
                 const int unit = sz == 4 ? 2 : 1;               // float: every rank's first tile column stays 16-byte aligned
                 for (int Z = 1; Z <= kMaxSplit && Z * unit <= npairs + unit - 1; ++Z) {
-                    if (fZ && Z != fZ) continue;
                     int m_lo, mz;
                     rank_share(npairs, unit, Z, 0, &m_lo, &mz);  // rank 0 has the largest share
                     const int tws = (int)(align_up((size_t)(shift + kConvTW + 2 * mz - 2) * sz, 16) / sz);
