@@ -69,16 +69,17 @@ __device__ __forceinline__ double t_log(double x) { return log(x); }
 //   brace = (t-1+2X^2) F(X) + c1 + S (c2 L - pi),  t = tau^2, c1 = tau pi + (t-1) ln tau, c2 = (t-1)/tau,
 //   S = sqrt(t+X^2), L = ln(X/(S+tau)).
 // ------------------------------------------------------------------------------------------------
-// Far-far field: for X >= 9 max(1, tau) (double; 8 max(1, tau) in float) the brace is summed from its expansion in
+// Far-far field: for X >= 9 max(1, tau) (double; 6.5 max(1, tau) in float) the brace is summed from its expansion in
 // 1/X, derived with sympy from the closed form (every coefficient carries the factor (t+1)^2; the 1/X term vanishes):
 //   brace = b0 + b2 / X^2 + b3 / X^3 + ... ,   b0 = (t-1) ln tau - t + pi tau - 1 (the total-mass limit),
 //   b2 = -(t+1)^2/3, b3 = pi (t+1)^2/8, b4 = 2 (t+1)^2 (t-3)/15, b5 = -pi (t+1)^2 (t-2)/16, ...
-// Truncated after 1/X^13 (double) / 1/X^8 (float) the relative error is <= 1e-13 / 2e-8 beyond those radii (reading
+// Truncated after 1/X^13 (double) / 1/X^8 (float) the relative error is <= 1e-13 / 3e-8 beyond those radii (reading
 // Q9b in DESIGN.md: verified against the closed form at 50 digits for tau = 0.3 ... 1000).  With v = 1/R (NOT 1/X: the
 // powers of Rs are folded into the coefficients, a_k = amp b_k Rs^k) the deflection is alpha = f (dx, dy),
 //   f = v^2 (a_0 + v^2 (a_2 + a_3 v + ... + a_K v^(K-2))):  one MUFU and K + 1 multiply-adds per evaluation.
 // The farther the ray, the shorter the sum: three levels (K, radius in units of max(1, tau) Rs), each within the same
-// error bound (double 1e-13: 2.2e-14 / 6.0e-14 / 5e-14 worst case at tau = 1 on the radius; float 4.2e-9 / 4.0e-9 / 3.5e-9):
+// error bound (double 1e-13: 2.2e-14 / 6.0e-14 / 5e-14 worst case at tau = 1 on the radius; float 3e-8 = half an ulp:
+// 2.7e-8 / 2.2e-8 / 2.1e-8):
 template <typename T> struct FarFar;
 template <> struct FarFar<double> {
     static constexpr int K = 13, K1 = 9, K2 = 7;
@@ -86,7 +87,7 @@ template <> struct FarFar<double> {
 };
 template <> struct FarFar<float> {
     static constexpr int K = 8, K1 = 5, K2 = 4;
-    static constexpr double kRadius = 8.0, kRadius1 = 24.0, kRadius2 = 46.0;
+    static constexpr double kRadius = 6.5, kRadius1 = 18.0, kRadius2 = 32.0;
 };
 
 // Field order = access order: the far-far loop reads the first (K + 3) values only (centre, a_0, a_2 ... a_K); the

@@ -382,7 +382,7 @@ def test_image_edge_cases(jt, orc, dtype):
 @pytest.mark.parametrize("s", [1, 2, 5])
 def test_image_series_levels_and_cores(jt, orc, dtype, s):
     """jt_simulate_image's per-warp-tile sort: a few VERY strong subhalos (alpha_Rs = 0.5-2 arcsec,
-    hundreds of times the priors') whose three far-far radii (9 / 20 / 44 max(1, tau) Rs in double, 8 / 24 / 46 in float),
+    hundreds of times the priors') whose three far-far radii (9 / 20 / 44 max(1, tau) Rs in double, 6.5 / 18 / 32 in float),
     far and near zones all fall inside the grid, so that every warp tile puts some of them in every class; two of them
     sit exactly on a ray and exactly between rays.  The source is broad and shallow (n = 1), so max|img| does not dwarf
     the pixels the subhalos act on.  The float64 tolerance here is 1e-12, a hundred times tighter than the north-star
