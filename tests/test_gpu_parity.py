@@ -531,3 +531,23 @@ def test_batch_c3_full_size_sampled(jt, orc):
     want = orc.simulate_batch(bw, systems=idx)
     worst = max(rel_err(got[b], want[k]) for k, b in enumerate(idx))
     assert worst < TOL_IMG["f32"], worst
+
+
+def test_results_are_bitwise_reproducible(jt):
+    """Arrival-order mechanisms (last warp / CTA to arrive reduces the split subhalo list, warp tiles handed out by a
+    counter in the batch kernel, convolution partial sums meeting in L2) must not leak into the numbers: every reduction
+    runs in a fixed order, so repeated calls agree bit for bit."""
+    import torch
+    for dtype in ("f64", "f32"):
+        w = workloads.config_c2(nx=48, n_tnfw=3000, dtype=dtype)          # few ray tiles: the subhalo list is split
+        a = gpu_simulate(jt, w, method="direct")
+        for _ in range(3):
+            assert np.array_equal(a, gpu_simulate(jt, w, method="direct"))
+        w5 = workloads.config_c4(nx=40, n_tnfw=2000, K=31, dtype=dtype)   # s = 5: CTA-wide tiles, per-CTA completion
+        b = gpu_simulate(jt, w5, method="direct")
+        for _ in range(3):
+            assert np.array_equal(b, gpu_simulate(jt, w5, method="direct"))
+    bw = workloads.config_c3(B=24, nx=32, n_tnfw=60, dtype="f32")
+    c = _gpu_batch(jt, bw)
+    for _ in range(3):
+        assert np.array_equal(c, _gpu_batch(jt, bw))
