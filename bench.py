@@ -629,6 +629,56 @@ def run_conv_sweep(args, rank):
                       "n_gpus": 1, "data": "synthetic", "rows": rows}), flush=True)
 
 
+def run_swarm(args, rank):
+    """--swarm: the shape of the paper's particle-swarm benchmark (64 ... 512 particles, 100 x 100 grid,
+    13-pixel PSF): one swarm step = every particle's image simulated and reduced to its
+    chi^2 against the same data by jt_simulate_batch_chi2 (images never leave the chip).  Device time per step from a
+    CUDA-graph replay, wall time per step with the particles' parameters copied from pinned host memory and the B chi^2
+    values copied back.  The paper's numbers (59 / 138 / 245 / 555 s with lenstronomy for whole fits of unstated
+    iteration counts) are context only: the optimiser is out of scope."""
+    if rank != 0:
+        return
+    import torch
+    import paper_2606_01547_b200 as jt
+    import workloads
+    torch.cuda.set_device(0)
+    jt.lib()
+    rows = []
+    for dtype, tdt in (("f64", torch.float64), ("f32", torch.float32)):
+        for B in (64, 128, 256, 512):
+            w = workloads.config_swarm(B=B, dtype=dtype)
+            g = jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample)
+            pin = lambda a: torch.as_tensor(np.ascontiguousarray(a), dtype=tdt).pin_memory()
+            h = [pin(w.sie), pin(w.shear), pin(w.sources), pin(w.psf)]
+            d = [t.to("cuda") for t in h]
+            truth = jt.simulate_batch(g, d[0][:1], d[1][:1], None, d[2][:1], d[3][:1])[0]
+            data = truth + torch.as_tensor(w.data, dtype=tdt, device="cuda")
+            sigma = torch.as_tensor(w.sigma, dtype=tdt, device="cuda")
+            chi2 = torch.empty(B, dtype=torch.float64, device="cuda")
+            h_chi2 = torch.empty(B, dtype=torch.float64).pin_memory()
+            step = lambda: jt.simulate_batch_chi2(g, d[0], d[1], None, d[2], d[3], data, sigma, chi2=chi2)
+            us = graph_time(torch, step)
+
+            def e2e():
+                for dd, hh in zip(d[:3], h[:3]):
+                    dd.copy_(hh, non_blocking=True)
+                step()
+                h_chi2.copy_(chi2, non_blocking=True)
+                torch.cuda.synchronize()
+            for _ in range(3):
+                e2e()
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                e2e()
+            wall = 1e6 * (time.perf_counter() - t0) / args.steps
+            rows.append({"dtype": dtype, "particles": B, "device_us_per_step": us, "e2e_us_per_step": wall,
+                         "particle_images_per_s": B / (us * 1e-6), "chi2_of_truth_per_pixel": float(h_chi2[0]) / (w.nx * w.ny)})
+    print(json.dumps({"metric": "swarm_step_us", "unit": "us per swarm step (all particles: image + chi^2)", "n_gpus": 1,
+                      "data": "synthetic", "grid": "100x100", "psf": "13x13", "rows": rows,
+                      "paper_context": "PAPER.md:122-126: whole PSO fits, lenstronomy 59/138/245/555 s for 64/128/256/512 particles"}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -643,12 +693,15 @@ def main():
     ap.add_argument("--no-per-config", action="store_true", help="skip the per_config block (C2-f64, C2-f32, C3-f32)")
     ap.add_argument("--conv-sweep", action="store_true", help="time jt_psf_convolve alone at the paper's shapes")
     ap.add_argument("--sweep-batch", type=int, default=1024, help="batch size of the batched rows of --conv-sweep")
+    ap.add_argument("--swarm", action="store_true", help="time the particle-swarm inner loop (NEXT-3) at the paper's sizes")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank, world, local_rank = dist_init(args.gpus)
     try:
         if args.conv_sweep:
             run_conv_sweep(args, rank)
+        elif args.swarm:
+            run_swarm(args, rank)
         elif args.impl == "reference":
             run_reference(args, rank, world)
         else:
