@@ -325,7 +325,7 @@ static int conv_regs(jt_dtype d, int OY) { return d == JT_F64 ? 16 * OY : 16 + 6
 // pair, kernel row) step of one warp occupies its scheduler's FMA pipe for 4 OY (float: 2 OY FFMA2) or 8 OY (double:
 // 4 OY DFMA) cycles plus the window load's register write-back; an SM runs ceil(CTAs / 148) CTAs' worth of such steps
 // on 4 schedulers, at an efficiency that grows with the warps resident per scheduler.
-static ConvPlan plan_conv(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx) {
+static ConvPlan plan_conv_search(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx) {
     ConvPlan best = {};
     best.ok = false;
     const size_t sz = dtype_size(d);
@@ -393,6 +393,20 @@ static ConvPlan plan_conv(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx)
         }
     }
     return best;
+}
+
+// The search visits ~1000 (OY, warps, bands, Z) combinations and an API call asks for the plan several times
+// (supported? / estimate / workspace / launch): the last few answers are kept per host thread.
+static ConvPlan plan_conv(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx) {
+    struct Slot { int d; int64_t B; int ny, nx, ky, kx; ConvPlan p; bool used; };
+    static thread_local Slot cache[4] = {};
+    static thread_local int next = 0;
+    for (const Slot& c : cache)
+        if (c.used && c.d == (int)d && c.B == B && c.ny == ny && c.nx == nx && c.ky == ky && c.kx == kx) return c.p;
+    Slot& c = cache[next];
+    next = (next + 1) & 3;
+    c = {(int)d, B, ny, nx, ky, kx, plan_conv_search(d, B, ny, nx, ky, kx), true};
+    return c.p;
 }
 
 // ------------------------------------------------------------------------------------------------ small problems
