@@ -305,7 +305,7 @@ def chi2_batch(models, data, sigma):
 
 # ------------------------------------------------------------------ SURVEY section 8(f) rows (oracle_next.c)
 DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7,
-                   "NIE": 8, "EPL": 9, "MULTIPOLE": 10}
+                   "NIE": 8, "EPL": 9, "MULTIPOLE": 10, "CSE": 11}
 LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
 
 

@@ -242,7 +242,7 @@ void orc_light_profiles(int64_t n, const double *bx, const double *by, int64_t n
  *          a'x + i a'y = 2 b/(1 + q) (b/R)^(t-1) sum_n a_n,  a_0 = e^(i phi),
  *          a_n = -f (2n - (2 - t))/(2n + (2 - t)) e^(2 i phi) a_(n-1),  summed until |a_n| < 1e-17 |sum| (<= 400 terms).
  */
-enum { ORC_NIE = 8, ORC_EPL = 9, ORC_MULTIPOLE = 10 };
+enum { ORC_NIE = 8, ORC_EPL = 9, ORC_MULTIPOLE = 10, ORC_CSE = 11 };
 
 static double atan_over(double z) { return fabs(z) < 1e-4 ? 1.0 - z * z / 3.0 + z * z * z * z / 5.0 : atan(z) / z; }
 static double atanh_over(double z) { return fabs(z) < 1e-4 ? 1.0 + z * z / 3.0 + z * z * z * z / 5.0 : atanh(z) / z; }
@@ -333,17 +333,45 @@ double orc_multipole_kappa(double x, double y, const double *p) {
     return 0.5 * p[1] * cos(p[0] * (atan2(dy, dx) - p[2])) / sqrt(dx * dx + dy * dy);
 }
 
+/*  11 CSE (cored steep ellipsoid; reading Q37)  p = {A, s, e1, e2, cx, cy}
+ *        kappa = A / (2 (s^2 + x'^2 + y'^2/q^2)^(3/2))  (Oguri 2021: the major axis along x', NOT the product-averaged
+ *        radius of definitions S and R), deflection in the lens frame with psi = sqrt(q^2 (s^2 + x'^2) + y'^2):
+ *          a'x = A q x' (psi + q^2 s) / (s psi [(psi + s)^2 + (1 - q^2) x'^2]),
+ *          a'y = A q y' (psi + s)     / (s psi [(psi + s)^2 + (1 - q^2) x'^2]). */
+void orc_cse_alpha(double x, double y, const double *p, double *ax, double *ay) {
+    double phi0, q;
+    orc_ellipticity(p[2], p[3], &phi0, &q);
+    const double c = cos(phi0), sn = sin(phi0), s = p[1];
+    const double dx = x - p[4], dy = y - p[5];
+    const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+    const double psi = sqrt(q * q * (s * s + xr * xr) + yr * yr);
+    const double den = s * psi * ((psi + s) * (psi + s) + (1.0 - q * q) * xr * xr);
+    const double axr = p[0] * q * xr * (psi + q * q * s) / den, ayr = p[0] * q * yr * (psi + s) / den;
+    *ax = c * axr - sn * ayr;
+    *ay = sn * axr + c * ayr;
+}
+double orc_cse_kappa(double x, double y, const double *p) {
+    double phi0, q;
+    orc_ellipticity(p[2], p[3], &phi0, &q);
+    const double c = cos(phi0), sn = sin(phi0);
+    const double dx = x - p[4], dy = y - p[5];
+    const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+    return 0.5 * p[0] / pow(p[1] * p[1] + xr * xr + yr * yr / (q * q), 1.5);
+}
+
 /* the typed list with the second set: types [n_def], params [n_def][8] */
 void orc_profile_alpha2(int type, const double *p, double x, double y, double *ax, double *ay) {
     if (type == ORC_NIE) orc_nie_alpha(x, y, p, ax, ay);
     else if (type == ORC_EPL) orc_epl_alpha(x, y, p, ax, ay);
     else if (type == ORC_MULTIPOLE) orc_multipole_alpha(x, y, p, ax, ay);
+    else if (type == ORC_CSE) orc_cse_alpha(x, y, p, ax, ay);
     else orc_profile_alpha(type, p, x, y, ax, ay);
 }
 double orc_profile_kappa2(int type, const double *p, double x, double y) {
     if (type == ORC_NIE) return orc_nie_kappa(x, y, p);
     if (type == ORC_EPL) return orc_epl_kappa(x, y, p);
     if (type == ORC_MULTIPOLE) return orc_multipole_kappa(x, y, p);
+    if (type == ORC_CSE) return orc_cse_kappa(x, y, p);
     return orc_profile_kappa(type, p, x, y);
 }
 void orc_ray_shoot_profiles2(int64_t n, const double *tx, const double *ty, int64_t n_def, const int32_t *types,

@@ -349,6 +349,36 @@ def test_multipole_is_the_gradient_of_its_potential(orc):
     assert orc.profile_alpha("MULTIPOLE", [3.0, 0.05, 0.1, 0.2, 0.3], 0.2, 0.3) == (0.0, 0.0)
 
 
+def test_cse_sphere_mass_integral_and_potential_flow(orc):
+    """CSE (reading Q37): q = 1 is the cored steep sphere, alpha = A (1/s - 1/sqrt(s^2 + r^2))/r (enclosed mass of
+    kappa = A/(2 (s^2 + r^2)^(3/2))); div alpha = 2 kappa and curl alpha = 0; the deflection from its OWN convergence by
+    brute-force 2-D integration (kappa ~ r^-3: the cut at rmax = 200 leaves 1e-4 of the mass outside); total mass
+    pi A q / s."""
+    rng = np.random.default_rng(87)
+    for s in (0.05, 0.4, 1.5):
+        for _ in range(10):
+            x, y = rng.uniform(-2, 2, 2)
+            ax, ay = orc.profile_alpha("CSE", [0.8, s, 0.0, 0.0, 0.0, 0.0], x, y)
+            r = math.hypot(x, y)
+            want = 0.8 * (1.0 / s - 1.0 / math.sqrt(s * s + r * r)) / r
+            assert abs(ax - want * x / r) < 1e-13 * max(1.0, want) and abs(ay - want * y / r) < 1e-13 * max(1.0, want)
+    for e1, e2, s in ((0.2, 0.1, 0.3), (-0.35, 0.3, 0.1), (0.5, -0.3, 1.0)):
+        p = [0.6, s, e1, e2, 0.1, 0.05]
+        for _ in range(30):
+            x, y = rng.uniform(-2, 2, 2)
+            div, curl = _div_curl(orc, "CSE", p, x, y, h=1e-5)
+            k = orc.profile_kappa("CSE", p, x, y)
+            assert abs(div - 2 * k) < 1e-7 * max(1.0, k) and abs(curl) < 1e-7
+    p = [0.6, 0.25, 0.3, -0.2, 0.0, 0.0]
+    kap = lambda u, v: orc.profile_kappa("CSE", p, u, v)
+    ax, ay = _brute_alpha(kap, 0.7, 0.2, rmax=200.0)
+    bx, by = orc.profile_alpha("CSE", p, 0.7, 0.2)
+    assert abs(ax - bx) < 2e-4 and abs(ay - by) < 2e-4
+    _, q = orc.ellipticity(0.3, -0.2)
+    far = orc.profile_alpha("CSE", p, 3000.0, 0.0)                    # a point mass of pi A q / s: alpha = M / (pi r)
+    assert abs(far[0] * 3000.0 - 0.6 * q / 0.25) < 1e-3
+
+
 def test_core_sersic_limits(orc):
     """CORE_SERSIC (reading Q33): Rb -> 0 is definition R; far outside the break it tends to it; the inner logarithmic
     slope is -gamma; I on the R_sersic isophote for Rb = 0 is amp."""
