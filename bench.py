@@ -48,8 +48,8 @@ TIER_NAMES = ("far_far_long", "far_far_mid", "far_far_short", "far", "mid", "col
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu --set full captures in
 # profiles/r02_ncu_{c4f64,c2f64,c2f32,c3f32}.txt (the kernels are ALU-bound: compulsory traffic is the records in, the
 # image out and, for C2, the partial sums of the split subhalo list)
-NCU_TRAFFIC_BYTES = {"C4-f64": 11405568 + 4258048, "C2-f64": 2339072 + 784384, "C2-f32": 1172480 + 527616,
-                     "C3-f32": 15828992 + 42210560}
+NCU_TRAFFIC_BYTES = {"C4-f64": 11405568 + 4258048, "C2-f64": 2339072 + 784384, "C2-f32": 1172992 + 382208,
+                     "C3-f32": 15794688 + 36633088}
 ALU_LANES_PER_SM = {"f32": 128, "f64": 64}
 WORKLOADS = ("C0-f64", "C1-f64", "C2-f32", "C2-f64", "C3-f32", "C4-f64")
 PER_CONFIG = ("C2-f64", "C2-f32", "C3-f32")        # reported beside the headline workload in the same JSON line

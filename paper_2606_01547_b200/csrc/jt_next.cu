@@ -200,6 +200,18 @@ __device__ __forceinline__ void profile_alpha(const jt_profile& d, double x, dou
             ay += sn * axr + c * ayr;
             return;
         }
+        case JT_DEFL_CSE: {                                    // reading Q37 (Oguri 2021): kappa = A/(2 (s^2 + x'^2 + y'^2/q^2)^(3/2))
+            double c, sn, q;
+            ellipticity(p[2], p[3], &c, &sn, &q);
+            const double dx = x - p[4], dy = y - p[5], s = p[1];
+            const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+            const double psi = sqrt(q * q * (s * s + xr * xr) + yr * yr);
+            const double pre = p[0] * q / (s * psi * ((psi + s) * (psi + s) + (1.0 - q * q) * xr * xr));
+            const double axr = pre * xr * (psi + q * q * s), ayr = pre * yr * (psi + s);
+            ax += c * axr - sn * ayr;
+            ay += sn * axr + c * ayr;
+            return;
+        }
         case JT_DEFL_MULTIPOLE: {                              // reading Q36: psi = r a_m/(1 - m^2) cos(m (phi - phi_m)), m >= 2
             const double dx = x - p[3], dy = y - p[4], m = p[0];
             if (dx == 0.0 && dy == 0.0) return;
