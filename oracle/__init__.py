@@ -97,6 +97,8 @@ def lib():
         L.orc_profile_kappa2.argtypes = [_i, _dp, _d, _d]
         L.orc_profile_kappa2.restype = _d
         L.orc_ray_shoot_profiles2.argtypes = [_i64, _dp, _dp, _i64, _i32p, _dp, _dp, _dp]
+        L.orc_pjaffe_ell_potential.argtypes = [_d, _d, _dp]
+        L.orc_pjaffe_ell_potential.restype = _d
         L.orc_multipole_potential.argtypes = [_d, _d, _dp]
         L.orc_multipole_potential.restype = _d
         L.orc_core_sersic_n.argtypes = [_i64, _dp, _dp, _dp, _d, _d, _dp]
@@ -305,7 +307,7 @@ def chi2_batch(models, data, sigma):
 
 # ------------------------------------------------------------------ SURVEY section 8(f) rows (oracle_next.c)
 DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7,
-                   "NIE": 8, "EPL": 9, "MULTIPOLE": 10, "CSE": 11}
+                   "NIE": 8, "EPL": 9, "MULTIPOLE": 10, "CSE": 11, "PJAFFE_ELLIPSE_POTENTIAL": 12}
 LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
 
 
@@ -413,3 +415,8 @@ def convolve_supersampled(rays, supersample, kernel_fine):
 def multipole_potential(x, y, m, a_m, phi_m, cx=0.0, cy=0.0):
     p = np.array([m, a_m, phi_m, cx, cy, 0, 0, 0], dtype=np.float64)
     return lib().orc_multipole_potential(float(x), float(y), _ptr(p))
+
+
+def pjaffe_ell_potential(x, y, sigma0, Ra, Rs, e1, e2, cx=0.0, cy=0.0):
+    p = np.array([sigma0, Ra, Rs, e1, e2, cx, cy, 0], dtype=np.float64)
+    return lib().orc_pjaffe_ell_potential(float(x), float(y), _ptr(p))

@@ -242,7 +242,7 @@ void orc_light_profiles(int64_t n, const double *bx, const double *by, int64_t n
  *          a'x + i a'y = 2 b/(1 + q) (b/R)^(t-1) sum_n a_n,  a_0 = e^(i phi),
  *          a_n = -f (2n - (2 - t))/(2n + (2 - t)) e^(2 i phi) a_(n-1),  summed until |a_n| < 1e-17 |sum| (<= 400 terms).
  */
-enum { ORC_NIE = 8, ORC_EPL = 9, ORC_MULTIPOLE = 10, ORC_CSE = 11 };
+enum { ORC_NIE = 8, ORC_EPL = 9, ORC_MULTIPOLE = 10, ORC_CSE = 11, ORC_PJAFFE_ELL = 12 };
 
 static double atan_over(double z) { return fabs(z) < 1e-4 ? 1.0 - z * z / 3.0 + z * z * z * z / 5.0 : atan(z) / z; }
 static double atanh_over(double z) { return fabs(z) < 1e-4 ? 1.0 + z * z / 3.0 + z * z * z * z / 5.0 : atanh(z) / z; }
@@ -359,12 +359,65 @@ double orc_cse_kappa(double x, double y, const double *p) {
     return 0.5 * p[0] / pow(p[1] * p[1] + xr * xr + yr * yr / (q * q), 1.5);
 }
 
+/*  12 PJAFFE_ELLIPSE_POTENTIAL (reading Q38)  p = {sigma0, Ra, Rs, e1, e2, cx, cy}: the PJAFFE lensing
+ *        POTENTIAL made elliptical, psi(x', y') = psi_PJ(Re), Re = sqrt(q x'^2 + y'^2/q) (the product-averaged radius of
+ *        definitions S and R), psi_PJ(R) = C [f(Ra) - f(Rs)], f(a) = sqrt(a^2 + R^2) - a ln(a + sqrt(a^2 + R^2)),
+ *        C = 2 sigma0 Ra Rs/(Rs - Ra), so that dpsi_PJ/dR is the PJAFFE deflection a(R) of reading Q29.  Then
+ *          a'x = a(Re) q x'/Re,  a'y = a(Re) y'/(q Re);   kappa = (psi_xx + psi_yy)/2 with a'(R) = 2 kappa_PJ(R) - a(R)/R. */
+static double pjaffe_a(const double *p, double R) {            /* p = sigma0, Ra, Rs */
+    const double Ra = p[1], Rs = p[2];
+    return 2.0 * p[0] * Ra * Rs / (Rs - Ra) * ((sqrt(Ra * Ra + R * R) - Ra) - (sqrt(Rs * Rs + R * R) - Rs)) / R;
+}
+static double pjaffe_kappa(const double *p, double R) {
+    const double Ra = p[1], Rs = p[2];
+    return p[0] * Ra * Rs / (Rs - Ra) * (1.0 / sqrt(Ra * Ra + R * R) - 1.0 / sqrt(Rs * Rs + R * R));
+}
+double orc_pjaffe_ell_potential(double x, double y, const double *p) {
+    double phi0, q;
+    orc_ellipticity(p[3], p[4], &phi0, &q);
+    const double c = cos(phi0), sn = sin(phi0);
+    const double dx = x - p[5], dy = y - p[6];
+    const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+    const double R2 = q * xr * xr + yr * yr / q, Ra = p[1], Rs = p[2];
+    const double sa = sqrt(Ra * Ra + R2), ss = sqrt(Rs * Rs + R2);
+    return 2.0 * p[0] * Ra * Rs / (Rs - Ra) * ((sa - Ra * log(Ra + sa)) - (ss - Rs * log(Rs + ss)));
+}
+void orc_pjaffe_ell_alpha(double x, double y, const double *p, double *ax, double *ay) {
+    double phi0, q;
+    orc_ellipticity(p[3], p[4], &phi0, &q);
+    const double c = cos(phi0), sn = sin(phi0);
+    const double dx = x - p[5], dy = y - p[6];
+    const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+    const double Re = sqrt(q * xr * xr + yr * yr / q);
+    *ax = 0.0;
+    *ay = 0.0;
+    if (Re == 0.0) return;
+    const double a = pjaffe_a(p, Re);
+    const double axr = a * q * xr / Re, ayr = a * yr / (q * Re);
+    *ax = c * axr - sn * ayr;
+    *ay = sn * axr + c * ayr;
+}
+double orc_pjaffe_ell_kappa(double x, double y, const double *p) {
+    double phi0, q;
+    orc_ellipticity(p[3], p[4], &phi0, &q);
+    const double c = cos(phi0), sn = sin(phi0);
+    const double dx = x - p[5], dy = y - p[6];
+    const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+    const double R2 = q * xr * xr + yr * yr / q, R = sqrt(R2);
+    const double a = pjaffe_a(p, R), da = 2.0 * pjaffe_kappa(p, R) - a / R;
+    const double gx = q * xr / R, gy = yr / (q * R);                 /* grad Re */
+    const double pxx = da * gx * gx + a * (q / R - q * q * xr * xr / (R2 * R));
+    const double pyy = da * gy * gy + a * (1.0 / (q * R) - yr * yr / (q * q * R2 * R));
+    return 0.5 * (pxx + pyy);
+}
+
 /* the typed list with the second set: types [n_def], params [n_def][8] */
 void orc_profile_alpha2(int type, const double *p, double x, double y, double *ax, double *ay) {
     if (type == ORC_NIE) orc_nie_alpha(x, y, p, ax, ay);
     else if (type == ORC_EPL) orc_epl_alpha(x, y, p, ax, ay);
     else if (type == ORC_MULTIPOLE) orc_multipole_alpha(x, y, p, ax, ay);
     else if (type == ORC_CSE) orc_cse_alpha(x, y, p, ax, ay);
+    else if (type == ORC_PJAFFE_ELL) orc_pjaffe_ell_alpha(x, y, p, ax, ay);
     else orc_profile_alpha(type, p, x, y, ax, ay);
 }
 double orc_profile_kappa2(int type, const double *p, double x, double y) {
@@ -372,6 +425,7 @@ double orc_profile_kappa2(int type, const double *p, double x, double y) {
     if (type == ORC_EPL) return orc_epl_kappa(x, y, p);
     if (type == ORC_MULTIPOLE) return orc_multipole_kappa(x, y, p);
     if (type == ORC_CSE) return orc_cse_kappa(x, y, p);
+    if (type == ORC_PJAFFE_ELL) return orc_pjaffe_ell_kappa(x, y, p);
     return orc_profile_kappa(type, p, x, y);
 }
 void orc_ray_shoot_profiles2(int64_t n, const double *tx, const double *ty, int64_t n_def, const int32_t *types,

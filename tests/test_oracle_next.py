@@ -379,6 +379,31 @@ def test_cse_sphere_mass_integral_and_potential_flow(orc):
     assert abs(far[0] * 3000.0 - 0.6 * q / 0.25) < 1e-3
 
 
+def test_pjaffe_ellipse_potential(orc):
+    """PJAFFE_ELLIPSE_POTENTIAL (reading Q38): e = 0 is PJAFFE exactly; alpha = grad psi by central differences of the
+    elliptical potential (whose radial derivative is the already pinned PJAFFE deflection); div alpha = 2 kappa with
+    the analytic Laplacian; curl alpha = 0."""
+    rng = np.random.default_rng(88)
+    for _ in range(20):
+        x, y = rng.uniform(-2, 2, 2)
+        a = orc.profile_alpha("PJAFFE_ELLIPSE_POTENTIAL", [0.7, 0.1, 0.9, 0.0, 0.0, 0.2, -0.1], x, y)
+        b = orc.profile_alpha("PJAFFE", [0.7, 0.1, 0.9, 0.2, -0.1], x, y)
+        assert abs(a[0] - b[0]) < 1e-14 and abs(a[1] - b[1]) < 1e-14
+    for e1, e2 in ((0.2, 0.1), (-0.3, 0.25), (0.05, -0.4)):
+        p = [0.7, 0.1, 0.9, e1, e2, 0.2, -0.1]
+        for _ in range(25):
+            x, y = rng.uniform(-2, 2, 2)
+            h = 1e-6
+            gx = (orc.pjaffe_ell_potential(x + h, y, *p) - orc.pjaffe_ell_potential(x - h, y, *p)) / (2 * h)
+            gy = (orc.pjaffe_ell_potential(x, y + h, *p) - orc.pjaffe_ell_potential(x, y - h, *p)) / (2 * h)
+            ax, ay = orc.profile_alpha("PJAFFE_ELLIPSE_POTENTIAL", p, x, y)
+            assert abs(ax - gx) < 2e-9 and abs(ay - gy) < 2e-9
+            div, curl = _div_curl(orc, "PJAFFE_ELLIPSE_POTENTIAL", p, x, y)
+            k = orc.profile_kappa("PJAFFE_ELLIPSE_POTENTIAL", p, x, y)
+            assert abs(div - 2 * k) < 5e-8 * max(1.0, abs(k)) and abs(curl) < 5e-8
+    assert orc.profile_alpha("PJAFFE_ELLIPSE_POTENTIAL", [0.7, 0.1, 0.9, 0.2, 0.1, 0.2, -0.1], 0.2, -0.1) == (0.0, 0.0)
+
+
 def test_core_sersic_limits(orc):
     """CORE_SERSIC (reading Q33): Rb -> 0 is definition R; far outside the break it tends to it; the inner logarithmic
     slope is -gamma; I on the R_sersic isophote for Rb = 0 is amp."""
