@@ -204,6 +204,7 @@ JT_API jt_status jt_lensing_maps(jt_dtype dtype, int64_t n, const void *theta_x,
  *   JT_DEFL_EPL         (:66-70)        theta_E, gamma, e1, e2, cx, cy     elliptical power law, 1 < gamma < 3 (Q32)
  *   JT_DEFL_MULTIPOLE   (:76)           m, a_m, phi_m, cx, cy              multipole of integer order m >= 2 (Q36)
  *   JT_DEFL_CSE         (:65)           A, s, e1, e2, cx, cy               cored steep ellipsoid, s > 0 (Q37)
+ *   JT_DEFL_PJAFFE_ELLIPSE_POTENTIAL (:84)  sigma0, Ra, Rs, e1, e2, cx, cy     PJAFFE potential made elliptical (Q38)
  *   light
  *   JT_LIGHT_SERSIC_ELLIPSE   (:103)    amp, R_sersic, n_sersic, e1, e2, cx, cy      definition R
  *   JT_LIGHT_GAUSSIAN_ELLIPSE (:98-101) amp (total flux), sigma, e1, e2, cx, cy; GAUSSIAN is e1 = e2 = 0,
@@ -211,7 +212,8 @@ JT_API jt_status jt_lensing_maps(jt_dtype dtype, int64_t n, const void *theta_x,
  * Formulas: DESIGN.md readings Q26-Q30.  Unknown types contribute nothing. */
 typedef enum { JT_DEFL_CONVERGENCE = 0, JT_DEFL_SIS = 1, JT_DEFL_NFW = 2, JT_DEFL_HERNQUIST = 3, JT_DEFL_PJAFFE = 4,
                JT_DEFL_SIE = 5, JT_DEFL_SHEAR = 6, JT_DEFL_TNFW = 7, JT_DEFL_NIE = 8, JT_DEFL_EPL = 9,
-               JT_DEFL_MULTIPOLE = 10, JT_DEFL_CSE = 11 } jt_deflector_type;
+               JT_DEFL_MULTIPOLE = 10, JT_DEFL_CSE = 11,
+               JT_DEFL_PJAFFE_ELLIPSE_POTENTIAL = 12 } jt_deflector_type;
 typedef enum { JT_LIGHT_SERSIC_ELLIPSE = 0, JT_LIGHT_GAUSSIAN_ELLIPSE = 1 } jt_light_type;
 typedef struct { int32_t type; int32_t reserved; double p[8]; } jt_profile;
 /* beta = theta - sum of the n_def deflectors.  theta, beta: device [n]; deflectors: device [n_def]. */

@@ -449,7 +449,7 @@ def lensing_maps(theta_x, theta_y, sie=None, shear=None, tnfw=None, stream=None)
 
 
 DEFLECTOR_TYPES = {"CONVERGENCE": 0, "SIS": 1, "NFW": 2, "HERNQUIST": 3, "PJAFFE": 4, "SIE": 5, "SHEAR": 6, "TNFW": 7,
-                   "NIE": 8, "EPL": 9, "MULTIPOLE": 10, "CSE": 11}
+                   "NIE": 8, "EPL": 9, "MULTIPOLE": 10, "CSE": 11, "PJAFFE_ELLIPSE_POTENTIAL": 12}
 LIGHT_TYPES = {"SERSIC_ELLIPSE": 0, "GAUSSIAN_ELLIPSE": 1}
 _PROFILE_DT = np.dtype([("type", np.int32), ("reserved", np.int32), ("p", np.float64, 8)])     # jt_profile, 72 bytes
 

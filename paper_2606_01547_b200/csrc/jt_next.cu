@@ -212,6 +212,20 @@ __device__ __forceinline__ void profile_alpha(const jt_profile& d, double x, dou
             ay += sn * axr + c * ayr;
             return;
         }
+        case JT_DEFL_PJAFFE_ELLIPSE_POTENTIAL: {               // reading Q38: psi(x', y') = psi_PJ(sqrt(q x'^2 + y'^2/q))
+            double c, sn, q;
+            ellipticity(p[3], p[4], &c, &sn, &q);
+            const double dx = x - p[5], dy = y - p[6];
+            const double xr = c * dx + sn * dy, yr = -sn * dx + c * dy;
+            const double R2 = q * xr * xr + yr * yr / q;
+            if (R2 == 0.0) return;
+            const double R = sqrt(R2), Ra = p[1], Rs = p[2];
+            const double a = 2.0 * p[0] * Ra * Rs / (Rs - Ra) * ((sqrt(Ra * Ra + R2) - Ra) - (sqrt(Rs * Rs + R2) - Rs)) / R;
+            const double axr = a * q * xr / R, ayr = a * yr / (q * R);
+            ax += c * axr - sn * ayr;
+            ay += sn * axr + c * ayr;
+            return;
+        }
         case JT_DEFL_MULTIPOLE: {                              // reading Q36: psi = r a_m/(1 - m^2) cos(m (phi - phi_m)), m >= 2
             const double dx = x - p[3], dy = y - p[4], m = p[0];
             if (dx == 0.0 && dy == 0.0) return;

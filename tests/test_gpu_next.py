@@ -176,7 +176,8 @@ def test_ray_shoot_profiles_nie_epl(jt, orc, dtype):
             ("EPL", [0.6, 2.3, 0.0, 0.0, 0.1, 1.4]), ("SHEAR", [0.03, -0.02]), ("SIS", [0.2, 1.5, -1.5]),
             ("MULTIPOLE", [3.0, 0.04, 0.2, -0.2, 0.3]), ("MULTIPOLE", [4.0, -0.03, 1.1, -0.2, 0.3]),
             ("MULTIPOLE", [2.0, 0.02, -0.4, 0.3, -0.1]),                # centred on ray 0
-            ("CSE", [0.05, 0.2, 0.3, -0.15, 0.5, 0.5]), ("CSE", [0.02, 0.05, 0.0, 0.0, -1.0, -0.4])]
+            ("CSE", [0.05, 0.2, 0.3, -0.15, 0.5, 0.5]), ("CSE", [0.02, 0.05, 0.0, 0.0, -1.0, -0.4]),
+            ("PJAFFE_ELLIPSE_POTENTIAL", [0.3, 0.1, 0.8, 0.25, -0.2, 0.9, 0.1])]
     if dtype == "f32":
         tx, ty = _f32r(tx), _f32r(ty)
     bx, by = jt.ray_shoot_profiles(to_dev(tx, dtype), to_dev(ty, dtype), defl)
