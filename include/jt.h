@@ -103,6 +103,33 @@ JT_API jt_status jt_ray_shoot(jt_dtype dtype, int64_t n_rays, const void *theta_
                        const jt_lens *lens, void *workspace, size_t workspace_bytes,
                        void *beta_x, void *beta_y, void *stream);
 
+/* jt_ray_shoot for callers that cannot supply a workspace because they cannot allocate device memory where they call
+ * this library: a callback inside a host framework that passes finished input / output buffers and forbids allocation
+ * (an XLA / JAX custom call, a serving-runtime plug-in, a fixed-budget acquisition loop), or a process whose memory
+ * pool already owns the device so that a cudaMalloc beside it fails, fragments or stalls every stream.  Same operation,
+ * same kernels and same results as jt_ray_shoot; the scratch is a fixed array of JT_NOALLOC_SCRATCH_BYTES that is part
+ * of the library image, so EVERY GPU on which the process uses libjt holds that much memory from the moment the
+ * library's code is loaded there until the process exits, called or not.  The entry point and everything below it call
+ * no cudaMalloc / cudaFree and no allocating library routine.
+ *   - Limit: the call is accepted iff jt_ray_shoot_workspace_bytes(dtype, n_rays, n_tnfw) <= JT_NOALLOC_SCRATCH_BYTES
+ *     (also returned by jt_ray_shoot_noalloc_capacity()); otherwise JT_ERR_WORKSPACE, nothing is enqueued and the
+ *     outputs are untouched.  The derived records cost 224 bytes (JT_F64) / 96 bytes (JT_F32) per subhalo, and a subhalo
+ *     list that is split over thread blocks adds 16 bytes per ray and chunk: BASELINE.json config 2 as a ray list
+ *     (160,000 rays, 10,000 subhalos: 30.5 MB in JT_F64, 29.4 MB in JT_F32) fits, the same rays through 50,000 subhalos
+ *     (49.8 MB in JT_F64) do not.  Ask the query rather than guessing.
+ *   - First call on each device: looks up the array's device address (cudaGetSymbolAddress, with that device current;
+ *     a failure is reported as JT_ERR_CUDA).  Make that first call outside any stream capture; later calls on the same
+ *     device do no set-up.
+ *   - All calls on a device share the one array.  Nothing needs to be cleared by the caller (each call rewrites what
+ *     it reads and zeroes its own counters first), but two calls whose kernels can overlap on the GPU -- different
+ *     streams without an ordering between them, or host threads on different streams -- race on it and both results
+ *     are garbage.  Keep calls on one stream, or order them with events.  jt_ray_shoot has no such restriction.
+ * theta_x, theta_y: device [n_rays] (in); beta_x, beta_y: device [n_rays] (out); lens as for jt_ray_shoot. */
+#define JT_NOALLOC_SCRATCH_BYTES (32u << 20)     /* 32 MiB per GPU */
+JT_API size_t    jt_ray_shoot_noalloc_capacity(void);
+JT_API jt_status jt_ray_shoot_noalloc(jt_dtype dtype, int64_t n_rays, const void *theta_x, const void *theta_y,
+                               const jt_lens *lens, void *beta_x, void *beta_y, void *stream);
+
 /* Step 2 ("surface brightness of the source is calculated on the ray-traced grid"):
  * flux[i] = sum_k Sersic_k(beta_x[i], beta_y[i]) -- surface brightness, no pixel-area factor.
  * beta_x, beta_y: device [n] (in).  flux: device [n] (out). */

@@ -31,6 +31,8 @@ from .binding import (  # noqa: F401
     psf_convolve_batch_workspace_bytes,
     psf_convolve_workspace_bytes,
     ray_shoot,
+    ray_shoot_noalloc,
+    ray_shoot_noalloc_capacity,
     ray_shoot_workspace_bytes,
     simulate_batch,
     simulate_image,

@@ -89,6 +89,9 @@ def lib():
         L.jt_ray_shoot_workspace_bytes.restype = sz
         L.jt_ray_shoot_workspace_bytes.argtypes = [ctypes.c_int, i64, i64]
         L.jt_ray_shoot.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Lens), vp, sz, vp, vp, vp]
+        L.jt_ray_shoot_noalloc_capacity.restype = sz
+        L.jt_ray_shoot_noalloc_capacity.argtypes = []
+        L.jt_ray_shoot_noalloc.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Lens), vp, vp, vp]
         L.jt_source_brightness.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Sources), vp, vp]
         L.jt_psf_convolve_workspace_bytes.restype = sz
         L.jt_psf_convolve_workspace_bytes.argtypes = [ctypes.c_int, i32, i32, i32, i32, ctypes.c_int]
@@ -286,6 +289,34 @@ def ray_shoot(theta_x, theta_y, sie=None, shear=None, tnfw=None, workspace=None,
     _check(lib().jt_ray_shoot(code, n, _ptr(theta_x), _ptr(theta_y), ctypes.byref(L), _ptr(ws), wsb,
                               _ptr(bx), _ptr(by), _stream(stream)), "jt_ray_shoot")
     return bx, by
+
+
+def ray_shoot_noalloc_capacity():
+    """Bytes of the library's built-in scratch array (JT_NOALLOC_SCRATCH_BYTES, held on every GPU that uses libjt)."""
+    return int(lib().jt_ray_shoot_noalloc_capacity())
+
+
+def ray_shoot_noalloc(theta_x, theta_y, beta_x, beta_y, sie=None, shear=None, tnfw=None, stream=None):
+    """jt_ray_shoot_noalloc: jt_ray_shoot without a workspace, for code that may not allocate device memory where it calls
+    us (a framework callback that only receives its input / output buffers, a process whose memory pool already owns the
+    GPU).  Nothing is allocated here either: the caller passes the outputs beta_x, beta_y (same shape and dtype as theta),
+    and the scratch is a fixed 32 MiB array inside libjt.  Problems whose ray_shoot_workspace_bytes exceeds
+    ray_shoot_noalloc_capacity() are refused.  All calls on a GPU share that array: keep them on one stream (calls that
+    overlap on the GPU corrupt each other), and make the first call on a device outside stream capture."""
+    for t, name in ((theta_x, "theta_x"), (theta_y, "theta_y"), (beta_x, "beta_x"), (beta_y, "beta_y")):
+        _dev(t, name)
+    code = _dt(theta_x)
+    n = theta_x.numel()
+    if _dt(beta_x) != code or _dt(beta_y) != code or _dt(theta_y) != code or beta_x.numel() != n or beta_y.numel() != n:
+        raise TypeError("beta_x, beta_y must match theta_x, theta_y in dtype and size")
+    L = _lens(code, sie, shear, tnfw)
+    need = ray_shoot_workspace_bytes(code, n, L.n_tnfw)
+    if need > ray_shoot_noalloc_capacity():
+        raise JtError(3, "jt_ray_shoot_noalloc (%d rays x %d subhalos need %d bytes of scratch, the built-in array holds %d)"
+                      % (n, L.n_tnfw, need, ray_shoot_noalloc_capacity()))
+    _check(lib().jt_ray_shoot_noalloc(code, n, _ptr(theta_x), _ptr(theta_y), ctypes.byref(L), _ptr(beta_x), _ptr(beta_y),
+                                      _stream(stream)), "jt_ray_shoot_noalloc")
+    return beta_x, beta_y
 
 
 def source_brightness(beta_x, beta_y, sources, stream=None):

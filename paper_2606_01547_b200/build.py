@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libjt.so")
 PROBE_LIB = os.path.join(HERE, "libjtprobe.so")
-SOURCES = ["jt_api.cu", "jt_trace.cu", "jt_trace_f32.cu", "jt_trace_f64.cu", "jt_conv.cu", "jt_fft.cu", "jt_batch.cu", "jt_next.cu"]
+SOURCES = ["jt_api.cu", "jt_trace.cu", "jt_trace_f32.cu", "jt_trace_f64.cu", "jt_conv.cu", "jt_fft.cu", "jt_batch.cu", "jt_next.cu", "jt_noalloc.cu"]
 PROBE_SOURCES = ["jt_probe.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

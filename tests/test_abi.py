@@ -98,3 +98,24 @@ def test_no_cpu_fallback_without_device(jt):
     st = L.jt_ray_shoot(1, 4, ctypes.c_void_p(256), ctypes.c_void_p(512), ctypes.byref(lens), None, 0,
                         ctypes.c_void_p(768), ctypes.c_void_p(1024), None)
     assert st in (2, 4)
+
+
+def test_noalloc_entry_point_limit_without_device(jt):
+    """jt_ray_shoot_noalloc (for callers that cannot allocate device memory) refuses, before touching any device, a
+    problem whose scratch does not fit its built-in 32 MiB array, and validates its arguments like jt_ray_shoot."""
+    from paper_2606_01547_b200 import binding as b
+    L = jt.lib()
+    cap = L.jt_ray_shoot_noalloc_capacity()
+    assert cap == 32 << 20
+    dummy = [ctypes.c_void_p(256 * (k + 1)) for k in range(9)]
+    lens = b._Lens()
+    lens.n_tnfw = 50000
+    lens.tnfw_cx, lens.tnfw_cy, lens.tnfw_Rs, lens.tnfw_alpha_Rs, lens.tnfw_r_trunc = [d.value for d in dummy[4:9]]
+    assert L.jt_ray_shoot_workspace_bytes(1, 160000, 50000) > cap
+    assert L.jt_ray_shoot_noalloc(1, 160000, dummy[0], dummy[1], ctypes.byref(lens), dummy[2], dummy[3], None) == 3
+    assert L.jt_ray_shoot_noalloc(7, 10, dummy[0], dummy[1], ctypes.byref(lens), dummy[2], dummy[3], None) == 2
+    assert L.jt_ray_shoot_noalloc(1, -1, dummy[0], dummy[1], ctypes.byref(lens), dummy[2], dummy[3], None) == 1
+    assert L.jt_ray_shoot_noalloc(1, 10, dummy[0], dummy[1], ctypes.byref(lens), dummy[0], dummy[3], None) == 1   # aliasing
+    assert L.jt_ray_shoot_noalloc(1, 0, None, None, ctypes.byref(lens), None, None, None) == 0                     # no-op
+    lens.tnfw_Rs = None
+    assert L.jt_ray_shoot_noalloc(1, 10, dummy[0], dummy[1], ctypes.byref(lens), dummy[2], dummy[3], None) == 1
