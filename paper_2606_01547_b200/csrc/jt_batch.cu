@@ -198,10 +198,10 @@ static size_t batch_smem_front(const BatchArgs<T>& a) {
 #define JT_BATCH_CASE(RR)                                                                              \
     case RR: {                                                                                         \
         auto kern = k_batch<T, RR, kBatchVar>;                                                         \
-        static bool attr_set = false;   /* once per instantiation: allow the full dynamic shared memory */ \
-        if (!attr_set) {                                                                               \
+        static PerDeviceOnce attr;   /* once per instantiation and device: allow the full dynamic shared memory */ \
+        if (attr.needed()) {                                                                           \
             JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBatchMaxSmem)); \
-            attr_set = true;                                                                           \
+            attr.mark();                                                                               \
         }                                                                                              \
         kern<<<(unsigned)B, kBatchThreads, smem, st>>>(a);                                             \
         break;                                                                                         \

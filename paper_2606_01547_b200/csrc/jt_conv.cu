@@ -471,10 +471,10 @@ static bool use_small(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx, Sma
 template <typename T>
 static jt_status conv_small_t(const SmallPlan& p, int ny, int nx, const T* img, int ky, int kx, const T* ker, T* out, cudaStream_t st) {
     auto kern = k_conv_small<T>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceOnce attr;                          // once per instantiation and device
+    if (attr.needed()) {
         JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmallMaxSmem));
-        attr_set = true;
+        attr.mark();
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)((nx + kConvTW - 1) / kConvTW), (unsigned)((ny + kSmallTH - 1) / kSmallTH));
@@ -549,10 +549,10 @@ template <typename T, int OY>
 static jt_status launch_ur(const ConvPlan& p, const CUtensorMap& map, const ConvArgs<T>& a, int64_t B, cudaStream_t st) {
     const int z = p.Z;
     auto kern = k_conv_ur<T, OY>;
-    static bool attr_set = false;                       // once per instantiation: allow the full 227 KB
-    if (!attr_set) {
+    static PerDeviceOnce attr;                          // once per instantiation and device: allow the full 227 KB
+    if (attr.needed()) {
         JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSmemPerSM - 1024)));
-        attr_set = true;
+        attr.mark();
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(p.tiles_y * B), (unsigned)p.tiles_x, (unsigned)z);

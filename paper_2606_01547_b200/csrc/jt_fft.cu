@@ -457,14 +457,14 @@ static jt_status conv_fft_t(FftPlan& p, int64_t B, const T* img, const T* ker, v
     auto k2r = k_fft_cols<true>;
     auto k2k = k_fft_cols_ker;
     auto k3 = k_fft_rows_inv<T>;
-    static bool attr_set = false;                  // once per instantiation: allow the full dynamic shared memory
-    if (!attr_set) {
+    static PerDeviceOnce attr;                     // once per instantiation and device: allow the full dynamic shared memory
+    if (attr.needed()) {
         JT_CUDA_TRY(cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         JT_CUDA_TRY(cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         JT_CUDA_TRY(cudaFuncSetAttribute(k2r, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         JT_CUDA_TRY(cudaFuncSetAttribute(k2k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
         JT_CUDA_TRY(cudaFuncSetAttribute(k3, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFftMaxSmem));
-        attr_set = true;
+        attr.mark();
     }
     const int ker_ctas = p.grid_rows_fwd - a.n_cta_img;
     const size_t img_elems = (size_t)a.ny * a.nx;

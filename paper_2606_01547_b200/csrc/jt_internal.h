@@ -1,6 +1,7 @@
 // jt_internal.h -- host-side plumbing shared by the translation units of libjt (not installed).
 #pragma once
 #include <cuda_runtime.h>
+#include <atomic>
 #include <stddef.h>
 #include <stdint.h>
 #include "../../include/jt.h"
@@ -25,6 +26,22 @@ void count_launch();
         cudaError_t _e = cudaGetLastError();                                 \
         if (_e != cudaSuccess) { jt::set_last_cuda_error((int)_e); return JT_ERR_CUDA; } \
     } while (0)
+
+// "Done once" for set-up that belongs to a DEVICE (cudaFuncSetAttribute acts on the device that is current): one bit per
+// device ordinal, safe against host threads racing (both then do the idempotent set-up).  Devices beyond bit 63 and a
+// failing cudaGetDevice simply repeat the set-up on every call.
+struct PerDeviceOnce {
+    std::atomic<uint64_t> done{0};
+    bool needed() {
+        int d = -1;
+        if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= 64) return true;
+        return (done.load(std::memory_order_acquire) >> d & 1ull) == 0;
+    }
+    void mark() {
+        int d = -1;
+        if (cudaGetDevice(&d) == cudaSuccess && d >= 0 && d < 64) done.fetch_or(1ull << d, std::memory_order_release);
+    }
+};
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 inline size_t dtype_size(jt_dtype d) { return d == JT_F32 ? 4 : 8; }

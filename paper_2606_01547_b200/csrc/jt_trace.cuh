@@ -777,10 +777,10 @@ jt_status launch_trace_t(const TraceArgs<T>& a, int R, cudaStream_t st);
     case RR: {                                                                                    \
         auto kern = k_trace<T, RR, GRID>;                                                         \
         const size_t dsm = trace_smem_bytes<T, RR, TraceCfg<T>::NT>(a.tile_recs);                 \
-        static bool attr_set = false;   /* once per instantiation: allow the full dynamic shared memory */ \
-        if (!attr_set) {                                                                          \
+        static PerDeviceOnce attr;   /* once per instantiation and device: allow the full dynamic shared memory */ \
+        if (attr.needed()) {                                                                      \
             JT_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 1024)); \
-            attr_set = true;                                                                      \
+            attr.mark();                                                                          \
         }                                                                                         \
         cfg.dynamicSmemBytes = dsm;                                                               \
         JT_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, a));                                           \
