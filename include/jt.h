@@ -141,7 +141,8 @@ JT_API jt_status jt_source_brightness(jt_dtype dtype, int64_t n, const void *bet
  * (zero padding, 'same' size, true convolution -- kernel flipped relative to correlation).
  * image: device [ny][nx] (in).  kernel: device [ky][kx], ky and kx odd (in); used as given, never
  * renormalised.  out: device [ny][nx].  method: DIRECT = register-blocked sum over a TMA-loaded shared-memory halo tile,
- * taps fed from the constant bank through uniform registers, kernel rows split over a thread-block cluster; FFT =
+ * taps fed from the constant bank through uniform registers; when the tiles alone cannot fill the SMs, pairs of kernel
+ * columns are dealt to independent thread blocks whose partial images are added through L2 in a fixed order; FFT =
  * zero-pad to P >= n+K-1, hand-written shared-memory FFTs; AUTO picks the path a time model calibrated on B200 expects
  * to be faster.  workspace: device scratch >= jt_psf_convolve_workspace_bytes(...) for the same arguments, 16-byte
  * aligned.  Non-finite pixels may reach outputs up to one pixel beyond the kernel's support (0 x inf).
@@ -236,7 +237,11 @@ JT_API jt_status jt_lensing_maps(jt_dtype dtype, int64_t n, const void *theta_x,
  *   JT_LIGHT_SERSIC_ELLIPSE   (:103)    amp, R_sersic, n_sersic, e1, e2, cx, cy      definition R
  *   JT_LIGHT_GAUSSIAN_ELLIPSE (:98-101) amp (total flux), sigma, e1, e2, cx, cy; GAUSSIAN is e1 = e2 = 0,
  *                                       MULTI_GAUSSIAN(_ELLIPSE) is several records
- * Formulas: DESIGN.md readings Q26-Q30.  Unknown types contribute nothing. */
+ * Formulas: DESIGN.md readings Q26-Q30.  Unknown types contribute nothing (deflector and light lists alike; a
+ * zero-filled light record is type 0 = SERSIC_ELLIPSE, not "unknown").
+ * Parameter domains (NOT checked on the device -- outside them the record yields IEEE inf / NaN, which then poisons every
+ * ray's sum, never a fault): Rs, Ra, R_sersic, n_sersic, sigma, s (CSE) > 0; PJAFFE Ra != Rs; theta_E >= 0; s_scale >= 0;
+ * 1 < gamma < 3; integer m >= 2; |e| < 1 (clamped to 0.9999 like everywhere else). */
 typedef enum { JT_DEFL_CONVERGENCE = 0, JT_DEFL_SIS = 1, JT_DEFL_NFW = 2, JT_DEFL_HERNQUIST = 3, JT_DEFL_PJAFFE = 4,
                JT_DEFL_SIE = 5, JT_DEFL_SHEAR = 6, JT_DEFL_TNFW = 7, JT_DEFL_NIE = 8, JT_DEFL_EPL = 9,
                JT_DEFL_MULTIPOLE = 10, JT_DEFL_CSE = 11,

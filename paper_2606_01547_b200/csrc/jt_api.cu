@@ -139,6 +139,7 @@ static jt_status psf_convolve_impl(jt_dtype dtype, int64_t B, int32_t ny, int32_
         return JT_ERR_UNSUPPORTED;
     const size_t need = conv_ws(dtype, B, ny, nx, ky, kx, method);
     if (need > 0 && (!workspace || workspace_bytes < need)) return JT_ERR_WORKSPACE;
+    if (need > 0 && ((uintptr_t)workspace & 15)) return JT_ERR_INVALID_VALUE;    // double2 partial sums, complex planes
     jt_status s = check_device();
     if (s != JT_OK) return s;
     return conv_dispatch(dtype, B, ny, nx, image, ky, kx, kernel, method, workspace, out, (cudaStream_t)stream);

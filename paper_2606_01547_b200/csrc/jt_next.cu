@@ -341,7 +341,8 @@ __device__ __forceinline__ double profile_light(const jt_profile& d, double bx, 
         const double pw = a > 0.0 ? exp(0.5 / p[2] * log(a)) : 0.0;
         return p[0] * exp(-bn * (pw - 1.0));
     }
-    ellipticity(p[2], p[3], &c, &s, &q);                      // JT_LIGHT_GAUSSIAN_ELLIPSE
+    if (d.type != JT_LIGHT_GAUSSIAN_ELLIPSE) return 0.0;      // unknown types contribute nothing (jt.h)
+    ellipticity(p[2], p[3], &c, &s, &q);
     const double dx = bx - p[4], dy = by - p[5];
     const double xr = c * dx + s * dy, yr = -s * dx + c * dy;
     const double i2s = 0.5 / (p[1] * p[1]);

@@ -71,6 +71,12 @@ def test_argument_validation_without_device(jt):
     assert need >= (64 + 64 + 21) * (84 // 2 + 1) * 16        # three half-spectrum planes of the 84 x 84 padded transform
     assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 2, dummy, need - 1, ctypes.c_void_p(512), None) == 3
     assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, 2, None, 0, ctypes.c_void_p(512), None) == 3
+    # a workspace that is only 8-byte aligned is refused by both methods (double2 / complex accesses would fault)
+    for m in (1, 2):
+        need = L.jt_psf_convolve_workspace_bytes(1, 64, 64, 21, 21, m)
+        assert L.jt_psf_convolve(1, 64, 64, dummy, 21, 21, dummy, m, ctypes.c_void_p(4096 + 8), need, ctypes.c_void_p(512), None) == 1
+        assert L.jt_psf_convolve_batch(1, ctypes.c_int64(1), 64, 64, dummy, 21, 21, dummy, m, ctypes.c_void_p(4096 + 8), need,
+                                       ctypes.c_void_p(512), None) == 1
     # zero-sized problems are no-ops
     assert L.jt_ray_shoot(1, 0, None, None, ctypes.byref(lens), None, 0, None, None, None) == 0
     del keep
