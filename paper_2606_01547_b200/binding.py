@@ -4,6 +4,8 @@ Tensors are torch CUDA tensors (float32 -> JT_F32, float64 -> JT_F64), contiguou
 torch stream is passed through.  Names and argument meaning follow include/jt.h one to one.
 """
 import ctypes
+import functools
+import inspect
 import os
 from dataclasses import dataclass
 
@@ -227,6 +229,25 @@ def _stream(stream):
     return ctypes.c_void_p(s.cuda_stream)
 
 
+def _on_stream(fn):
+    """Decorator of the wrappers that take `stream`: when a stream other than torch's current one is given, the wrapper
+    body runs with that stream current, so every tensor it creates -- outputs, scratch workspace, uploaded profile
+    records -- is allocated from, filled on and later recycled in order with the stream the kernels run on.  (Created on
+    the current stream instead, an upload could still be in flight when the kernel starts, and the caching allocator
+    could hand a temporary to someone else while the kernel still reads it.)  Inputs the caller made on another stream
+    remain the caller's to order, as with any torch op on a side stream."""
+    idx = list(inspect.signature(fn).parameters).index("stream")
+
+    @functools.wraps(fn)
+    def wrapper(*args, **kw):
+        stream = kw["stream"] if "stream" in kw else (args[idx] if len(args) > idx else None)
+        if stream is None or stream == torch.cuda.current_stream(stream.device):
+            return fn(*args, **kw)
+        with torch.cuda.stream(stream):
+            return fn(*args, **kw)
+    return wrapper
+
+
 def _check(status, where):
     if status != 0:
         raise JtError(status, where)
@@ -278,6 +299,7 @@ def ray_shoot_workspace_bytes(dtype, n_rays, n_tnfw):
     return int(lib().jt_ray_shoot_workspace_bytes(_code(dtype), n_rays, n_tnfw))
 
 
+@_on_stream
 def ray_shoot(theta_x, theta_y, sie=None, shear=None, tnfw=None, workspace=None, stream=None):
     """jt_ray_shoot: beta = theta - alpha(theta).  Returns (beta_x, beta_y)."""
     _dev(theta_x, "theta_x"), _dev(theta_y, "theta_y")
@@ -296,6 +318,7 @@ def ray_shoot_noalloc_capacity():
     return int(lib().jt_ray_shoot_noalloc_capacity())
 
 
+@_on_stream
 def ray_shoot_noalloc(theta_x, theta_y, beta_x, beta_y, sie=None, shear=None, tnfw=None, stream=None):
     """jt_ray_shoot_noalloc: jt_ray_shoot without a workspace, for code that may not allocate device memory where it calls
     us (a framework callback that only receives its input / output buffers, a process whose memory pool already owns the
@@ -319,6 +342,7 @@ def ray_shoot_noalloc(theta_x, theta_y, beta_x, beta_y, sie=None, shear=None, tn
     return beta_x, beta_y
 
 
+@_on_stream
 def source_brightness(beta_x, beta_y, sources, stream=None):
     """jt_source_brightness: sum of elliptical Sersic components at (beta_x, beta_y)."""
     _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y")
@@ -335,6 +359,7 @@ def psf_convolve_workspace_bytes(dtype, ny, nx, ky, kx, method="auto"):
     return int(lib().jt_psf_convolve_workspace_bytes(_code(dtype), ny, nx, ky, kx, _METHODS[method]))
 
 
+@_on_stream
 def psf_convolve(image, kernel, method="auto", workspace=None, out=None, stream=None):
     """jt_psf_convolve: zero-padded 'same' true convolution of image [ny][nx] with kernel [ky][kx]."""
     _dev(image, "image"), _dev(kernel, "kernel")
@@ -355,6 +380,7 @@ def psf_convolve_batch_workspace_bytes(dtype, B, ny, nx, ky, kx, method="auto"):
     return int(lib().jt_psf_convolve_batch_workspace_bytes(_code(dtype), B, ny, nx, ky, kx, _METHODS[method]))
 
 
+@_on_stream
 def psf_convolve_batch(images, kernel, method="auto", workspace=None, out=None, stream=None):
     """jt_psf_convolve_batch: images [B][ny][nx], one kernel [ky][kx] for all of them."""
     _dev(images, "images"), _dev(kernel, "kernel")
@@ -377,6 +403,7 @@ def simulate_image_workspace_bytes(dtype, grid, n_tnfw, ky, kx, method="auto"):
     return int(lib().jt_simulate_image_workspace_bytes(_code(dtype), ctypes.byref(g), n_tnfw, ky, kx, _METHODS[method]))
 
 
+@_on_stream
 def simulate_image(grid, sie, shear, tnfw, sources, psf, dtype=None, method="auto", workspace=None, out=None,
                    stream=None, device="cuda"):
     """jt_simulate_image: grid -> ray-shoot -> Sersic -> bin -> PSF convolution.  psf=None skips the convolution."""
@@ -421,6 +448,7 @@ def _batch_struct(sie, shear, tnfw, sersic, psf):
     return code, P
 
 
+@_on_stream
 def simulate_batch(grid, sie, shear, tnfw, sersic, psf, out=None, stream=None):
     """jt_simulate_batch: B independent systems.  sie [B][5], shear [B][2], tnfw [B][5][M], sersic [B][n][7], psf [B][ky][kx]."""
     code, P = _batch_struct(sie, shear, tnfw, sersic, psf)
@@ -434,6 +462,7 @@ def simulate_batch(grid, sie, shear, tnfw, sersic, psf, out=None, stream=None):
 
 
 # ------------------------------------------------------------------ SURVEY section 8(f) rows
+@_on_stream
 def chi2_batch(models, data, sigma, out=None, stream=None):
     """jt_chi2_batch: chi2[b] = sum ((models[b] - data) / sigma)^2 as a float64 tensor [B]."""
     _dev(models, "models"), _dev(data, "data"), _dev(sigma, "sigma")
@@ -447,6 +476,7 @@ def chi2_batch(models, data, sigma, out=None, stream=None):
     return out
 
 
+@_on_stream
 def simulate_batch_chi2(grid, sie, shear, tnfw, sersic, psf, data, sigma, images=False, chi2=None, stream=None):
     """jt_simulate_batch_chi2: the batch kernel with the chi^2 against (data, sigma) accumulated in the same thread block.
     Returns chi2 [B] (float64), or (chi2, images) with images=True / an images tensor."""
@@ -468,6 +498,7 @@ def simulate_batch_chi2(grid, sie, shear, tnfw, sersic, psf, data, sigma, images
     return chi2 if img is None else (chi2, img)
 
 
+@_on_stream
 def lensing_maps(theta_x, theta_y, sie=None, shear=None, tnfw=None, stream=None):
     """jt_lensing_maps: (kappa, gamma1, gamma2, mu) of SIE + shear + TNFW at the given points."""
     _dev(theta_x, "theta_x"), _dev(theta_y, "theta_y")
@@ -494,6 +525,7 @@ def profile_records(records, table, device="cuda"):
     return torch.as_tensor(a.view(np.uint8).reshape(-1).copy(), device=device)
 
 
+@_on_stream
 def ray_shoot_profiles(theta_x, theta_y, deflectors, stream=None):
     """jt_ray_shoot_profiles: beta = theta - sum of typed deflectors [(name, params), ...] (or a profile_records tensor)."""
     _dev(theta_x, "theta_x"), _dev(theta_y, "theta_y")
@@ -506,6 +538,7 @@ def ray_shoot_profiles(theta_x, theta_y, deflectors, stream=None):
     return bx, by
 
 
+@_on_stream
 def light_profiles(beta_x, beta_y, components, stream=None):
     """jt_light_profiles: sum of typed light components [(name, params), ...] at (beta_x, beta_y)."""
     _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y")
@@ -517,6 +550,7 @@ def light_profiles(beta_x, beta_y, components, stream=None):
     return flux
 
 
+@_on_stream
 def light_core_sersic(beta_x, beta_y, params, stream=None):
     """jt_light_core_sersic: params = (amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2, cx, cy)."""
     _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y")
@@ -527,6 +561,7 @@ def light_core_sersic(beta_x, beta_y, params, stream=None):
     return flux
 
 
+@_on_stream
 def light_shapelets(beta_x, beta_y, n_max, beta, cx, cy, coef, stream=None):
     """jt_light_shapelets: coef is a device tensor [(n_max+1)(n_max+2)/2] of the call's dtype (N ascending, n2 = 0..N)."""
     _dev(beta_x, "beta_x"), _dev(beta_y, "beta_y"), _dev(coef, "coef")
@@ -538,6 +573,7 @@ def light_shapelets(beta_x, beta_y, n_max, beta, cx, cy, coef, stream=None):
     return flux
 
 
+@_on_stream
 def simulate_image_supersampled_psf(grid, sie, shear, tnfw, sources, psf_fine, dtype=None, method="auto", workspace=None, out=None,
                                     stream=None):
     """jt_simulate_image_supersampled_psf (NEXT-4): psf_fine is sampled on the RAY grid [ky][kx]."""

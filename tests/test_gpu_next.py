@@ -160,6 +160,24 @@ def test_light_profiles(jt, orc, dtype):
     assert float((a - b).abs().max()) < 1e-12 * float(a.abs().max())
 
 
+def test_unknown_profile_types_contribute_nothing(jt):
+    """include/jt.h: "Unknown types contribute nothing" -- a record of a type the library does not know (its parameters
+    all zero, so a Gaussian reading of it would be 0/0) must leave the light sum and the deflection untouched."""
+    import torch
+    from paper_2606_01547_b200 import binding as b
+    rng = np.random.default_rng(47)
+    x, y = to_dev(rng.uniform(-1, 1, 3000), "f64"), to_dev(rng.uniform(-1, 1, 3000), "f64")
+    ser = [("SERSIC_ELLIPSE", [10.0, 0.2, 1.5, 0.05, 0.02, 0.05, 0.0])]
+    light = dict(b.LIGHT_TYPES, UNKNOWN=99, NEGATIVE=-3)
+    recs = b.profile_records(ser + [("UNKNOWN", []), ("NEGATIVE", [])], light)
+    assert torch.equal(jt.light_profiles(x, y, recs), jt.light_profiles(x, y, ser))
+    sis = [("SIS", [1.0, 0.01, -0.02])]
+    defl = dict(b.DEFLECTOR_TYPES, UNKNOWN=99)
+    a = jt.ray_shoot_profiles(x, y, b.profile_records(sis + [("UNKNOWN", [])], defl))
+    w = jt.ray_shoot_profiles(x, y, sis)
+    assert torch.equal(a[0], w[0]) and torch.equal(a[1], w[1])
+
+
 # ------------------------------------------------------------------ NEXT-1, second set
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_ray_shoot_profiles_nie_epl(jt, orc, dtype):
@@ -229,3 +247,29 @@ def test_simulate_image_supersampled_psf(jt, orc, dtype, s, method):
     got = jt.simulate_image_supersampled_psf(g, w.sie, w.shear, to_dev(w.tnfw, dtype), w.sources, to_dev(kf, dtype), dtype=dtype,
                                              method=method).double().cpu().numpy()
     assert rel_err(got, want) < (1e-10 if dtype == "f64" else 2e-4)
+
+
+def test_wrappers_on_a_side_stream(jt):
+    """A caller-chosen stream that is not torch's current one: the binding uploads the profile records and allocates its
+    outputs and scratch on THAT stream, so the result equals the default-stream result (no upload still in flight when
+    the kernel starts, no temporary recycled under it).  Repeated, with allocator churn on the default stream between."""
+    import torch
+    rng = np.random.default_rng(53)
+    x, y = to_dev(rng.uniform(-1, 1, 50000), "f64"), to_dev(rng.uniform(-1, 1, 50000), "f64")
+    comps = [("GAUSSIAN_ELLIPSE", [1.0, 0.1 + 0.01 * k, 0.0, 0.0, 0.02 * k - 0.7, 0.1]) for k in range(70)]
+    defl = [("SIS", [1.0, 0.01, -0.02]), ("NFW", [0.3, 0.2, -0.1, 0.1]), ("SHEAR", [0.03, -0.02])]
+    tn = to_dev(np.array([[0.3], [0.2], [0.05], [0.01], [0.25]]) * np.ones((1, 3000)), "f64")
+    want_l, want_d = jt.light_profiles(x, y, comps), jt.ray_shoot_profiles(x, y, defl)
+    want_r = jt.ray_shoot(x[:2000], y[:2000], (1.0, 0.1, 0.0, 0.0, 0.0), None, tn)        # split list: scratch workspace
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    for _ in range(5):
+        got_l = jt.light_profiles(x, y, comps, stream=side)
+        got_d = jt.ray_shoot_profiles(x, y, defl, stream=side)
+        got_r = jt.ray_shoot(x[:2000], y[:2000], (1.0, 0.1, 0.0, 0.0, 0.0), None, tn, stream=side)
+        junk = [torch.full((50000,), float("nan"), dtype=torch.float64, device="cuda") for _ in range(8)]   # default stream
+        del junk
+        side.synchronize()
+        assert torch.equal(got_l, want_l)
+        assert torch.equal(got_d[0], want_d[0]) and torch.equal(got_d[1], want_d[1])
+        assert torch.equal(got_r[0], want_r[0]) and torch.equal(got_r[1], want_r[1])
