@@ -230,14 +230,18 @@ JT_API jt_status jt_lensing_maps(jt_dtype dtype, int64_t n, const void *theta_x,
  *   JT_DEFL_TNFW        (:87)           Rs, alpha_Rs, r_trunc, cx, cy definition T
  *   JT_DEFL_NIE         (:80)           theta_E, e1, e2, s_scale, cx, cy   definition S with a core (reading Q31)
  *   JT_DEFL_EPL         (:66-70)        theta_E, gamma, e1, e2, cx, cy     elliptical power law, 1 < gamma < 3 (Q32)
- *   JT_DEFL_MULTIPOLE   (:76)           m, a_m, phi_m, cx, cy              multipole of integer order m >= 2 (Q36)
- *   JT_DEFL_CSE         (:65)           A, s, e1, e2, cx, cy               cored steep ellipsoid, s > 0 (Q37)
+ *   JT_DEFL_MULTIPOLE   (:78)           m, a_m, phi_m, cx, cy              multipole of integer order m >= 2 (Q36)
+ *   JT_DEFL_CSE         (:66)           A, s, e1, e2, cx, cy               cored steep ellipsoid, s > 0 (Q37)
  *   JT_DEFL_PJAFFE_ELLIPSE_POTENTIAL (:84)  sigma0, Ra, Rs, e1, e2, cx, cy     PJAFFE potential made elliptical (Q38)
  *   light
  *   JT_LIGHT_SERSIC_ELLIPSE   (:103)    amp, R_sersic, n_sersic, e1, e2, cx, cy      definition R
  *   JT_LIGHT_GAUSSIAN_ELLIPSE (:98-101) amp (total flux), sigma, e1, e2, cx, cy; GAUSSIAN is e1 = e2 = 0,
  *                                       MULTI_GAUSSIAN(_ELLIPSE) is several records
- * Formulas: DESIGN.md readings Q26-Q30.  Unknown types contribute nothing (deflector and light lists alike; a
+ * NIE (s_scale > 0), CSE and PJAFFE_ELLIPSE_POTENTIAL with q != 1: how the core / scale radii are spread over the two axes
+ * is THIS library's reading (Q31, Q37, Q38) and may differ from the lenstronomy / JAXtronomy profile of the same name --
+ * upstream could not be consulted; parity with upstream is unpinned for them.  DESIGN.md section 3 ("Conventions for
+ * q != 1") gives the remembered differences and the parameter mapping.  At q = 1 there is no difference.
+ * Formulas: DESIGN.md readings Q26-Q38.  Unknown types contribute nothing (deflector and light lists alike; a
  * zero-filled light record is type 0 = SERSIC_ELLIPSE, not "unknown").
  * Parameter domains (NOT checked on the device -- outside them the record yields IEEE inf / NaN, which then poisons every
  * ray's sum, never a fault): Rs, Ra, R_sersic, n_sersic, sigma, s (CSE) > 0; PJAFFE Ra != Rs; theta_E >= 0; s_scale >= 0;
@@ -255,7 +259,7 @@ JT_API jt_status jt_ray_shoot_profiles(jt_dtype dtype, int64_t n, const void *th
 JT_API jt_status jt_light_profiles(jt_dtype dtype, int64_t n, const void *beta_x, const void *beta_y, int64_t n_comp,
                             const jt_profile *components, void *flux, void *stream);
 
-/* CORE_SERSIC (PAPER.md:102; reading Q33): params (HOST, 10 doubles) = amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2,
+/* CORE_SERSIC (PAPER.md:97; reading Q33): params (HOST, 10 doubles) = amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2,
  * cx, cy;  I = amp (1 + (Rb/R)^alpha)^(gamma/alpha) exp(-b_n [((R^alpha + Rb^alpha)/R_sersic^alpha)^(1/(alpha n)) - 1]),
  * R the product-averaged radius of definition R.  beta_x, beta_y, flux: device [n]. */
 JT_API jt_status jt_light_core_sersic(jt_dtype dtype, int64_t n, const void *beta_x, const void *beta_y, const double *params,

@@ -310,7 +310,7 @@ double orc_epl_kappa(double x, double y, const double *p) {
     return 0.5 * (3.0 - p[1]) * pow(p[0] / sqrt(q * xr * xr + yr * yr / q), p[1] - 1.0);
 }
 
-/*  10 MULTIPOLE (PAPER.md:76)  p = {m, a_m, phi_m, cx, cy}, integer m >= 2 (reading Q36): the potential
+/*  10 MULTIPOLE (PAPER.md:78)  p = {m, a_m, phi_m, cx, cy}, integer m >= 2 (reading Q36): the potential
  *        psi = r a_m/(1 - m^2) cos(m (phi - phi_m)), whose Laplacian gives kappa = a_m cos(m (phi - phi_m))/(2 r);
  *        alpha_r = dpsi/dr = a_m/(1 - m^2) cos(m (phi - phi_m)), alpha_phi = (1/r) dpsi/dphi = -m a_m/(1 - m^2) sin(m (phi - phi_m)),
  *        (alpha_x, alpha_y) = (alpha_r cos phi - alpha_phi sin phi, alpha_r sin phi + alpha_phi cos phi); alpha(0) = 0. */
@@ -333,7 +333,7 @@ double orc_multipole_kappa(double x, double y, const double *p) {
     return 0.5 * p[1] * cos(p[0] * (atan2(dy, dx) - p[2])) / sqrt(dx * dx + dy * dy);
 }
 
-/*  11 CSE (PAPER.md:65, cored steep ellipsoid; reading Q37)  p = {A, s, e1, e2, cx, cy}
+/*  11 CSE (PAPER.md:66, cored steep ellipsoid; reading Q37)  p = {A, s, e1, e2, cx, cy}
  *        kappa = A / (2 (s^2 + x'^2 + y'^2/q^2)^(3/2))  (Oguri 2021: the major axis along x', NOT the product-averaged
  *        radius of definitions S and R), deflection in the lens frame with psi = sqrt(q^2 (s^2 + x'^2) + y'^2):
  *          a'x = A q x' (psi + q^2 s) / (s psi [(psi + s)^2 + (1 - q^2) x'^2]),
@@ -444,7 +444,7 @@ void orc_ray_shoot_profiles2(int64_t n, const double *tx, const double *ty, int6
     }
 }
 
-/*   light 2 CORE_SERSIC  p = {amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2}, centre passed apart
+/*   light 2 CORE_SERSIC   p = {amp, R_sersic, n_sersic, Rb, gamma, alpha, e1, e2}, centre passed apart
  *        (eight parameters fill the record): with R the product-averaged radius of definition R about (cx, cy),
  *          I = amp (1 + (Rb/R)^alpha)^(gamma/alpha) exp(-b_n [ ((R^alpha + Rb^alpha)/R_sersic^alpha)^(1/(alpha n)) - 1 ])
  *        (Graham et al. 2003 / Trujillo et al. 2004 core-Sersic with b_n of reading Q10): Rb -> 0 IS definition R; the
