@@ -282,6 +282,37 @@ JT_API jt_status jt_simulate_image_supersampled_psf(jt_dtype dtype, const jt_gri
                                              jt_conv_method method, void *workspace, size_t workspace_bytes, void *out,
                                              void *stream);
 
+/* Read-only launch plans (host only: no device is touched, nothing is enqueued).  The library picks among several launch
+ * shapes per call from time models; these queries say which one a call with the same arguments takes, so that a test can
+ * assert the path it is named after and a user can see what AUTO resolves to.
+ * jt_psf_convolve_plan: `image` may be NULL (then its address is taken to be 16-byte aligned).
+ *   method    JT_CONV_DIRECT / JT_CONV_FFT -- what the call runs (AUTO resolved)
+ *   path      JT_PATH_CONV_SMALL  one launch, taps + halo tile staged by the CTA (tiny kernels on small single images)
+ *             JT_PATH_CONV_TILE   tap kernel + constant-bank sweep kernel (k_conv_ur); then: tma = 1 halo tile by TMA,
+ *                                 0 plain loads (image address or row pitch not 16-byte aligned, tile side > 256);
+ *                                 z_split > 1 = kernel-column pairs dealt to z_split CTAs per tile, partial images added
+ *                                 through L2; row_bands > 1 = the 60 KB constant bank holds only a band of kernel rows,
+ *                                 one sweep launch per band
+ *             JT_PATH_CONV_FFT    hand-written FFT (pad_y x pad_x padded transform)
+ *   oy, warps rows per thread and warps per CTA of the tile kernel; est_us the time model's estimate. */
+typedef enum { JT_PATH_CONV_SMALL = 0, JT_PATH_CONV_TILE = 1, JT_PATH_CONV_FFT = 2 } jt_conv_path;
+typedef struct {
+    int32_t method, path, tma, z_split, row_bands, oy, warps, pad_y, pad_x, reserved;
+    double  est_us;
+} jt_conv_plan;
+JT_API jt_status jt_psf_convolve_plan(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, int32_t ky, int32_t kx,
+                               jt_conv_method method, const void *image, jt_conv_plan *plan);
+/* Ray-tracing kernel (k_trace) of jt_simulate_image (grid != NULL) or jt_ray_shoot (grid == NULL, n_rays used):
+ *   rays_per_thread  R (grid mode: R = s means one pixel row per thread, the launch-latency shape for next to no subhalos)
+ *   threads          per CTA;  wide = 1: CTA-wide ray tiles binned through shared memory (s does not divide 32)
+ *   n_chunks         > 1: the subhalo list is split over CTAs, partial sums meet in the workspace;  chunk_len subhalos each
+ *   n_ctas           ray tiles x chunks;  tile_recs = subhalo records per shared-memory stage of the TMA ring */
+typedef struct {
+    int32_t rays_per_thread, threads, wide, n_chunks, tile_recs, reserved;
+    int64_t chunk_len, n_ctas;
+} jt_trace_plan;
+JT_API jt_status jt_trace_plan_query(jt_dtype dtype, const jt_grid *grid, int64_t n_rays, int64_t n_tnfw, jt_trace_plan *plan);
+
 /* Measurement aid (bench.py's roofline leg).  jt_profile_enable(1) makes every following
  * jt_simulate_image call on this host thread record CUDA events on its stream before the ray-tracing kernel, between it
  * and the convolution, and after the convolution, and copy the kernel's JT_N_TIERS tier counters (48 bytes) to a pinned host

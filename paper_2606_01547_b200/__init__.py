@@ -27,6 +27,8 @@ from .binding import (  # noqa: F401
     profile_read,
     profile_tiers,
     psf_convolve,
+    psf_convolve_plan,
+    trace_plan,
     psf_convolve_batch,
     psf_convolve_batch_workspace_bytes,
     psf_convolve_workspace_bytes,

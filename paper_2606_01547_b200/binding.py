@@ -51,6 +51,16 @@ class _Sources(ctypes.Structure):
                 ("e2", _dp), ("cx", _dp), ("cy", _dp)]
 
 
+class _ConvPlan(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("method", "path", "tma", "z_split", "row_bands", "oy", "warps", "pad_y", "pad_x",
+                                               "reserved")] + [("est_us", ctypes.c_double)]
+
+
+class _TracePlan(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_int32) for n in ("rays_per_thread", "threads", "wide", "n_chunks", "tile_recs", "reserved")] + \
+               [("chunk_len", ctypes.c_int64), ("n_ctas", ctypes.c_int64)]
+
+
 class _Batch(ctypes.Structure):
     _fields_ = [("sie", ctypes.c_void_p), ("shear", ctypes.c_void_p), ("n_tnfw", ctypes.c_int32),
                 ("tnfw", ctypes.c_void_p), ("n_src", ctypes.c_int32), ("sersic", ctypes.c_void_p),
@@ -94,6 +104,8 @@ def lib():
         L.jt_ray_shoot_noalloc_capacity.restype = sz
         L.jt_ray_shoot_noalloc_capacity.argtypes = []
         L.jt_ray_shoot_noalloc.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Lens), vp, vp, vp]
+        L.jt_psf_convolve_plan.argtypes = [ctypes.c_int, i64, i32, i32, i32, i32, ctypes.c_int, vp, ctypes.POINTER(_ConvPlan)]
+        L.jt_trace_plan_query.argtypes = [ctypes.c_int, ctypes.POINTER(_Grid), i64, i64, ctypes.POINTER(_TracePlan)]
         L.jt_source_brightness.argtypes = [ctypes.c_int, i64, vp, vp, ctypes.POINTER(_Sources), vp, vp]
         L.jt_psf_convolve_workspace_bytes.restype = sz
         L.jt_psf_convolve_workspace_bytes.argtypes = [ctypes.c_int, i32, i32, i32, i32, ctypes.c_int]
@@ -340,6 +352,31 @@ def ray_shoot_noalloc(theta_x, theta_y, beta_x, beta_y, sie=None, shear=None, tn
     _check(lib().jt_ray_shoot_noalloc(code, n, _ptr(theta_x), _ptr(theta_y), ctypes.byref(L), _ptr(beta_x), _ptr(beta_y),
                                       _stream(stream)), "jt_ray_shoot_noalloc")
     return beta_x, beta_y
+
+
+_CONV_PATHS = {0: "small", 1: "tile", 2: "fft"}
+
+
+def psf_convolve_plan(dtype, ny, nx, ky, kx, method="auto", B=1, image=None):
+    """jt_psf_convolve_plan: the launch path a convolution call with these arguments takes (host only).  Returns a dict:
+    method ("direct"/"fft"), path ("small"/"tile"/"fft"), tma, z_split, row_bands, oy, warps, pad_y, pad_x, est_us."""
+    p = _ConvPlan()
+    _check(lib().jt_psf_convolve_plan(_code(dtype), B, ny, nx, ky, kx, _METHODS[method], _ptr(image), ctypes.byref(p)),
+           "jt_psf_convolve_plan")
+    d = {n: getattr(p, n) for n, _ in _ConvPlan._fields_ if n != "reserved"}
+    d["method"] = "direct" if p.method == 1 else "fft"
+    d["path"] = _CONV_PATHS[p.path]
+    return d
+
+
+def trace_plan(dtype, grid=None, n_rays=0, n_tnfw=0):
+    """jt_trace_plan_query: launch shape of the ray-tracing kernel for jt_simulate_image (grid given) or jt_ray_shoot
+    (n_rays given).  Returns a dict: rays_per_thread, threads, wide, n_chunks, tile_recs, chunk_len, n_ctas."""
+    p = _TracePlan()
+    g = grid._c() if grid is not None else None
+    _check(lib().jt_trace_plan_query(_code(dtype), ctypes.byref(g) if g is not None else None, n_rays, n_tnfw, ctypes.byref(p)),
+           "jt_trace_plan_query")
+    return {n: getattr(p, n) for n, _ in _TracePlan._fields_ if n != "reserved"}
 
 
 @_on_stream

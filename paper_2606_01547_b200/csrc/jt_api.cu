@@ -145,6 +145,32 @@ static jt_status psf_convolve_impl(jt_dtype dtype, int64_t B, int32_t ny, int32_
     return conv_dispatch(dtype, B, ny, nx, image, ky, kx, kernel, method, workspace, out, (cudaStream_t)stream);
 }
 
+jt_status jt_psf_convolve_plan(jt_dtype dtype, int64_t B, int32_t ny, int32_t nx, int32_t ky, int32_t kx, jt_conv_method method,
+                               const void* image, jt_conv_plan* plan) {
+    if (!valid_dtype(dtype) || !valid_method(method)) return JT_ERR_UNSUPPORTED;
+    if (!plan || B < 1 || ny < 1 || nx < 1 || !valid_kernel_size(ky, kx)) return JT_ERR_INVALID_VALUE;
+    if (method == JT_CONV_DIRECT && !conv_direct_supported(dtype, ny, nx, ky, kx)) return JT_ERR_UNSUPPORTED;
+    const jt_conv_method m = resolve_conv_method(dtype, B, ny, nx, ky, kx, method);
+    if (m == JT_CONV_FFT && !conv_fft_supported(dtype, ny, nx, ky, kx)) return JT_ERR_UNSUPPORTED;
+    jt_conv_plan p = {};
+    if (m == JT_CONV_FFT) conv_fft_describe(dtype, B, ny, nx, ky, kx, &p);
+    else conv_direct_describe(dtype, B, ny, nx, ky, kx, image, &p);
+    *plan = p;
+    return JT_OK;
+}
+
+jt_status jt_trace_plan_query(jt_dtype dtype, const jt_grid* grid, int64_t n_rays, int64_t n_tnfw, jt_trace_plan* plan) {
+    if (!valid_dtype(dtype)) return JT_ERR_UNSUPPORTED;
+    if (!plan || n_tnfw < 0 || (grid ? !valid_grid(grid) : n_rays < 1)) return JT_ERR_INVALID_VALUE;
+    const TracePlan t = grid ? plan_trace_grid(dtype, grid, n_tnfw) : plan_trace_rays(dtype, n_rays, n_tnfw);
+    jt_trace_plan p = {};
+    p.rays_per_thread = t.R; p.threads = t.threads; p.wide = grid && t.wide ? 1 : 0;
+    p.n_chunks = t.n_chunks; p.chunk_len = t.chunk_len; p.n_ctas = t.n_tiles * t.n_chunks;
+    p.tile_recs = n_tnfw > 0 ? trace_tile_recs(dtype, t) : 0;
+    *plan = p;
+    return JT_OK;
+}
+
 jt_status jt_psf_convolve(jt_dtype dtype, int32_t ny, int32_t nx, const void* image, int32_t ky, int32_t kx,
                           const void* kernel, jt_conv_method method, void* workspace, size_t workspace_bytes, void* out,
                           void* stream) {

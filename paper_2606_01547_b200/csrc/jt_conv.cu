@@ -540,6 +540,25 @@ static bool make_tensor_map(CUtensorMap* map, const T* img, int64_t B, int ny, i
     return r == CUDA_SUCCESS;
 }
 
+// what launch_conv_direct would do for these arguments (jt_psf_convolve_plan); mirrors its decisions, enqueues nothing
+void conv_direct_describe(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx, const void* img, jt_conv_plan* out) {
+    SmallPlan sp;
+    out->method = JT_CONV_DIRECT;
+    if (use_small(d, B, ny, nx, ky, kx, &sp)) {
+        out->path = JT_PATH_CONV_SMALL;
+        out->z_split = 1; out->row_bands = 1; out->oy = kSmallOY; out->warps = kSmallNW;
+        out->est_us = sp.est_us;
+        return;
+    }
+    const ConvPlan p = plan_conv(d, B, ny, nx, ky, kx);
+    const size_t sz = dtype_size(d);
+    out->path = JT_PATH_CONV_TILE;
+    out->tma = !(((uintptr_t)img & 15) || ((size_t)nx * sz) % 16 || (B > 1 && ((size_t)nx * ny * sz) % 16) || p.tws > 256 ||
+                 p.ths > 256);                                   // make_tensor_map's conditions
+    out->z_split = p.Z; out->row_bands = p.launches; out->oy = p.OY; out->warps = p.NW;
+    out->est_us = p.est_us;
+}
+
 // The constant bank is one per device: calls on different streams take turns through an event (the library's only
 // cross-call state besides the error code; not used while the stream is being captured into a graph).
 static std::mutex g_const_mu;

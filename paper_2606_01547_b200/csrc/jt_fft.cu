@@ -396,6 +396,13 @@ static FftPlan plan_fft(int ny, int nx, int ky, int kx, int64_t B = 1) {
 }
 
 bool conv_fft_supported(jt_dtype, int ny, int nx, int ky, int kx) { return plan_fft(ny, nx, ky, kx).ok; }
+void conv_fft_describe(jt_dtype d, int64_t B, int ny, int nx, int ky, int kx, jt_conv_plan* out) {
+    const FftPlan p = plan_fft(ny, nx, ky, kx, B);
+    out->method = JT_CONV_FFT;
+    out->path = JT_PATH_CONV_FFT;
+    out->pad_y = p.a.Py; out->pad_x = p.a.Px;
+    out->est_us = conv_fft_estimate_us(d, B, ny, nx, ky, kx);
+}
 
 // A batch is transformed in groups of G images (all of it when its planes fit kFftGroupBytes of workspace).
 constexpr size_t kFftGroupBytes = (size_t)2 << 30;

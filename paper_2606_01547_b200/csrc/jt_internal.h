@@ -72,6 +72,7 @@ struct TracePlan {
 TracePlan plan_trace_grid(jt_dtype dtype, const jt_grid* g, int64_t n_tnfw);
 TracePlan plan_trace_rays(jt_dtype dtype, int64_t n_rays, int64_t n_tnfw);
 
+int       trace_tile_recs(jt_dtype dtype, const TracePlan& plan);
 jt_status launch_trace_grid(jt_dtype dtype, const jt_grid* g, const jt_lens* lens, const SrcSet& src,
                             const TracePlan& plan, void* workspace, void* pre_psf, bool count_tiers, cudaStream_t st);
 void*     trace_tier_counters(const TracePlan& plan, void* workspace);
@@ -88,6 +89,8 @@ double    conv_direct_estimate_us(jt_dtype dtype, int64_t B, int ny, int nx, int
 double    conv_fft_estimate_us(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
 jt_status launch_conv_direct(jt_dtype dtype, int64_t B, int ny, int nx, const void* img, int ky, int kx, const void* ker,
                              void* workspace, void* out, cudaStream_t st);   // B images [B][ny][nx], one kernel
+void      conv_direct_describe(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx, const void* img, jt_conv_plan* out);
+void      conv_fft_describe(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx, jt_conv_plan* out);
 bool      conv_fft_supported(jt_dtype dtype, int ny, int nx, int ky, int kx);
 size_t    fft_conv_workspace_bytes(jt_dtype dtype, int64_t B, int ny, int nx, int ky, int kx);
 jt_status launch_conv_fft(jt_dtype dtype, int64_t B, int ny, int nx, const void* img, int ky, int kx, const void* ker,

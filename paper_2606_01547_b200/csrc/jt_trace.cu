@@ -118,6 +118,10 @@ static int pick_tile_recs(int R, int64_t chunk_len) {
     return (int)(need < tr ? (need < 32 ? 32 : need) : tr);
 }
 
+int trace_tile_recs(jt_dtype dtype, const TracePlan& plan) {
+    return dtype == JT_F64 ? pick_tile_recs<double>(plan.R, plan.chunk_len) : pick_tile_recs<float>(plan.R, plan.chunk_len);
+}
+
 // Fills the lens part of the arguments and enqueues k_make_recs (derived records, zeroed counters).
 template <typename T>
 static jt_status fill_lens(TraceArgs<T>& a, const jt_lens* lens, const TracePlan& plan, void* workspace, bool count_tiers,

@@ -125,3 +125,28 @@ def test_noalloc_entry_point_limit_without_device(jt):
     assert L.jt_ray_shoot_noalloc(1, 0, None, None, ctypes.byref(lens), None, None, None) == 0                     # no-op
     lens.tnfw_Rs = None
     assert L.jt_ray_shoot_noalloc(1, 10, dummy[0], dummy[1], ctypes.byref(lens), dummy[2], dummy[3], None) == 1
+
+
+def test_plan_queries_without_device(jt):
+    """jt_psf_convolve_plan / jt_trace_plan_query are host-only: every launch shape the library has is reachable and named
+    (the GPU parity tests assert these same plans on the cases they run)."""
+    seen = set()
+    for dtype in ("f64", "f32"):
+        for shape in [(60, 60, 11, 11), (100, 100, 31, 31), (130, 75, 45, 45), (180, 180, 135, 135), (500, 500, 101, 101)]:
+            p = jt.psf_convolve_plan(dtype, *shape, method="direct")
+            seen.add((p["path"], p["tma"], p["z_split"] > 1, p["row_bands"] > 1))
+            assert jt.psf_convolve_plan(dtype, *shape, method="fft")["path"] == "fft"
+            assert jt.psf_convolve_plan(dtype, *shape, method="auto")["est_us"] <= p["est_us"] * (1 + 1e-12)
+        p = jt.psf_convolve_plan(dtype, 16, 20, 5, 5, method="direct", B=130)
+        seen.add((p["path"], p["tma"], p["z_split"] > 1, p["row_bands"] > 1))
+    assert {("small", 0, False, False), ("tile", 1, True, False), ("tile", 0, True, False), ("tile", 1, True, True),
+            ("tile", 1, False, False)} <= seen, seen
+    g = jt.Grid(200, 200, 0.04, supersample=2)
+    p = jt.trace_plan("f32", g, n_tnfw=10000)
+    assert p["n_chunks"] > 1 and p["n_ctas"] % p["n_chunks"] == 0 and p["chunk_len"] * p["n_chunks"] >= 10000
+    assert jt.trace_plan("f64", jt.Grid(500, 500, 0.02, supersample=5), n_tnfw=50000)["wide"] == 1
+    assert jt.trace_plan("f64", jt.Grid(60, 60, 0.05), n_tnfw=0)["rays_per_thread"] == 1
+    assert jt.trace_plan("f64", None, n_rays=1000, n_tnfw=0)["rays_per_thread"] == 8
+    L = jt.lib()
+    assert L.jt_psf_convolve_plan(0, 1, 8, 8, 4, 3, 0, None, None) == 1
+    assert L.jt_trace_plan_query(0, None, 0, 0, None) == 1

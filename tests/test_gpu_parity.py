@@ -29,10 +29,21 @@ def _f32r(a):
     return np.asarray(a, dtype=np.float64).astype(np.float32).astype(np.float64)
 
 
+def _trace_plan(jt, w):
+    """Launch shape of the ray-tracing kernel for a workloads.Workload (jt_trace_plan_query)."""
+    return jt.trace_plan(w.dtype, jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample), n_tnfw=w.n_tnfw)
+
+
 # ------------------------------------------------------------------ step 1: jt_ray_shoot
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("n,M", [(1, 0), (5000, 0), (4097, 1), (3001, 700), (20000, 513)])
+@pytest.mark.parametrize("n,M", [(1, 0), (5000, 0), (4097, 1), (3001, 700), (20000, 513), (20000, 10000)])
 def test_ray_shoot_random(jt, orc, dtype, n, M):
+    """Arbitrary ray positions (RAYS mode of k_trace); the last case is C2's subhalo count on 20,000 random rays."""
+    plan = jt.trace_plan(dtype, None, n_rays=n, n_tnfw=M)
+    assert plan["rays_per_thread"] == 8 and plan["wide"] == 0
+    assert (plan["n_chunks"] > 1) == (M >= 513), plan          # few ray tiles + many subhalos: the list is split over CTAs
+    if M == 10000:
+        assert plan["tile_recs"] >= 160 and plan["chunk_len"] > plan["tile_recs"]         # the record ring is refilled within a CTA
     rng = np.random.default_rng(100 + n + M)
     tx, ty = rng.uniform(-1.5, 1.5, n), rng.uniform(-1.5, 1.5, n)
     tn = _rand_lens(rng, M)
@@ -182,6 +193,20 @@ def test_source_brightness(jt, orc, dtype):
                                          (200, 200, 21, 21), (33, 31, 1, 1), (180, 180, 135, 135), (301, 203, 101, 7),
                                          (300, 420, 101, 101), (64, 1000, 3, 201), (70, 66, 151, 9)])
 def test_convolve_direct(jt, orc, dtype, ny, nx, ky, kx):
+    plan = jt.psf_convolve_plan(dtype, ny, nx, ky, kx, method="direct")
+    assert plan["method"] == "direct"
+    # every launch shape of the direct convolution is named by a case here (jt_psf_convolve_plan)
+    expect = {(8, 8, 3, 3): "small", (60, 60, 11, 11): "small", (37, 91, 7, 13): "small", (33, 31, 1, 1): "small",
+              (100, 100, 31, 31): "tile", (64, 64, 21, 21): "tile", (130, 75, 45, 45): "tile", (200, 200, 21, 21): "tile",
+              (180, 180, 135, 135): "tile", (300, 420, 101, 101): "tile"}
+    if (ny, nx, ky, kx) in expect:
+        assert plan["path"] == expect[(ny, nx, ky, kx)], plan
+    if (ny, nx, ky, kx) in ((100, 100, 31, 31), (64, 64, 21, 21), (200, 200, 21, 21)):
+        assert plan["tma"] == 1 and plan["z_split"] > 1 and plan["row_bands"] == 1, plan     # TMA tile, column pairs split (L2 reduction)
+    if (ny, nx, ky, kx) == (130, 75, 45, 45):
+        assert plan["tma"] == 0, plan                                    # 75-element rows: pitch not a multiple of 16 bytes -> plain loads
+    if (ny, nx, ky, kx) == (180, 180, 135, 135):
+        assert plan["row_bands"] > 1 and plan["tma"] == 1, plan          # taps exceed the 60 KB constant bank: bands of kernel rows
     rng = np.random.default_rng(ny * 1000 + nx + ky)
     img = rng.uniform(0, 1, (ny, nx))
     ker = rng.uniform(0, 1, (ky, kx))
@@ -199,6 +224,14 @@ def test_convolve_direct(jt, orc, dtype, ny, nx, ky, kx):
 def test_convolve_batch(jt, orc, dtype, B, ny, nx, k):
     """jt_psf_convolve_batch (B images, one kernel) = the oracle's convolution image by image, both methods;
     covers the TMA tile path (aligned pitch) and the plain-load fallback (33 x 47: odd pitch)."""
+    plan = jt.psf_convolve_plan(dtype, ny, nx, k, k, method="direct", B=B)
+    assert plan["path"] == "tile", plan                                  # the one-launch kernel is for single images only
+    assert plan["tma"] == (0 if (ny, nx) == (33, 47) else 1), plan
+    if B == 130:
+        assert plan["z_split"] == 1, plan                                # enough tiles: no split, no L2 reduction
+    if k == 135:
+        assert plan["row_bands"] > 1, plan
+    assert jt.psf_convolve_plan(dtype, ny, nx, k, k, method="fft", B=B)["path"] == "fft"
     rng = np.random.default_rng(B * 100 + k)
     imgs = rng.uniform(0, 1, (B, ny, nx))
     ker = rng.uniform(0, 1, (k, k))
@@ -216,10 +249,13 @@ def test_convolve_direct_unaligned_view(jt, orc):
     rng = np.random.default_rng(12)
     flat = to_dev(rng.uniform(0, 1, 64 * 64 + 1), "f32")
     img = flat[1:].view(64, 64)
-    ker = to_dev(rng.uniform(0, 1, (9, 9)) / 40.0, "f32")
+    ker = to_dev(rng.uniform(0, 1, (21, 21)) / 220.0, "f32")             # 21 x 21: the tile kernel (9 x 9 would take the one-launch path)
+    aligned = jt.psf_convolve_plan("f32", 64, 64, 21, 21, method="direct")
+    plan = jt.psf_convolve_plan("f32", 64, 64, 21, 21, method="direct", image=img)
+    assert aligned["path"] == plan["path"] == "tile" and aligned["tma"] == 1 and plan["tma"] == 0, (aligned, plan)
     got = jt.psf_convolve(img, ker, method="direct").double().cpu().numpy()
     want = orc.convolve(img.double().cpu().numpy(), ker.double().cpu().numpy())
-    assert rel_err(got, want) < 2e-6
+    assert rel_err(got, want) < max(2e-6, 3.0 * 21 * 2.0 ** -24)
 
 
 def test_convolve_delta_and_shift(jt):
@@ -309,23 +345,33 @@ def _check_image(jt, orc, w, method="auto", tol=None):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config_c0(jt, orc, dtype):
+    w = workloads.config_c0(dtype=dtype)
+    plan = _trace_plan(jt, w)
+    assert plan["rays_per_thread"] == w.supersample == 1 and plan["n_chunks"] == 1, plan      # latency shape: one pixel row per thread
+    assert jt.psf_convolve_plan(dtype, w.ny, w.nx, *w.psf.shape, method="direct")["path"] == "small"   # one-launch convolution
     _check_image(jt, orc, workloads.config_c0(dtype=dtype), method="direct")
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config_c1(jt, orc, dtype):
+    plan = _trace_plan(jt, workloads.config_c1(dtype=dtype))
+    assert plan["rays_per_thread"] == 3 and plan["wide"] == 1 and plan["n_chunks"] == 1, plan  # R = s row mode, CTA-wide tiles (s = 3)
     _check_image(jt, orc, workloads.config_c1(dtype=dtype), method="direct")
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config_c2_reduced(jt, orc, dtype):
     """C2's recipe at 48x48 pixels and 1,500 subhalos: several subhalo tiles plus a ragged tail, split list."""
+    plan = _trace_plan(jt, workloads.config_c2(nx=48, n_tnfw=1500, dtype=dtype))
+    assert plan["n_chunks"] > 1 and plan["wide"] == 0 and plan["rays_per_thread"] == 8, plan
     _check_image(jt, orc, workloads.config_c2(nx=48, n_tnfw=1500, dtype=dtype), method="direct")
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config_c4_reduced(jt, orc, dtype):
     """C4's recipe (s=5, 3 sources, AiryMix PSF) at 30x30 pixels, 700 subhalos, K=41."""
+    plan = _trace_plan(jt, workloads.config_c4(nx=30, n_tnfw=700, K=41, half_width=0.6, dtype=dtype))
+    assert plan["wide"] == 1 and plan["rays_per_thread"] == 10 and plan["n_chunks"] > 1, plan  # CTA-wide tiles AND a split list
     _check_image(jt, orc, workloads.config_c4(nx=30, n_tnfw=700, K=41, half_width=0.6, dtype=dtype), method="direct")
 
 
@@ -334,6 +380,7 @@ def test_supersampling_factors(jt, orc, s):
     """Every supported s: the warp-shuffle binning (definition B) with ragged tiles, off-centre, non-square grid."""
     w = workloads.config_c1(nx=23, supersample=s, K=9)
     w.ny, w.cx, w.cy = 17, 0.013, -0.021
+    assert _trace_plan(jt, w)["wide"] == (1 if 32 % s else 0)              # warp-shuffle binning vs CTA-wide shared-memory binning
     _check_image(jt, orc, w, method="direct")
 
 
@@ -442,6 +489,8 @@ def test_c2_full_size_whole_image(jt, orc, dtype):
     box's host cores).  Every warp tile of the grid -- centre, Einstein ring, edges -- takes part, so the
     position-dependent tier decisions (far-far / far / mid / cold) are all covered."""
     w = workloads.config_c2(dtype=dtype)
+    plan = _trace_plan(jt, w)
+    assert plan["n_chunks"] > 1 and plan["wide"] == 0 and plan["chunk_len"] > 4 * plan["tile_recs"], plan     # split list, long ring runs
     want_pre = orc.prepsf_rows(w, 0, w.ny)
     got_pre = gpu_simulate(jt, w, conv=False)
     assert rel_err(got_pre, want_pre) < TOL_IMG[dtype]
@@ -456,6 +505,11 @@ def test_c4_full_size_rows(jt, orc):
     with all 50,002 deflectors (1.25e10 evaluations, SURVEY.md section 8(d) C4 plan); (2) both convolution methods on
     the FULL image: the oracle's direct convolution of the GPU's pre-PSF image against the GPU's convolved images."""
     w = workloads.config_c4(dtype="f64")
+    plan = _trace_plan(jt, w)
+    assert plan["wide"] == 1 and plan["rays_per_thread"] == 10 and plan["n_chunks"] == 1 and plan["n_ctas"] == 5000, plan
+    cp = jt.psf_convolve_plan("f64", w.ny, w.nx, *w.psf.shape, method="direct")
+    assert cp["path"] == "tile" and cp["row_bands"] > 1 and cp["z_split"] > 1, cp
+    assert jt.psf_convolve_plan("f64", w.ny, w.nx, *w.psf.shape, method="auto")["path"] == "fft"
     pre = gpu_simulate(jt, w, conv=False)
     scale = np.max(np.abs(pre))
     for j in np.linspace(0, w.ny - 1, 20).astype(int):
