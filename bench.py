@@ -42,7 +42,9 @@ SM_COUNT = 148
 # FMUL2 / FADD2 counts as two: it holds the pipe for two cycles); f64: FP64-pipe instructions.  Order: far-far series at
 # its three lengths (longest first), far form, near form on a warp tile outside / inside X^2 = 2 (both run the mid form
 # on every ray; the per-ray generic fix-up inside is not counted).  The mix of classes is measured per run with
-# jt_profile_tiers.
+# jt_profile_tiers.  tests/test_roofline_numerator.py recounts the far-far and near entries from the built library's SASS
+# on every CPU test run, so they cannot go stale; the far entry (29.6 / 50.6) is a count of the source (the form is inlined,
+# it has no loop of its own) and weighs 3-7 % of the evaluations.
 TIER_COST = {"f32": (13.25, 10.25, 9.25, 29.6, 36.0, 36.0), "f64": (23.25, 19.25, 17.25, 50.6, 77.0, 77.0)}
 TIER_NAMES = ("far_far_long", "far_far_mid", "far_far_short", "far", "mid", "cold")
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu --set full captures in

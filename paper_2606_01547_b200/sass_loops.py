@@ -47,6 +47,46 @@ def opcode(text):
     return t.split()[0].split(".")[0]
 
 
+_DUMP = {}
+
+
+def loop_table(kernel, lib=None):
+    """[(n_instructions, n_inner_loops, opcode Counter), ...] for every loop of the ONE kernel whose demangled name contains
+    `kernel`, innermost first.  The SASS dump of a library is cached per path (cuobjdump takes half a minute on libjt.so).
+    tests/test_roofline_numerator.py checks bench.py's TIER_COST against this."""
+    lib = lib or os.path.join(HERE, "libjt.so")
+    if lib not in _DUMP:
+        ks = kernels(lib)
+        _DUMP[lib] = (ks, demangle(list(ks)))
+    ks, dm = _DUMP[lib]
+    hits = [n for n in ks if kernel in dm[n]]
+    if len(hits) != 1:
+        raise LookupError("kernel substring %r matches %d functions" % (kernel, len(hits)))
+    body = ks[hits[0]]
+    index = {a: i for i, (a, _) in enumerate(body)}
+    loops = []
+    for i, (a, t) in enumerate(body):
+        m = re.search(r"\bBRA(?:\.U)?\b.*\b0x([0-9a-f]+)", t)
+        if m:
+            tgt = int(m.group(1), 16)
+            if tgt <= a and tgt in index:
+                loops.append((index[tgt], i))
+    loops.sort(key=lambda l: l[1] - l[0])
+    out = []
+    for lo, hi in loops:
+        inner = [l for l in loops if l != (lo, hi) and lo <= l[0] and l[1] <= hi]
+        out.append((hi - lo + 1, len(inner), collections.Counter(opcode(t) for _, t in body[lo:hi + 1])))
+    return out
+
+
+def fp64_ops(hist):
+    return sum(hist[o] for o in FP64)
+
+
+def fp32_lane_ops(hist):
+    return sum(hist[o] * (2 if o.endswith("2") else 1) for o in FP32)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("kernel")
