@@ -709,6 +709,69 @@ def run_swarm(args, rank):
           flush=True)
 
 
+def run_next(args, rank):
+    """--next: the paper's own per-profile benchmark (tables "Deflection angle calculations" and "Flux
+    calculations": ONE deflection / flux call per profile on a 60 x 60 and a 180 x 180 grid) through the SURVEY 8(f) entry
+    points, plus jt_lensing_maps on C2's lens.  Device time per call from a CUDA-graph replay (no Python / ctypes cost in
+    the number).  Stated bound: at 3,600 / 32,400 points these calls are launch-latency-bound (one launch of one-point-per-
+    thread double-precision code, ~2-4 us whatever the profile, 15 - 127 thread blocks on 148 SMs); the rate column is what
+    it is, no roofline fraction is claimed for them.  The paper's table gives speed-up RATIOS over lenstronomy on other
+    hardware, no absolute times: context only."""
+    if rank != 0:
+        return
+    import torch
+    import paper_2606_01547_b200 as jt
+    from paper_2606_01547_b200 import binding as b
+    import workloads
+    torch.cuda.set_device(0)
+    jt.lib()
+    defl = [("CONVERGENCE", [0.1, 0.0, 0.0]), ("SIS", [1.0, 0.01, -0.02]), ("NFW", [0.3, 0.2, -0.1, 0.1]),
+            ("HERNQUIST", [0.4, 0.5, 0.1, 0.0]), ("PJAFFE", [0.5, 0.1, 0.6, 0.0, 0.1]), ("SIE", [1.0, 0.1, -0.05, 0.0, 0.0]),
+            ("SHEAR", [0.03, 0.01]), ("TNFW", [0.2, 0.1, 1.0, 0.8, 0.3]), ("NIE", [1.1, 0.2, -0.1, 0.15, 0.3, -0.1]),
+            ("EPL", [1.0, 2.3, 0.15, 0.1, -0.2, 0.3]), ("MULTIPOLE", [3.0, 0.04, 0.2, -0.2, 0.3]),
+            ("CSE", [0.05, 0.2, 0.3, -0.15, 0.5, 0.5]), ("PJAFFE_ELLIPSE_POTENTIAL", [0.5, 0.1, 0.6, 0.2, -0.1, 0.0, 0.1])]
+    light = [("SERSIC_ELLIPSE", [10.0, 0.2, 1.5, 0.05, 0.02, 0.05, 0.0]), ("GAUSSIAN_ELLIPSE", [1.0, 0.2, 0.2, -0.1, 0.05, 0.0])]
+    rows = []
+    for dtype, tdt in (("f64", torch.float64), ("f32", torch.float32)):
+        for n in (60, 180):
+            u = (np.arange(n) - (n - 1) / 2) * 0.05
+            x = torch.as_tensor(np.repeat(u[None, :], n, 0).reshape(-1).copy(), dtype=tdt, device="cuda")
+            y = torch.as_tensor(np.repeat(u[:, None], n, 1).reshape(-1).copy(), dtype=tdt, device="cuda")
+            calls = []
+            for name, p in defl:
+                rec = b.profile_records([(name, p)], b.DEFLECTOR_TYPES)
+                calls.append(("deflection", name, lambda rec=rec: jt.ray_shoot_profiles(x, y, rec)))
+            for name, p in light:
+                rec = b.profile_records([(name, p)], b.LIGHT_TYPES)
+                calls.append(("flux", name, lambda rec=rec: jt.light_profiles(x, y, rec)))
+            mg = b.profile_records([("GAUSSIAN_ELLIPSE", [1.0, 0.05 * 2 ** k, 0.2, -0.1, 0.05, 0.0]) for k in range(5)], b.LIGHT_TYPES)
+            calls.append(("flux", "MULTI_GAUSSIAN_ELLIPSE(5)", lambda: jt.light_profiles(x, y, mg)))
+            calls.append(("flux", "CORE_SERSIC", lambda: jt.light_core_sersic(x, y, [10.0, 0.3, 2.0, 0.05, 0.2, 2.0, 0.1, -0.05, 0.0, 0.0])))
+            for n_max in (6, 10):
+                coef = torch.as_tensor(np.random.default_rng(n_max).normal(size=(n_max + 1) * (n_max + 2) // 2), dtype=tdt, device="cuda")
+                calls.append(("flux", "SHAPELETS(n_max=%d)" % n_max,
+                              lambda n_max=n_max, coef=coef: jt.light_shapelets(x, y, n_max, 0.3, 0.0, 0.0, coef)))
+            for kind, name, call in calls:
+                us = graph_time(torch, call)
+                rows.append({"kind": kind, "profile": name, "dtype": dtype, "grid": "%dx%d" % (n, n), "us_per_call": us,
+                             "points_per_s": n * n / (us * 1e-6)})
+        # NEXT-2: kappa, gamma1, gamma2, mu of C2's lens (SIE + shear + 10,000 TNFW) on C2's 160,000 ray positions
+        w = workloads.config_c2(dtype=dtype)
+        m = w.nx * w.supersample
+        u = (np.arange(m) - (m - 1) / 2) * (w.pixel_scale / w.supersample)
+        x = torch.as_tensor(np.repeat(u[None, :], m, 0).reshape(-1).copy(), dtype=tdt, device="cuda")
+        y = torch.as_tensor(np.repeat(u[:, None], m, 1).reshape(-1).copy(), dtype=tdt, device="cuda")
+        tn = torch.as_tensor(np.ascontiguousarray(w.tnfw), dtype=tdt, device="cuda")
+        us = graph_time(torch, lambda: jt.lensing_maps(x, y, w.sie, w.shear, tn), n_rep=3)
+        rows.append({"kind": "lensing_maps", "profile": "SIE+SHEAR+10000 TNFW (C2)", "dtype": dtype, "grid": "400x400 rays",
+                     "us_per_call": us, "point_deflector_evals_per_s": m * m * (w.n_tnfw + 2) / (us * 1e-6),
+                     "bound": "alu (double-precision libdevice code in both dtype modes; correct-first, not tier-tuned)"})
+    print(json.dumps({"metric": "next_profile_call_us", "unit": "us per call (CUDA-graph replay)", "n_gpus": 1,
+                      "data": "synthetic", "bound": "launch latency at 60^2 / 180^2 points (see docstring)", "rows": rows,
+                      "paper_context": "PAPER.md:59-108 lists speed-up ratios over lenstronomy per profile, no absolute times"}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -724,6 +787,7 @@ def main():
     ap.add_argument("--conv-sweep", action="store_true", help="time jt_psf_convolve alone at the paper's shapes")
     ap.add_argument("--sweep-batch", type=int, default=1024, help="batch size of the batched rows of --conv-sweep")
     ap.add_argument("--swarm", action="store_true", help="time the particle-swarm inner loop (NEXT-3) at the paper's sizes")
+    ap.add_argument("--next", action="store_true", help="time one call per SURVEY 8(f) profile on 60^2 / 180^2 grids + jt_lensing_maps")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank, world, local_rank = dist_init(args.gpus)
@@ -732,6 +796,8 @@ def main():
             run_conv_sweep(args, rank)
         elif args.swarm:
             run_swarm(args, rank)
+        elif args.next:
+            run_next(args, rank)
         elif args.impl == "reference":
             run_reference(args, rank, world)
         else:

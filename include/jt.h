@@ -19,7 +19,9 @@
  *     State it keeps between calls, all of it listed here: per host thread the last CUDA error code, the
  *     launch counter and -- only while jt_profile_enable(1) is in force -- four CUDA events and a 48-byte
  *     pinned host buffer; per process one 60 KB __constant__ buffer per device (the taps of the direct
- *     convolution) with the event that orders its users (see jt_psf_convolve).
+ *     convolution) with the event that orders its users (see jt_psf_convolve), the 32 MiB scratch array of
+ *     jt_ray_shoot_noalloc per device, one bit per kernel and device ("shared-memory attribute set") and, per host
+ *     thread, the last four convolution plans.
  *   - "device [n]" = pointer to device memory holding n elements of the call's dtype
  *     (float for JT_F32, double for JT_F64), aligned to the element size.  "host" = ordinary
  *     host memory.  Arrays are row-major, x (column) fastest.
