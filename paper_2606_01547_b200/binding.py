@@ -465,6 +465,46 @@ def simulate_image(grid, sie, shear, tnfw, sources, psf, dtype=None, method="aut
     return out
 
 
+class PreparedImage:
+    """jt_simulate_image with the argument marshalling done ONCE: the C structs, the workspace, the output tensor and the
+    stream handle are built at construction, and each call is a single ctypes call (PAPER.md:89 is about exactly this
+    per-call overhead; C0 spends 10 us on the device and several times that in marshalling through simulate_image()).
+    Marshalling only: every step still runs in libjt's kernels.  The tensors passed in (tnfw, psf) are referenced, not
+    copied: updating them IN PLACE between calls is how a caller changes subhalos or PSF; SIE / shear / sources are
+    frozen (build another PreparedImage to change them).  Calls go to the stream given here (default: the stream current
+    at construction); the returned tensor is the same `out` every time."""
+
+    def __init__(self, grid, sie, shear, tnfw, sources, psf, dtype=None, method="auto", workspace=None, out=None, stream=None,
+                 device="cuda"):
+        code = _code(dtype) if dtype is not None else (_dt(psf) if psf is not None else _dt(tnfw))
+        self._g = grid._c()
+        self._L = _lens(code, sie, shear, tnfw)
+        self._S, self._keep = _sources(sources)
+        ky, kx = (0, 0) if psf is None else psf.shape
+        if psf is not None:
+            _dev(psf, "psf")
+            if _dt(psf) != code:
+                raise TypeError("psf dtype differs from the call's dtype")
+            device = psf.device
+        elif tnfw is not None:
+            device = tnfw.device
+        self._stream = torch.cuda.current_stream(device) if stream is None else stream
+        with torch.cuda.stream(self._stream):
+            self._ws, wsb = _workspace(simulate_image_workspace_bytes(code, grid, self._L.n_tnfw, ky, kx, method), device, workspace)
+            self.out = out if out is not None else torch.empty((grid.ny, grid.nx), dtype=_torch_dtype(code), device=device)
+        self._tensors = (tnfw, psf)                                    # keep the referenced device memory alive
+        fn = lib().jt_simulate_image
+        args = (code, ctypes.byref(self._g), ctypes.byref(self._L), ctypes.byref(self._S), ky, kx, _ptr(psf), _METHODS[method],
+                _ptr(self._ws), wsb, _ptr(self.out), ctypes.c_void_p(self._stream.cuda_stream))
+        self._call = functools.partial(fn, *args)
+
+    def __call__(self):
+        status = self._call()
+        if status != 0:
+            raise JtError(status, "jt_simulate_image")
+        return self.out
+
+
 def _batch_struct(sie, shear, tnfw, sersic, psf):
     _dev(sie, "sie"), _dev(shear, "shear")
     code = _dt(sie)

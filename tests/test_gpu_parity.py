@@ -624,3 +624,21 @@ def test_second_device_in_one_process(jt, orc):
                 assert rel_err(gpu_simulate(jt, w, method=method), want) < TOL_IMG["f64"], (dev, method)
             got_b = _gpu_batch(jt, bw)
             assert max(rel_err(got_b[b], want_b[b]) for b in range(bw.B)) < TOL_IMG["f32"], dev
+
+
+def test_prepared_image_equals_simulate_image(jt):
+    """binding.PreparedImage (marshalling done once, one ctypes call per image) returns bit for bit what simulate_image
+    returns, call after call, and sees in-place updates of the subhalo tensor."""
+    import torch
+    for w in (workloads.config_c0(), workloads.config_c1(), workloads.config_c2(nx=48, n_tnfw=1500, dtype="f32")):
+        g = jt.Grid(w.nx, w.ny, w.pixel_scale, w.cx, w.cy, w.supersample)
+        tn = to_dev(w.tnfw, w.dtype) if w.n_tnfw > 0 else None
+        psf = to_dev(w.psf, w.dtype)
+        want = jt.simulate_image(g, w.sie, w.shear, tn, w.sources, psf, dtype=w.dtype)
+        prep = jt.PreparedImage(g, w.sie, w.shear, tn, w.sources, psf, dtype=w.dtype)
+        for _ in range(3):
+            assert torch.equal(prep(), want)
+        if tn is not None:
+            tn[3] *= 2.0                                   # alpha_Rs doubled in place
+            want2 = jt.simulate_image(g, w.sie, w.shear, tn, w.sources, psf, dtype=w.dtype)
+            assert torch.equal(prep(), want2) and not torch.equal(want2, want)
